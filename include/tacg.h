@@ -1,0 +1,167 @@
+/* tacg.h -- C ABI of libtacg: the data-parallel hot path behind TACG/GESR expert
+ * placement (arxiv/paper_2606_01007), hand-written CUDA for sm_100a (B200).
+ *
+ * Citations are PAPER.md:<line> (the paper text) and SURVEY.md section 8; the
+ * readings Q1..Q28 taken where the paper is silent are listed in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *   - Every pointer marked "dev" is DEVICE memory owned and allocated by the
+ *     caller (e.g. a torch tensor's data_ptr()); the library never frees it and
+ *     keeps no pointer after the call returns.  Scalars are passed by value.
+ *   - Calls enqueue work on the ctx stream and return; outputs are valid after
+ *     the caller synchronises that stream.  TACG_VALIDATE forces one
+ *     synchronisation because it reads back an error word.
+ *   - Return value: TACG_OK (0) or a negative tacg_status.  No error other than
+ *     TACG_ERR_CUDA leaves an output partially written: shape / NULL errors are
+ *     detected on the host before any launch.
+ *   - Layouts are dense row-major with the last index fastest.
+ *   - Limits: 1 <= k <= 16, 1 <= E <= 512, 1 <= P <= 64, 1 <= F <= 8,
+ *     0 <= r <= 8, L >= 1, N >= 0.  Counts are uint32 (one C entry overflows
+ *     only after 2^32 co-occurrences; documented, not checked).
+ *   - Preconditions when not validating: the expert ids of one token are
+ *     distinct (top-k without replacement).  A negative expert
+ *     id is an empty slot (skipped); a negative family is a padding token
+ *     (skipped).  Behaviour on duplicate ids is undefined without TACG_VALIDATE.
+ *
+ * There is no CPU fallback anywhere in this library: a call on a machine
+ * without an sm_100 device fails with TACG_ERR_ARCH / TACG_ERR_CUDA.
+ */
+#ifndef TACG_H_
+#define TACG_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum tacg_status {
+    TACG_OK = 0,
+    TACG_ERR_NULL = -1,      /* a required pointer is NULL */
+    TACG_ERR_SHAPE = -2,     /* a size is outside the limits above, or E > P*capacity */
+    TACG_ERR_BAD_INDEX = -3, /* TACG_VALIDATE only: expert id >= E, duplicate id in a token, family >= F */
+    TACG_ERR_PLACEMENT = -4, /* TACG_VALIDATE only: primary outside [0,P), partition over capacity,
+                                replica outside [-1,P), equal to the primary or duplicated */
+    TACG_ERR_CUDA = -5,      /* a CUDA runtime call failed; text via tacg_last_detail */
+    TACG_ERR_ARCH = -6       /* the device is not compute capability 10.x */
+} tacg_status;
+
+/* flags of tacg_coact_accumulate */
+#define TACG_ZERO_FIRST 0x1u /* zero D, C and ntok on the stream before accumulating */
+#define TACG_VALIDATE   0x2u /* check indices / family (coact) or primary / replicas (eval, select) on device */
+#define TACG_PATH_AUTO  0x00u /* pick the co-activation kernel by shape */
+#define TACG_PATH_HIST  0x10u /* force the shared-memory / global atomic histogram kernel */
+#define TACG_PATH_MMA   0x20u /* force the tcgen05 kind::i8 X^T X kernel; TACG_ERR_SHAPE if the shape is unsupported */
+#define TACG_PATH_MASK  0x30u
+
+typedef struct tacg_ctx tacg_ctx; /* opaque: device id, stream, scratch buffers, last error text */
+
+/* Create a context on `device` bound to `cuda_stream` (a cudaStream_t, or NULL for
+ * the legacy default stream).  Fails with TACG_ERR_ARCH unless the device is sm_100. */
+int tacg_create(tacg_ctx** out, int device, void* cuda_stream);
+int tacg_destroy(tacg_ctx* ctx);
+/* Static description of a status code; never freed. */
+const char* tacg_strerror(int code);
+/* Copies the detail text of the last failing call on ctx (cudaGetErrorString text,
+ * or "layer l token t ..." for validation) into buf (NUL-terminated, at most n bytes). */
+int tacg_last_detail(tacg_ctx* ctx, char* buf, size_t n);
+/* Which co-activation kernel the last tacg_coact_accumulate on ctx ran:
+ * TACG_PATH_HIST or TACG_PATH_MMA (0 before the first call). */
+int tacg_last_path(tacg_ctx* ctx);
+/* Number of kernel launches the library has enqueued on ctx since creation. */
+int64_t tacg_launch_count(tacg_ctx* ctx);
+/* Library version, "major.minor". */
+const char* tacg_version(void);
+
+/* S1+S2 -- per-family usage and co-activation counts
+ * ("usage vector u ... coactivation matrix A ... frequency of expert pairs selected
+ * by the same token", per layer and task family).
+ *   for every layer l, token t with f = family[t] >= 0, expert set T = {indices[l,t,*] >= 0}:
+ *     D[l,f,e] += 1 for e in T;  C[l,f,i,j] += 1 and C[l,f,j,i] += 1 for every unordered
+ *     pair {i,j} of T;  C[l,f,e,e] is never touched;  ntok[f] += 1 once per token.
+ * All three outputs ACCUMULATE (+=) so a long trace can be streamed in chunks;
+ * TACG_ZERO_FIRST clears them first.  Integer results, bit-exact. */
+int tacg_coact_accumulate(tacg_ctx* ctx,
+                          const int16_t* indices, /* dev [L,N,k] expert ids of each token, per layer */
+                          const int8_t* family,   /* dev [N] task family of each token, shared by all layers */
+                          int64_t N, int k, int L, int E, int F,
+                          uint32_t* D,            /* dev [L,F,E]   in/out */
+                          uint32_t* C,            /* dev [L,F,E,E] in/out, symmetric, zero diagonal */
+                          uint64_t* ntok,         /* dev [F]       in/out tokens per family */
+                          uint32_t flags);
+
+/* S3..S7 -- preferences (Eq. 2-6), task-modulated graph W = A-tilde
+ * (Eq. 7-8), expert->partition affinity (inner sum of Eq. 10,
+ * PAPER.md:121) and all-pairs swap gains (the "only if it improves" quantity of
+ * PAPER.md:124 for every pair, north_star):
+ *   u = D/sum_e D;  A^f = C^f/max(1,ntok[f]);  c = rowsum|A^f|;  dx = x^f - mean_{f'!=f} x^f';
+ *   z = (dx-mu)/(sigma+eps) over experts (population sigma);  s = z(du)+z(dc);
+ *   pref[e,:] = softmax_f(s/tau);  Abar = mean_f A^f;  Ahat = Abar/max Abar;
+ *   W = (1-alpha) Ahat + alpha (pref pref^T) .* Ahat;  aff[e,m] = sum_{e': primary[e']=m} W[e,e'];
+ *   gain[i,j] = aff[i,b]+aff[j,a]-aff[i,a]-aff[j,b]-2W[i,j] (a=primary[i] != b=primary[j]), else 0.
+ * Computed in fp64 on device, stored as fp32.  Any output pointer may be NULL
+ * (skipped).  primary may be NULL when aff and gain are NULL.  P and capacity are
+ * checked (E <= P*capacity) when primary is given. */
+int tacg_affinity_swapgain(tacg_ctx* ctx,
+                           const uint32_t* D,    /* dev [L,F,E] */
+                           const uint32_t* C,    /* dev [L,F,E,E] */
+                           const uint64_t* ntok, /* dev [F] */
+                           int L, int E, int F, int P, int capacity,
+                           const int8_t* primary, /* dev [L,E] partition of each expert, or NULL */
+                           float alpha, float tau, float eps,
+                           float* pref,           /* dev [L,E,F] or NULL */
+                           float* W,              /* dev [L,E,E] or NULL */
+                           float* aff,            /* dev [L,E,P] or NULL */
+                           float* gain);          /* dev [L,E,E] or NULL */
+
+/* S8 -- GESR serving selection for ONE given load snapshot (Eq. 13-14 and the
+ * fallback; pick rule Q17/Q18 of DESIGN.md):
+ *   feas[m] = S[m] <= (1+theta) * mean(S);  experts without replicas are served by their
+ *   primary (pass 1, they form the accessed set R);  each replicated expert, in slot order,
+ *   picks among its feasible candidates (all candidates if none is feasible) the one
+ *   minimising (not in R u {home}, S[c], candidate slot), and joins R.
+ *   home = (token_offset + t) mod P.   serve[l,t,j] = -1 for an empty slot.
+ * replicas may be NULL (or r = 0): serve = primary[indices]. */
+int gesr_select(tacg_ctx* ctx,
+                const int16_t* indices, /* dev [L,N,k] */
+                int64_t N, int k, int L, int E, int P,
+                const int8_t* primary,  /* dev [L,E] */
+                const int8_t* replicas, /* dev [L,E,r], -1 = none; or NULL */
+                int r,
+                const double* load_snapshot, /* dev [L,P] */
+                float theta, int64_t token_offset,
+                int8_t* serve,          /* dev [L,N,k] out */
+                uint32_t flags);        /* 0 or TACG_VALIDATE */
+
+/* S8..S12 -- score a placement over a held-out trace (Eq. 13-15,
+ * Comm per PAPER.md:363, Jain/MaxVio Eq. 17-18).  Tokens are processed
+ * in micro-batches of `microbatch` consecutive tokens; every token of a micro-batch sees
+ * the load state left by the previous micro-batch (north_star), then
+ * state[m] = rho*state[m] + delta[m] (one rounded multiply, one rounded add, double).
+ * With replicas == NULL or r == 0 the result does not depend on microbatch/theta/rho.
+ * Outputs are OVERWRITTEN.  Integer outputs are bit-exact; fairness is computed in
+ * fp64 and stored as fp32. */
+int tacg_eval_placement(tacg_ctx* ctx,
+                        const int16_t* indices, /* dev [L,N,k] */
+                        const int8_t* family,   /* dev [N] */
+                        int64_t N, int k, int L, int E, int F, int P,
+                        const int8_t* primary,  /* dev [L,E] */
+                        const int8_t* replicas, /* dev [L,E,r] or NULL */
+                        int r, float theta, double rho,
+                        int64_t microbatch,     /* B tokens; <= 0 or no replicas: one batch */
+                        int64_t token_offset,   /* home = (token_offset + t) mod P */
+                        double* load_state,     /* dev [L,P] in/out EMA state; NULL = start from 0, discard */
+                        uint64_t* load,         /* dev [L,P] out dispatches served per partition */
+                        uint64_t* comm_span,    /* dev [L,F] out sum over tokens of max(0,|cards|-1) */
+                        uint64_t* comm_remote,  /* dev [L,F] out sum over tokens of |cards \ {home}| */
+                        uint64_t* ntok,         /* dev [F]   out tokens per family */
+                        float* fairness,        /* dev [L+1,3] out (jain, maxvio, cv); row L = loads summed over layers */
+                        uint8_t* cost_per_token,/* dev [L,N] out |cards \ {home}| per token, or NULL */
+                        int8_t* serve,          /* dev [L,N,k] out serving partition per slot, or NULL */
+                        uint32_t flags);        /* 0 or TACG_VALIDATE */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TACG_H_ */

@@ -1,0 +1,247 @@
+"""ctypes binding of libtacg.so: same names as include/tacg.h, marshalling only.
+
+Every function takes torch CUDA tensors (or None) and passes their data_ptr() through;
+shapes and dtypes are checked here, every step of the path runs in the library's kernels.
+The convenience wrappers allocate the output tensors (device memory is torch's job) and
+return them in a dict.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtacg.so")
+
+TACG_ZERO_FIRST = 0x1
+TACG_VALIDATE = 0x2
+TACG_PATH_AUTO = 0x00
+TACG_PATH_HIST = 0x10
+TACG_PATH_MMA = 0x20
+
+EXPORTS = (
+    "tacg_create", "tacg_destroy", "tacg_strerror", "tacg_last_detail", "tacg_last_path",
+    "tacg_launch_count", "tacg_version", "tacg_coact_accumulate", "tacg_affinity_swapgain",
+    "gesr_select", "tacg_eval_placement",
+)
+
+_lib = None
+
+
+class TacgError(RuntimeError):
+    def __init__(self, code: int, where: str, detail: str = ""):
+        self.code = code
+        msg = f"{where}: {lib().tacg_strerror(code).decode()} ({code})"
+        if detail:
+            msg += f" -- {detail}"
+        super().__init__(msg)
+
+
+def lib_path() -> str:
+    return _SO
+
+
+def lib():
+    """Loads libtacg.so (built by paper_2606_01007_b200.build / __graft_entry__.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise FileNotFoundError(
+                f"{_SO} is missing: run `python -m paper_2606_01007_b200.build` (there is no CPU fallback)")
+        L = C.CDLL(_SO)
+        vp, i32, i64, u32, f32, f64 = C.c_void_p, C.c_int, C.c_int64, C.c_uint32, C.c_float, C.c_double
+        L.tacg_create.argtypes = [C.POINTER(vp), i32, vp]
+        L.tacg_destroy.argtypes = [vp]
+        L.tacg_strerror.argtypes = [i32]
+        L.tacg_strerror.restype = C.c_char_p
+        L.tacg_last_detail.argtypes = [vp, C.c_char_p, C.c_size_t]
+        L.tacg_last_path.argtypes = [vp]
+        L.tacg_launch_count.argtypes = [vp]
+        L.tacg_launch_count.restype = i64
+        L.tacg_version.restype = C.c_char_p
+        L.tacg_coact_accumulate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp, u32]
+        L.tacg_affinity_swapgain.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, f32, f32, f32,
+                                             vp, vp, vp, vp]
+        L.gesr_select.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp, vp, i32, vp, f32, i64, vp, u32]
+        L.tacg_eval_placement.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, i32, vp, vp, i32, f32, f64,
+                                          i64, i64, vp, vp, vp, vp, vp, vp, vp, vp, u32]
+        for name in EXPORTS:
+            getattr(L, name)
+        _lib = L
+    return _lib
+
+
+def version() -> str:
+    return lib().tacg_version().decode()
+
+
+def _ptr(t: Optional[torch.Tensor], dtype=None, name="tensor"):
+    if t is None:
+        return None
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (the library has no CPU path)")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"{name} must be {dtype}, got {t.dtype}")
+    return C.c_void_p(t.data_ptr())
+
+
+class Context:
+    """tacg_ctx bound to a device and a torch stream (default: the current stream)."""
+
+    def __init__(self, device: int = 0, stream: Optional[torch.cuda.Stream] = None):
+        self._h = C.c_void_p()
+        self.device = int(device)
+        if stream is None and torch.cuda.is_available():
+            stream = torch.cuda.current_stream(self.device)
+        self.stream = stream
+        sp = C.c_void_p(stream.cuda_stream) if stream is not None else None
+        rc = lib().tacg_create(C.byref(self._h), self.device, sp)
+        if rc != 0:
+            self._h = C.c_void_p()
+            raise TacgError(rc, "tacg_create")
+
+    def close(self):
+        if self._h:
+            lib().tacg_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def detail(self) -> str:
+        buf = C.create_string_buffer(256)
+        lib().tacg_last_detail(self._h, buf, 256)
+        return buf.value.decode(errors="replace")
+
+    def last_path(self) -> int:
+        return int(lib().tacg_last_path(self._h))
+
+    def launch_count(self) -> int:
+        return int(lib().tacg_launch_count(self._h))
+
+    def check(self, rc: int, where: str):
+        if rc != 0:
+            raise TacgError(rc, where, self.detail())
+
+    # ---- raw calls: same names and argument order as include/tacg.h ----
+    def tacg_coact_accumulate(self, indices, family, N, k, L, E, F, D, Cm, ntok, flags=0) -> int:
+        return lib().tacg_coact_accumulate(
+            self._h, _ptr(indices, torch.int16, "indices"), _ptr(family, torch.int8, "family"),
+            int(N), int(k), int(L), int(E), int(F), _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"),
+            _ptr(ntok, torch.int64, "ntok"), int(flags))
+
+    def tacg_affinity_swapgain(self, D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps,
+                               pref, W, aff, gain) -> int:
+        return lib().tacg_affinity_swapgain(
+            self._h, _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"), _ptr(ntok, torch.int64, "ntok"),
+            int(L), int(E), int(F), int(P), int(capacity), _ptr(primary, torch.int8, "primary"),
+            float(alpha), float(tau), float(eps), _ptr(pref, torch.float32, "pref"),
+            _ptr(W, torch.float32, "W"), _ptr(aff, torch.float32, "aff"), _ptr(gain, torch.float32, "gain"))
+
+    def gesr_select(self, indices, N, k, L, E, P, primary, replicas, r, load_snapshot, theta,
+                    token_offset, serve, flags=0) -> int:
+        return lib().gesr_select(
+            self._h, _ptr(indices, torch.int16, "indices"), int(N), int(k), int(L), int(E), int(P),
+            _ptr(primary, torch.int8, "primary"), _ptr(replicas, torch.int8, "replicas"), int(r),
+            _ptr(load_snapshot, torch.float64, "load_snapshot"), float(theta), int(token_offset),
+            _ptr(serve, torch.int8, "serve"), int(flags))
+
+    def tacg_eval_placement(self, indices, family, N, k, L, E, F, P, primary, replicas, r, theta, rho,
+                            microbatch, token_offset, load_state, load, comm_span, comm_remote, ntok,
+                            fairness, cost_per_token, serve, flags=0) -> int:
+        return lib().tacg_eval_placement(
+            self._h, _ptr(indices, torch.int16, "indices"), _ptr(family, torch.int8, "family"),
+            int(N), int(k), int(L), int(E), int(F), int(P), _ptr(primary, torch.int8, "primary"),
+            _ptr(replicas, torch.int8, "replicas"), int(r), float(theta), float(rho), int(microbatch),
+            int(token_offset), _ptr(load_state, torch.float64, "load_state"),
+            _ptr(load, torch.int64, "load"), _ptr(comm_span, torch.int64, "comm_span"),
+            _ptr(comm_remote, torch.int64, "comm_remote"), _ptr(ntok, torch.int64, "ntok"),
+            _ptr(fairness, torch.float32, "fairness"), _ptr(cost_per_token, torch.uint8, "cost_per_token"),
+            _ptr(serve, torch.int8, "serve"), int(flags))
+
+
+# ---- convenience wrappers: allocate outputs with torch, call, return a dict ----
+# uint32 / uint64 device buffers are held as torch int32 / int64 tensors (same bits).
+
+def tacg_coact_accumulate(ctx: Context, indices, family, E: int, F: int, D=None, Cm=None, ntok=None,
+                          flags: int = TACG_ZERO_FIRST):
+    L, N, k = indices.shape
+    dev = indices.device
+    if D is None:
+        D = torch.empty((L, F, E), dtype=torch.int32, device=dev)
+        flags |= TACG_ZERO_FIRST
+    if Cm is None:
+        Cm = torch.empty((L, F, E, E), dtype=torch.int32, device=dev)
+        flags |= TACG_ZERO_FIRST
+    if ntok is None:
+        ntok = torch.empty((F,), dtype=torch.int64, device=dev)
+        flags |= TACG_ZERO_FIRST
+    ctx.check(ctx.tacg_coact_accumulate(indices, family, N, k, L, E, F, D, Cm, ntok, flags),
+              "tacg_coact_accumulate")
+    return dict(D=D, C=Cm, ntok=ntok)
+
+
+def tacg_affinity_swapgain(ctx: Context, D, Cm, ntok, P: int, capacity: int, primary, alpha=0.25, tau=1.0,
+                           eps=1e-6, want=("pref", "W", "aff", "gain")):
+    L, F, E = D.shape
+    dev = D.device
+    out = dict(pref=None, W=None, aff=None, gain=None)
+    if "pref" in want:
+        out["pref"] = torch.empty((L, E, F), dtype=torch.float32, device=dev)
+    if "W" in want:
+        out["W"] = torch.empty((L, E, E), dtype=torch.float32, device=dev)
+    if "aff" in want and primary is not None:
+        out["aff"] = torch.empty((L, E, P), dtype=torch.float32, device=dev)
+    if "gain" in want and primary is not None:
+        out["gain"] = torch.empty((L, E, E), dtype=torch.float32, device=dev)
+    ctx.check(ctx.tacg_affinity_swapgain(D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps,
+                                         out["pref"], out["W"], out["aff"], out["gain"]),
+              "tacg_affinity_swapgain")
+    return out
+
+
+def gesr_select(ctx: Context, indices, E: int, P: int, primary, replicas, load_snapshot, theta: float,
+                token_offset: int = 0, flags: int = 0):
+    L, N, k = indices.shape
+    r = 0 if replicas is None else replicas.shape[2]
+    serve = torch.empty((L, N, k), dtype=torch.int8, device=indices.device)
+    ctx.check(ctx.gesr_select(indices, N, k, L, E, P, primary, replicas if r else None, r, load_snapshot,
+                              theta, token_offset, serve, flags), "gesr_select")
+    return serve
+
+
+def tacg_eval_placement(ctx: Context, indices, family, E: int, F: int, P: int, primary, replicas=None,
+                        theta: float = 0.15, rho: float = 0.995, microbatch: int = 0, token_offset: int = 0,
+                        load_state=None, want_cost: bool = False, want_serve: bool = False, flags: int = 0):
+    L, N, k = indices.shape
+    dev = indices.device
+    r = 0 if replicas is None else replicas.shape[2]
+    out = dict(
+        load=torch.empty((L, P), dtype=torch.int64, device=dev),
+        comm_span=torch.empty((L, F), dtype=torch.int64, device=dev),
+        comm_remote=torch.empty((L, F), dtype=torch.int64, device=dev),
+        ntok=torch.empty((F,), dtype=torch.int64, device=dev),
+        fairness=torch.empty((L + 1, 3), dtype=torch.float32, device=dev),
+        cost=torch.empty((L, N), dtype=torch.uint8, device=dev) if want_cost else None,
+        serve=torch.empty((L, N, k), dtype=torch.int8, device=dev) if want_serve else None,
+        load_state=load_state,
+    )
+    ctx.check(ctx.tacg_eval_placement(indices, family, N, k, L, E, F, P, primary, replicas if r else None, r,
+                                      theta, rho, microbatch, token_offset, load_state, out["load"],
+                                      out["comm_span"], out["comm_remote"], out["ntok"], out["fairness"],
+                                      out["cost"], out["serve"], flags), "tacg_eval_placement")
+    return out

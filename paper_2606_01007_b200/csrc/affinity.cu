@@ -1,0 +1,304 @@
+// S3..S7: preferences (Eq. 2-6), task-modulated graph (Eq. 7-8,
+// PAPER.md:97-108), expert->partition affinity (Eq. 10 inner sum) and all-pairs
+// swap gains (north_star).  All arithmetic is fp64 on device (DESIGN.md
+// "Precision": the z-score divides rounding noise by eps when sigma ~ 0, Q6), results are
+// rounded once to fp32 on store.  Four small kernels, each a grid over (row block, layer):
+//   rowstats : per (l,f,i) integer row sums of C and the row maximum of Abar
+//   pref     : per layer, u/c/du/dc/z/s/softmax and max Abar
+//   graph_aff: W rows and their per-partition segmented sums (aff)
+//   gain     : all-pairs swap gains from aff (fp64 scratch) and W (recomputed in fp64)
+// The E x E work is HBM/L2 streaming of C (4*F*E*E bytes per layer); the contraction
+// pref.pref^T has inner dimension F <= 8 and W.M is a segmented row sum over a one-hot
+// membership matrix, so neither is tensor-core work.
+#include "tacg_common.cuh"
+
+namespace {
+
+constexpr int kRowsPerCta = 8;     // one warp per matrix row
+constexpr int kRowThreads = kRowsPerCta * 32;
+
+struct AffScratch {
+    unsigned long long* rowsum;  // [L,F,E]
+    double* rowmax;              // [L,E]
+    double* amax;                // [L]
+    double* pref64;              // [L,E,F]
+    double* aff64;               // [L,E,P]
+};
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_max(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// Abar[i,j] = (1/F) sum_f C[f,i,j] / max(1,ntok[f])   (readings Q2, Q4)
+__device__ __forceinline__ double abar_entry(const unsigned* __restrict__ Cl, const double* nf, int F, int E, int i, int j) {
+    double s = 0.0;
+    for (int f = 0; f < F; ++f) s += (double)__ldg(&Cl[((size_t)f * E + i) * E + j]) / nf[f];
+    return s / (double)F;
+}
+
+// W[i,j] of Eq. 8 from Abar, max Abar and the preference rows of i and j (Eq. 7).
+__device__ __forceinline__ double w_entry(double abar, double amax, const double* pi, const double* pj, int F, double alpha) {
+    const double ah = amax > 0.0 ? abar / amax : 0.0;
+    double at = 0.0;
+    for (int f = 0; f < F; ++f) at += pi[f] * pj[f];
+    return (1.0 - alpha) * ah + alpha * (at * ah);
+}
+
+__global__ void __launch_bounds__(kRowThreads)
+rowstats_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, AffScratch s) {
+    const int l = blockIdx.y;
+    const int i = blockIdx.x * kRowsPerCta + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (i >= E) return;
+    double nf[8];
+    for (int f = 0; f < F; ++f) nf[f] = (double)max(1ull, ntok[f]);
+    const unsigned* Cl = C + (size_t)l * F * E * E;
+    double rmax = 0.0;
+    for (int j = lane; j < E; j += 32) rmax = fmax(rmax, abar_entry(Cl, nf, F, E, i, j));
+    rmax = warp_max(rmax);
+    for (int f = 0; f < F; ++f) {
+        unsigned long long acc = 0;
+        for (int j = lane; j < E; j += 32) acc += __ldg(&Cl[((size_t)f * E + i) * E + j]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane == 0) s.rowsum[((size_t)l * F + f) * E + i] = acc;
+    }
+    if (lane == 0) s.rowmax[(size_t)l * E + i] = rmax;
+}
+
+__device__ double block_sum(double v, double* red) {
+    v = warp_sum(v);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+    __syncthreads();
+    double t = 0.0;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+    return t;
+}
+
+// One CTA per layer.  Dynamic smem: u[F][E], c[F][E], sc[F][E] doubles.
+__global__ void __launch_bounds__(256)
+pref_kernel(const unsigned* __restrict__ D, const unsigned long long* __restrict__ ntok, int E, int F, double tau,
+            double eps, AffScratch s, float* __restrict__ pref_out) {
+    extern __shared__ double psm[];
+    __shared__ double red[8];
+    double* u = psm;
+    double* c = psm + (size_t)F * E;
+    double* sc = psm + (size_t)2 * F * E;
+    const int l = blockIdx.x;
+    const unsigned* Dl = D + (size_t)l * F * E;
+    // O2: u = D / sum D (Q1), c = rowsum(C)/N_f (Eq. 2 right; counts >= 0 so |.| is the identity, Q3)
+    for (int f = 0; f < F; ++f) {
+        double part = 0.0;
+        for (int e = threadIdx.x; e < E; e += blockDim.x) part += (double)Dl[f * E + e];   // exact: integers < 2^53
+        const double tot = fmax(1.0, block_sum(part, red));
+        const double nf = (double)max(1ull, ntok[f]);
+        for (int e = threadIdx.x; e < E; e += blockDim.x) {
+            u[f * E + e] = (double)Dl[f * E + e] / tot;
+            c[f * E + e] = (double)s.rowsum[((size_t)l * F + f) * E + e] / nf;
+            sc[f * E + e] = 0.0;
+        }
+    }
+    __syncthreads();
+    // O3, O4: relative advantage (Eq. 2-3) and z-score over experts (Eq. 4), summed into s (Eq. 5)
+    for (int pass = 0; pass < 2; ++pass) {
+        const double* x = pass == 0 ? u : c;
+        for (int f = 0; f < F; ++f) {
+            double part = 0.0;
+            for (int e = threadIdx.x; e < E; e += blockDim.x) {
+                double other = 0.0;
+                if (F > 1) {
+                    for (int g = 0; g < F; ++g)
+                        if (g != f) other += x[g * E + e];
+                    other /= (double)(F - 1);
+                }
+                part += x[f * E + e] - other;
+            }
+            const double mu = block_sum(part, red) / (double)E;
+            double vpart = 0.0;
+            for (int e = threadIdx.x; e < E; e += blockDim.x) {
+                double other = 0.0;
+                if (F > 1) {
+                    for (int g = 0; g < F; ++g)
+                        if (g != f) other += x[g * E + e];
+                    other /= (double)(F - 1);
+                }
+                const double d = (x[f * E + e] - other) - mu;
+                vpart += d * d;
+            }
+            const double sigma = sqrt(block_sum(vpart, red) / (double)E);
+            for (int e = threadIdx.x; e < E; e += blockDim.x) {
+                double other = 0.0;
+                if (F > 1) {
+                    for (int g = 0; g < F; ++g)
+                        if (g != f) other += x[g * E + e];
+                    other /= (double)(F - 1);
+                }
+                sc[f * E + e] += ((x[f * E + e] - other) - mu) / (sigma + eps);
+            }
+        }
+    }
+    __syncthreads();
+    // O5: temperature softmax over families (Eq. 6), max subtracted
+    for (int e = threadIdx.x; e < E; e += blockDim.x) {
+        double m = -INFINITY;
+        for (int f = 0; f < F; ++f) m = fmax(m, sc[f * E + e] / tau);
+        double ex[8];
+        double tot = 0.0;
+        for (int f = 0; f < F; ++f) {
+            ex[f] = exp(sc[f * E + e] / tau - m);
+            tot += ex[f];
+        }
+        for (int f = 0; f < F; ++f) {
+            const double p = ex[f] / tot;
+            s.pref64[((size_t)l * E + e) * F + f] = p;
+            if (pref_out) pref_out[((size_t)l * E + e) * F + f] = (float)p;
+        }
+    }
+    // max Abar over the layer (Q8)
+    double mx = 0.0;
+    for (int e = threadIdx.x; e < E; e += blockDim.x) mx = fmax(mx, s.rowmax[(size_t)l * E + e]);
+    mx = warp_max(mx);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t = fmax(t, red[w]);
+        s.amax[l] = t;
+    }
+}
+
+// Dynamic smem: wrow[kRowsPerCta][E] doubles, then order[E] int16 (experts sorted by partition),
+// start[65] int.
+__global__ void __launch_bounds__(kRowThreads)
+graph_aff_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, int P,
+                 const int8_t* __restrict__ primary, double alpha, AffScratch s, float* __restrict__ W_out,
+                 float* __restrict__ aff_out) {
+    extern __shared__ double gsm[];
+    double* wrow = gsm;
+    short* order = reinterpret_cast<short*>(gsm + (size_t)kRowsPerCta * E);
+    __shared__ int start[65];
+    const int l = blockIdx.y;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int8_t* pr = primary ? primary + (size_t)l * E : nullptr;
+    if (pr) {
+        // counting sort of the experts by partition, ascending expert id inside a partition
+        if (threadIdx.x < P) {
+            int n = 0;
+            for (int e = 0; e < E; ++e) n += (pr[e] == (int)threadIdx.x);
+            start[threadIdx.x + 1] = n;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            start[0] = 0;
+            for (int m = 0; m < P; ++m) start[m + 1] += start[m];
+        }
+        __syncthreads();
+        if (threadIdx.x < P) {
+            int pos = start[threadIdx.x];
+            for (int e = 0; e < E; ++e)
+                if (pr[e] == (int)threadIdx.x) order[pos++] = (short)e;
+        }
+        __syncthreads();
+    }
+    const int i = blockIdx.x * kRowsPerCta + warp;
+    if (i >= E) return;
+    double nf[8], pi[8];
+    for (int f = 0; f < F; ++f) {
+        nf[f] = (double)max(1ull, ntok[f]);
+        pi[f] = s.pref64[((size_t)l * E + i) * F + f];
+    }
+    const unsigned* Cl = C + (size_t)l * F * E * E;
+    const double amax = s.amax[l];
+    double* wr = wrow + (size_t)warp * E;
+    for (int j = lane; j < E; j += 32) {
+        const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), amax, pi, s.pref64 + ((size_t)l * E + j) * F, F, alpha);
+        wr[j] = w;
+        if (W_out) W_out[((size_t)l * E + i) * E + j] = (float)w;
+    }
+    __syncwarp();
+    if (pr) {
+        // aff[i,m] = sum over the members of partition m, in ascending expert id (Eq. 10 inner sum)
+        for (int m = lane; m < P; m += 32) {
+            double acc = 0.0;
+            for (int q = start[m]; q < start[m + 1]; ++q) acc += wr[order[q]];
+            s.aff64[((size_t)l * E + i) * P + m] = acc;
+            if (aff_out) aff_out[((size_t)l * E + i) * P + m] = (float)acc;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kRowThreads)
+gain_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, int P,
+            const int8_t* __restrict__ primary, double alpha, AffScratch s, float* __restrict__ gain_out) {
+    const int l = blockIdx.y;
+    const int i = blockIdx.x * kRowsPerCta + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (i >= E) return;
+    const int8_t* pr = primary + (size_t)l * E;
+    double nf[8], pi[8];
+    for (int f = 0; f < F; ++f) {
+        nf[f] = (double)max(1ull, ntok[f]);
+        pi[f] = s.pref64[((size_t)l * E + i) * F + f];
+    }
+    const unsigned* Cl = C + (size_t)l * F * E * E;
+    const double amax = s.amax[l];
+    const double* affl = s.aff64 + (size_t)l * E * P;
+    const int a = pr[i] & 63;
+    for (int j = lane; j < E; j += 32) {
+        const int b = pr[j] & 63;
+        double g = 0.0;
+        if (a != b) {
+            const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), amax, pi, s.pref64 + ((size_t)l * E + j) * F, F, alpha);
+            g = affl[(size_t)i * P + b] + affl[(size_t)j * P + a] - affl[(size_t)i * P + a] - affl[(size_t)j * P + b] - 2.0 * w;
+        }
+        gain_out[((size_t)l * E + i) * E + j] = (float)g;
+    }
+}
+
+}  // namespace
+
+int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L, int E,
+                         int F, int P, const int8_t* primary, double alpha, double tau, double eps, float* pref,
+                         float* W, float* aff, float* gain) {
+    size_t off = 0;
+    const size_t o_rowsum = off; off += tacg_align_up(sizeof(unsigned long long) * (size_t)L * F * E, 256);
+    const size_t o_rowmax = off; off += tacg_align_up(sizeof(double) * (size_t)L * E, 256);
+    const size_t o_amax = off;   off += tacg_align_up(sizeof(double) * (size_t)L, 256);
+    const size_t o_pref = off;   off += tacg_align_up(sizeof(double) * (size_t)L * E * F, 256);
+    const size_t o_aff = off;    off += tacg_align_up(sizeof(double) * (size_t)L * E * P, 256);
+    char* base = static_cast<char*>(tacg_scratch(ctx, off));
+    if (!base) return TACG_ERR_CUDA;
+    AffScratch s;
+    s.rowsum = reinterpret_cast<unsigned long long*>(base + o_rowsum);
+    s.rowmax = reinterpret_cast<double*>(base + o_rowmax);
+    s.amax = reinterpret_cast<double*>(base + o_amax);
+    s.pref64 = reinterpret_cast<double*>(base + o_pref);
+    s.aff64 = reinterpret_cast<double*>(base + o_aff);
+    const unsigned long long* nt = reinterpret_cast<const unsigned long long*>(ntok);
+    const dim3 rows((E + kRowsPerCta - 1) / kRowsPerCta, L);
+    rowstats_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, s);
+    TACG_LAUNCH_CHECK(ctx);
+    const size_t psm = sizeof(double) * (size_t)3 * F * E;
+    TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(pref_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
+    pref_kernel<<<L, 256, psm, ctx->stream>>>(D, nt, E, F, tau, eps, s, pref);
+    TACG_LAUNCH_CHECK(ctx);
+    if (W || aff || gain) {
+        const size_t gsm = sizeof(double) * (size_t)kRowsPerCta * E + sizeof(short) * (size_t)E;
+        graph_aff_kernel<<<rows, kRowThreads, gsm, ctx->stream>>>(C, nt, E, F, P, primary, alpha, s, W, aff);
+        TACG_LAUNCH_CHECK(ctx);
+    }
+    if (gain) {
+        gain_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, P, primary, alpha, s, gain);
+        TACG_LAUNCH_CHECK(ctx);
+    }
+    return TACG_OK;
+}

@@ -1,0 +1,106 @@
+// Internal declarations shared by the translation units of libtacg (CUDA path only;
+// nothing here is shared with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "tacg.h"
+
+struct tacg_ctx {
+    int device;
+    cudaStream_t stream;
+    int sm_count;
+    int smem_optin;        // max dynamic shared memory per block (opt-in), bytes
+    void* scratch;         // grows on demand, reused across calls
+    size_t scratch_bytes;
+    unsigned long long* errword;  // device: [0] = first bad record + 1 (0 = none), [1] = kind
+    char detail[256];
+    int last_path;
+    int64_t launches;
+};
+
+#define TACG_CUDA_TRY(ctx, expr)                                                        \
+    do {                                                                                \
+        cudaError_t _e = (expr);                                                        \
+        if (_e != cudaSuccess) {                                                        \
+            snprintf((ctx)->detail, sizeof((ctx)->detail), "%s: %s (%s:%d)", #expr,     \
+                     cudaGetErrorString(_e), __FILE__, __LINE__);                       \
+            return TACG_ERR_CUDA;                                                       \
+        }                                                                               \
+    } while (0)
+
+#define TACG_LAUNCH_CHECK(ctx)                  \
+    do {                                        \
+        (ctx)->launches += 1;                   \
+        TACG_CUDA_TRY(ctx, cudaGetLastError()); \
+    } while (0)
+
+// Returns a device scratch pointer of at least `bytes` (256-byte aligned), or nullptr
+// after recording the CUDA error text in ctx->detail.
+void* tacg_scratch(tacg_ctx* ctx, size_t bytes);
+
+static inline size_t tacg_align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// ---- launchers (each returns a tacg_status) ----
+int tacg_launch_family_count(tacg_ctx* ctx, const int8_t* family, int64_t N, int F, uint64_t* ntok);
+int tacg_launch_validate_trace(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N,
+                               int k, int L, int E, int F);
+int tacg_launch_validate_placement(tacg_ctx* ctx, int L, int E, int P, int capacity,
+                                   const int8_t* primary, const int8_t* replicas, int r);
+int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k,
+                           int L, int E, int F, uint32_t* D, uint32_t* C);
+bool tacg_coact_mma_supported(int k, int E, int F);
+int tacg_launch_coact_mma(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k,
+                          int L, int E, int F, uint32_t* D, uint32_t* C);
+int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L,
+                         int E, int F, int P, const int8_t* primary, double alpha, double tau, double eps,
+                         float* pref, float* W, float* aff, float* gain);
+int tacg_launch_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P,
+                       const int8_t* primary, const int8_t* replicas, int r, const double* snapshot,
+                       float theta, int64_t token_offset, int8_t* serve);
+int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k, int L,
+                     int E, int F, int P, const int8_t* primary, const int8_t* replicas, int r, float theta,
+                     double rho, int64_t microbatch, int64_t token_offset, double* load_state,
+                     uint64_t* load, uint64_t* comm_span, uint64_t* comm_remote, float* fairness,
+                     uint8_t* cost_per_token, int8_t* serve);
+
+// ---- device helpers ----
+#ifdef __CUDACC__
+// Loads the KT expert ids of one token row.  KT in {2,4,6,8}: vector loads (the host
+// checked the base alignment); KT == 0: k runtime, 2-byte loads.
+template <int KT>
+__device__ __forceinline__ void tacg_load_ids(const int16_t* __restrict__ row, int k, int (&e)[KT > 0 ? KT : 16]) {
+    if constexpr (KT == 8) {
+        const int4 v = __ldg(reinterpret_cast<const int4*>(row));
+        e[0] = (short)(v.x & 0xffff); e[1] = v.x >> 16;
+        e[2] = (short)(v.y & 0xffff); e[3] = v.y >> 16;
+        e[4] = (short)(v.z & 0xffff); e[5] = v.z >> 16;
+        e[6] = (short)(v.w & 0xffff); e[7] = v.w >> 16;
+    } else if constexpr (KT == 6) {
+        const int* p = reinterpret_cast<const int*>(row);
+        const int a = __ldg(p), b = __ldg(p + 1), c = __ldg(p + 2);
+        e[0] = (short)(a & 0xffff); e[1] = a >> 16;
+        e[2] = (short)(b & 0xffff); e[3] = b >> 16;
+        e[4] = (short)(c & 0xffff); e[5] = c >> 16;
+    } else if constexpr (KT == 4) {
+        const int2 v = __ldg(reinterpret_cast<const int2*>(row));
+        e[0] = (short)(v.x & 0xffff); e[1] = v.x >> 16;
+        e[2] = (short)(v.y & 0xffff); e[3] = v.y >> 16;
+    } else if constexpr (KT == 2) {
+        const int a = __ldg(reinterpret_cast<const int*>(row));
+        e[0] = (short)(a & 0xffff); e[1] = a >> 16;
+    } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) e[j] = (j < k) ? (int)__ldg(row + j) : -1;
+    }
+}
+
+// The compile-time slot count for a (k, base pointer) pair; 0 = generic path.
+static inline int tacg_pick_kt(int k, const void* base) {
+    const uintptr_t a = reinterpret_cast<uintptr_t>(base);
+    if ((k == 2 || k == 4 || k == 6 || k == 8) && (a % 16) == 0) return k;
+    return 0;
+}
+#endif
