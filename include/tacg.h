@@ -74,6 +74,18 @@ int64_t tacg_launch_count(tacg_ctx* ctx);
 /* Library version, "major.minor". */
 const char* tacg_version(void);
 
+/* Optional device timing of the library's own kernels (used by bench.py for the roofline
+ * figure): while enabled, every launch of the slot's kernel(s) is bracketed by CUDA events
+ * on the ctx stream.  tacg_profile_read synchronises those events, returns the summed
+ * duration in milliseconds and the number of bracketed launches since the last read, and
+ * resets the slot.  Timing is off by default and costs nothing when off. */
+#define TACG_PROF_COACT    0 /* the co-activation kernel (histogram or tcgen05), one launch per call */
+#define TACG_PROF_AFFINITY 1 /* the kernels of tacg_affinity_swapgain, bracketed as one group per call */
+#define TACG_PROF_EVAL     2 /* eval_kernel, one launch per call */
+#define TACG_PROF_SLOTS    3
+int tacg_profile_enable(tacg_ctx* ctx, int on);
+int tacg_profile_read(tacg_ctx* ctx, int slot, double* total_ms, int64_t* launches);
+
 /* S1+S2 -- per-family usage and co-activation counts
  * ("usage vector u ... coactivation matrix A ... frequency of expert pairs selected
  * by the same token", per layer and task family).

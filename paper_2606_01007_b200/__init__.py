@@ -9,5 +9,5 @@ from .binding import (  # noqa: F401
     Context, TacgError, lib, lib_path, version,
     tacg_coact_accumulate, tacg_affinity_swapgain, gesr_select, tacg_eval_placement,
     TACG_ZERO_FIRST, TACG_VALIDATE, TACG_PATH_AUTO, TACG_PATH_HIST, TACG_PATH_MMA,
-    EXPORTS,
+    TACG_PROF_COACT, TACG_PROF_AFFINITY, TACG_PROF_EVAL, EXPORTS,
 )

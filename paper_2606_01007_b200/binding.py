@@ -21,10 +21,11 @@ TACG_VALIDATE = 0x2
 TACG_PATH_AUTO = 0x00
 TACG_PATH_HIST = 0x10
 TACG_PATH_MMA = 0x20
+TACG_PROF_COACT, TACG_PROF_AFFINITY, TACG_PROF_EVAL = 0, 1, 2
 
 EXPORTS = (
     "tacg_create", "tacg_destroy", "tacg_strerror", "tacg_last_detail", "tacg_last_path",
-    "tacg_launch_count", "tacg_version", "tacg_coact_accumulate", "tacg_affinity_swapgain",
+    "tacg_launch_count", "tacg_version", "tacg_profile_enable", "tacg_profile_read", "tacg_coact_accumulate", "tacg_affinity_swapgain",
     "gesr_select", "tacg_eval_placement",
 )
 
@@ -62,6 +63,8 @@ def lib():
         L.tacg_launch_count.argtypes = [vp]
         L.tacg_launch_count.restype = i64
         L.tacg_version.restype = C.c_char_p
+        L.tacg_profile_enable.argtypes = [vp, i32]
+        L.tacg_profile_read.argtypes = [vp, i32, C.POINTER(f64), C.POINTER(i64)]
         L.tacg_coact_accumulate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp, u32]
         L.tacg_affinity_swapgain.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, f32, f32, f32,
                                              vp, vp, vp, vp]
@@ -132,6 +135,15 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().tacg_launch_count(self._h))
+
+    def profile_enable(self, on: bool = True):
+        self.check(lib().tacg_profile_enable(self._h, 1 if on else 0), "tacg_profile_enable")
+
+    def profile_read(self, slot: int):
+        """(total_ms, launches) of the slot's kernels since the last read (synchronises their events)."""
+        ms, n = C.c_double(0.0), C.c_int64(0)
+        self.check(lib().tacg_profile_read(self._h, int(slot), C.byref(ms), C.byref(n)), "tacg_profile_read")
+        return ms.value, n.value
 
     def check(self, rc: int, where: str):
         if rc != 0:

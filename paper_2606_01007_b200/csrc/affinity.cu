@@ -285,6 +285,7 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     s.aff64 = reinterpret_cast<double*>(base + o_aff);
     const unsigned long long* nt = reinterpret_cast<const unsigned long long*>(ntok);
     const dim3 rows((E + kRowsPerCta - 1) / kRowsPerCta, L);
+    tacg_prof_scope prof(ctx, TACG_PROF_AFFINITY);
     rowstats_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, s);
     TACG_LAUNCH_CHECK(ctx);
     const size_t psm = sizeof(double) * (size_t)3 * F * E;

@@ -178,6 +178,7 @@ int launch_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int
     const long long blocks = (N + kHistThreads - 1) / kHistThreads;
     if ((long long)cpl > blocks) cpl = (int)max(1ll, blocks);
     const int grid = L * cpl;
+    tacg_prof_scope prof(ctx, TACG_PROF_COACT);
     if (use_smem) {
         auto kern = coact_hist_kernel<KT, true>;
         TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -374,6 +374,7 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     p.delta = reinterpret_cast<unsigned long long*>(base + o_delta);
     p.barrier = reinterpret_cast<unsigned*>(base + o_bar);
     if (p.cpl > 1) TACG_CUDA_TRY(ctx, cudaMemsetAsync(base, 0, off, ctx->stream));
+    tacg_prof_scope prof(ctx, TACG_PROF_EVAL);
     if (waits) {
         void* args[] = {&p};
         TACG_CUDA_TRY(ctx, cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(kEvalThreads), args, smem,

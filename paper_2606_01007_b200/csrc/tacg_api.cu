@@ -91,6 +91,7 @@ int tacg_create(tacg_ctx** out, int device, void* cuda_stream) {
     ctx->detail[0] = 0;
     ctx->last_path = 0;
     ctx->launches = 0;
+    ctx->profiling = false;
     if (cudaMalloc(&ctx->errword, 2 * sizeof(unsigned long long)) != cudaSuccess) {
         delete ctx;
         return TACG_ERR_CUDA;
@@ -103,6 +104,8 @@ int tacg_destroy(tacg_ctx* ctx) {
     if (!ctx) return TACG_ERR_NULL;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    for (int sl = 0; sl < TACG_PROF_SLOTS; ++sl)
+        for (auto& pr : ctx->prof[sl]) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
     if (ctx->scratch) cudaFree(ctx->scratch);
     if (ctx->errword) cudaFree(ctx->errword);
     delete ctx;
@@ -114,6 +117,32 @@ int tacg_last_detail(tacg_ctx* ctx, char* buf, size_t n) {
     if (n == 0) return TACG_OK;
     strncpy(buf, ctx->detail, n - 1);
     buf[n - 1] = 0;
+    return TACG_OK;
+}
+
+int tacg_profile_enable(tacg_ctx* ctx, int on) {
+    if (!ctx) return TACG_ERR_NULL;
+    ctx->profiling = on != 0;
+    return TACG_OK;
+}
+
+int tacg_profile_read(tacg_ctx* ctx, int slot, double* total_ms, int64_t* launches) {
+    if (!ctx || !total_ms || !launches) return TACG_ERR_NULL;
+    if (slot < 0 || slot >= TACG_PROF_SLOTS) return TACG_ERR_SHAPE;
+    double tot = 0.0;
+    int64_t n = 0;
+    for (auto& pr : ctx->prof[slot]) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(pr.second) == cudaSuccess && cudaEventElapsedTime(&ms, pr.first, pr.second) == cudaSuccess) {
+            tot += ms;
+            n += 1;
+        }
+        cudaEventDestroy(pr.first);
+        cudaEventDestroy(pr.second);
+    }
+    ctx->prof[slot].clear();
+    *total_ms = tot;
+    *launches = n;
     return TACG_OK;
 }
 

@@ -6,6 +6,9 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <utility>
+#include <vector>
+
 #include "tacg.h"
 
 struct tacg_ctx {
@@ -19,6 +22,27 @@ struct tacg_ctx {
     char detail[256];
     int last_path;
     int64_t launches;
+    bool profiling;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof[TACG_PROF_SLOTS];
+};
+
+// Event brackets around the library's own kernels (tacg_profile_enable); no-ops when off.
+struct tacg_prof_scope {
+    tacg_ctx* ctx;
+    int slot;
+    cudaEvent_t e0, e1;
+    tacg_prof_scope(tacg_ctx* c, int s) : ctx(c), slot(s), e0(nullptr), e1(nullptr) {
+        if (ctx->profiling && cudaEventCreate(&e0) == cudaSuccess && cudaEventCreate(&e1) == cudaSuccess)
+            cudaEventRecord(e0, ctx->stream);
+        else
+            e0 = e1 = nullptr;
+    }
+    ~tacg_prof_scope() {
+        if (e1) {
+            cudaEventRecord(e1, ctx->stream);
+            ctx->prof[slot].emplace_back(e0, e1);
+        }
+    }
 };
 
 #define TACG_CUDA_TRY(ctx, expr)                                                        \

@@ -1,0 +1,85 @@
+"""Host-side placement driver (harness) -- consumes the library's outputs.
+
+These are the consumers of the hot path, not part of it: a capacity-preserving best-swap
+local search driven by the GPU swap gains (standing in for the repair loop of
+PAPER.md:119-124; the paper's spectral stage is NEXT f1), and the GESR replica table with
+the canonical lambda1 = lambda2 = 0 (centrality only).  All
+E x E arithmetic stays in tacg_affinity_swapgain; the host only takes argmaxes.
+"""
+from __future__ import annotations
+
+from typing import Optional, Tuple
+
+import numpy as np
+import torch
+
+from . import binding as _b
+
+
+def default_placement(L: int, E: int, capacity: int) -> np.ndarray:
+    """primary[l,e] = e // capacity (the paper's 'Baseline' placement)."""
+    return np.tile((np.arange(E) // capacity).astype(np.int8), (L, 1))
+
+
+def local_search(ctx: "_b.Context", D, Cm, ntok, P: int, capacity: int, alpha: float = 0.25, tau: float = 1.0,
+                 eps: float = 1e-6, max_swaps: Optional[int] = None,
+                 primary0: Optional[np.ndarray] = None) -> Tuple[np.ndarray, np.ndarray]:
+    """Best-swap local search on every layer at once.  Each round calls
+    tacg_affinity_swapgain for all layers, copies gain/aff/W back and applies, per layer, the
+    swap with the largest gain if it exceeds 1e-7 * sum|terms| (ties -> smallest (i,j)).
+    Returns (primary int8[L,E], swaps per layer)."""
+    L, F, E = D.shape
+    primary = default_placement(L, E, capacity) if primary0 is None else primary0.astype(np.int8).copy()
+    if max_swaps is None:
+        max_swaps = 4 * E
+    swaps = np.zeros(L, dtype=np.int64)
+    active = np.ones(L, dtype=bool)
+    dev = D.device
+    ar = np.arange(E)
+    for _ in range(max_swaps):
+        out = _b.tacg_affinity_swapgain(ctx, D, Cm, ntok, P, capacity, torch.from_numpy(primary).to(dev),
+                                        alpha=alpha, tau=tau, eps=eps, want=("W", "aff", "gain"))
+        G = out["gain"].cpu().numpy()
+        aff = out["aff"].cpu().numpy()
+        W = out["W"].cpu().numpy()
+        any_swap = False
+        for l in np.nonzero(active)[0]:
+            g = np.triu(G[l], 1)
+            flat = int(np.argmax(g))            # first maximum = smallest (i,j)
+            i, j = divmod(flat, E)
+            best = float(g[i, j])
+            a, b = int(primary[l, i]), int(primary[l, j])
+            terms = abs(aff[l, i, b]) + abs(aff[l, j, a]) + abs(aff[l, i, a]) + abs(aff[l, j, b]) + 2 * abs(W[l, i, j])
+            if a != b and best > 1e-7 * terms and best > 0:
+                primary[l, i], primary[l, j] = b, a
+                swaps[l] += 1
+                any_swap = True
+            else:
+                active[l] = False
+        if not any_swap:
+            break
+    return primary, swaps
+
+
+def replica_table(ctx: "_b.Context", D, Cm, ntok, P: int, capacity: int, primary: np.ndarray, n_rep: int, r: int,
+                  alpha: float = 0.25, tau: float = 1.0, eps: float = 1e-6) -> np.ndarray:
+    """GESR offline step with lambda1 = lambda2 = 0: generic experts = top n_rep by centrality
+    (row sum of the pooled graph; Ahat = W at alpha = 0 is Abar up to a positive factor), their
+    secondaries = the r non-primary partitions with the largest affinity (Eq. 12).  Ties -> lower id."""
+    L, F, E = D.shape
+    rep = np.full((L, E, max(r, 0)), -1, dtype=np.int8)
+    if r <= 0 or n_rep <= 0:
+        return rep
+    dev = D.device
+    pooled = _b.tacg_affinity_swapgain(ctx, D, Cm, ntok, P, capacity, None, alpha=0.0, tau=tau, eps=eps, want=("W",))
+    cent = pooled["W"].double().sum(dim=2).cpu().numpy()
+    out = _b.tacg_affinity_swapgain(ctx, D, Cm, ntok, P, capacity, torch.from_numpy(primary.astype(np.int8)).to(dev),
+                                    alpha=alpha, tau=tau, eps=eps, want=("aff",))
+    aff = out["aff"].cpu().numpy()
+    for l in range(L):
+        order = sorted(range(E), key=lambda e: (-cent[l, e], e))
+        for e in order[:n_rep]:
+            cands = sorted((m for m in range(P) if m != int(primary[l, e])), key=lambda m: (-aff[l, e, m], m))
+            for i, m in enumerate(cands[:r]):
+                rep[l, e, i] = m
+    return rep
