@@ -1,239 +1,382 @@
-// S1+S2 histogram path (TACG_PATH_HIST): dispatch counts D and pair counts C by atomic
-// increments.  One thread per token; a CTA keeps a private upper-triangular
-// uint32 histogram per family in shared memory when it fits and flushes it once with
-// global reductions, otherwise it increments global memory directly.
-// Also: the family histogram ntok[F] and the TACG_VALIDATE kernels.
+// S1+S2 histogram path (TACG_PATH_HIST): dispatch counts D and pair counts C.
+//
+// Two kernels, no global atomics:
+//   coact_hist_kernel      persistent, one CTA per SM.  A CTA owns a contiguous range of
+//                          (layer, token-chunk) items and keeps a PRIVATE strict-upper-triangular
+//                          uint32 pair histogram in shared memory (all F families when they fit,
+//                          else one family per CTA with the tokens of that family compacted through
+//                          a per-warp queue).  It is written once per (CTA, layer) to a scratch slot
+//                          with 16-byte stores.
+//   coact_finalize_kernel  one CTA per (layer, family): sums the slots of that layer, mirrors the
+//                          triangle into the symmetric C (zero diagonal untouched), derives D, adds
+//                          ntok.  With TACG_ZERO_FIRST it stores, otherwise it adds to what is there.
+//
+// D is not counted with its own atomics.  A token with all k slots valid and distinct puts each of
+// its experts into exactly k-1 pair increments, so D[e] = (sum of the pair bins touching e) / (k-1);
+// a token with empty slots adds the shortfall to a per-expert correction counter, which makes the
+// identity exact for every token (see slow_token()).
+//
+// Fallback for shapes whose single-family triangle does not fit in shared memory (E > ~330):
+// coact_global_kernel, plain global atomics.
 #include "tacg_common.cuh"
 
 namespace {
 
-constexpr int kHistThreads = 512;
+constexpr int kThreads = 1024;           // one CTA per SM
+constexpr int kWarps = kThreads / 32;
+constexpr int kQueue = 160;              // per-warp token queue of the family-filter mode (<= 31 + 128 entries)
 
-// index of the unordered pair i < j in a row-major strict upper triangle of an E x E matrix
-__device__ __forceinline__ int tri_index(int i, int j, int E) { return i * (2 * E - i - 1) / 2 + (j - i - 1); }
+struct HistParams {
+    const int16_t* indices;
+    const int8_t* family;
+    long long N;
+    int k, L, E, F;
+    int nfg;            // 1: a CTA counts all F families; F: CTA c counts family c % F only
+    int Fs;             // families per slot (F or 1)
+    int tri;            // E(E-1)/2
+    int chunk;          // tokens per work item
+    int cps;            // items per layer
+    long long T;        // L * cps
+    int groups;         // CTAs / nfg; group g owns items [g*T/groups, (g+1)*T/groups)
+    unsigned* scratch;  // [(groups+L-1)*nfg][slot_words]
+    int slot_words;     // Fs*(tri+E+1) rounded up to 4
+};
 
-template <int KT, bool SMEM>
-__global__ void __launch_bounds__(kHistThreads)
-coact_hist_kernel(const int16_t* __restrict__ indices, const int8_t* __restrict__ family, long long N, int k, int L,
-                  int E, int F, int ctas_per_layer, unsigned* __restrict__ D, unsigned* __restrict__ C) {
-    extern __shared__ unsigned hsm[];   // SMEM: [F][tri] pair bins, then [F][E] dispatch bins
-    const int tri = E * (E - 1) / 2;
-    const int layer = blockIdx.x / ctas_per_layer;
-    const int part = blockIdx.x % ctas_per_layer;
-    if (layer >= L) return;
-    if (SMEM) {
-        for (int i = threadIdx.x; i < F * (tri + E); i += blockDim.x) hsm[i] = 0u;
-        __syncthreads();
+__host__ __device__ __forceinline__ long long group_lo(long long g, long long T, int groups) { return g * T / groups; }
+
+// the group that owns item x
+__device__ __forceinline__ int group_of_item(long long x, long long T, int groups) {
+    int g = (int)((x * groups) / T);
+    if (g >= groups) g = groups - 1;
+    while (g + 1 < groups && group_lo(g + 1, T, groups) <= x) ++g;
+    while (g > 0 && group_lo(g, T, groups) > x) --g;
+    return g;
+}
+
+// R(i) + j is the bin of the pair i < j in a row-major strict upper triangle of an E x E matrix:
+// R(i) = i(2E-1-i)/2 - i - 1 = i(2E-3-i)/2 - 1 (the product is always even).
+__device__ __forceinline__ int tri_row(int i, int E) { return ((i * (2 * E - 3 - i)) >> 1) - 1; }
+
+__device__ __forceinline__ void cswap(int& a, int& b) {
+    const int lo = min(a, b), hi = max(a, b);
+    a = lo; b = hi;
+}
+
+template <int K>
+__device__ __forceinline__ void sort_ids(int (&e)[K]) {
+    if constexpr (K == 2) {
+        cswap(e[0], e[1]);
+    } else if constexpr (K == 4) {
+        cswap(e[0], e[1]); cswap(e[2], e[3]); cswap(e[0], e[2]); cswap(e[1], e[3]); cswap(e[1], e[2]);
+    } else if constexpr (K == 6) {
+        cswap(e[0], e[5]); cswap(e[1], e[3]); cswap(e[2], e[4]);
+        cswap(e[1], e[2]); cswap(e[3], e[4]);
+        cswap(e[0], e[3]); cswap(e[2], e[5]);
+        cswap(e[0], e[1]); cswap(e[2], e[3]); cswap(e[4], e[5]);
+        cswap(e[1], e[2]); cswap(e[3], e[4]);
+    } else if constexpr (K == 8) {
+        cswap(e[0], e[2]); cswap(e[1], e[3]); cswap(e[4], e[6]); cswap(e[5], e[7]);
+        cswap(e[0], e[4]); cswap(e[1], e[5]); cswap(e[2], e[6]); cswap(e[3], e[7]);
+        cswap(e[0], e[1]); cswap(e[2], e[3]); cswap(e[4], e[5]); cswap(e[6], e[7]);
+        cswap(e[2], e[4]); cswap(e[3], e[5]);
+        cswap(e[1], e[4]); cswap(e[3], e[6]);
+        cswap(e[1], e[2]); cswap(e[3], e[4]); cswap(e[5], e[6]);
     }
-    unsigned* hD = hsm + (size_t)F * tri;
-    const int16_t* base = indices + (size_t)layer * (size_t)N * (size_t)k;
-    unsigned* Dl = D + (size_t)layer * F * E;
-    unsigned* Cl = C + (size_t)layer * F * E * E;
-    // contiguous token slice of this CTA, in units of kHistThreads tokens
-    const long long blocks = (N + kHistThreads - 1) / kHistThreads;
-    const long long per = (blocks + ctas_per_layer - 1) / ctas_per_layer;
-    const long long t_begin = (long long)part * per * kHistThreads;
-    long long t_end = t_begin + per * kHistThreads;
-    if (t_end > N) t_end = N;
-    for (long long t = t_begin + threadIdx.x; t < t_end; t += kHistThreads) {
-        const int f = family[t];
-        if ((unsigned)f >= (unsigned)F) continue;       // padding token (or out of range: skipped)
-        int e[KT > 0 ? KT : 16];
-        tacg_load_ids<KT>(base + (size_t)t * k, k, e);
-        const int kk = KT > 0 ? KT : k;
+}
+
+// Any token: every slot is checked.  For each valid slot a, cnt = number of pair increments the
+// slot takes part in; the correction counter receives (k-1) - cnt so that
+// (pair bins touching e) + corr[e] = (k-1) * (valid slots holding e)   holds exactly.
+template <int KMAX>
+__device__ __forceinline__ void slow_token(const int (&e)[KMAX], int k, int E, unsigned* hist, unsigned* corr) {
+    const int km1 = max(k - 1, 1);
+    for (int a = 0; a < k; ++a) {
+        const int i = e[a];
+        if ((unsigned)i >= (unsigned)E) continue;   // empty slot (or id out of range: skipped)
+        int cnt = 0;
+        for (int b = 0; b < k; ++b) {
+            const int j = e[b];
+            if (b == a || (unsigned)j >= (unsigned)E || j == i) continue;
+            ++cnt;
+            if (b > a) atomicAdd(&hist[tri_row(min(i, j), E) + max(i, j)], 1u);
+        }
+        if (km1 - cnt) atomicAdd(&corr[i], (unsigned)(km1 - cnt));
+    }
+}
+
+// One token of a family whose triangle starts at hist (corr = its correction counters).
+template <int KT>
+__device__ __forceinline__ void count_token(const int16_t* __restrict__ row, int k, int E, unsigned* hist,
+                                            unsigned* corr) {
+    int e[KT > 0 ? KT : 16];
+    tacg_load_ids<KT>(row, k, e);
+    if constexpr (KT >= 2) {
+        int s[KT];
 #pragma unroll
-        for (int a = 0; a < (KT > 0 ? KT : 16); ++a) {
-            if (a >= kk) break;
-            const int i = e[a];
-            if ((unsigned)i >= (unsigned)E) continue;   // empty slot
-            if (SMEM) atomicAdd(&hD[f * E + i], 1u);
-            else atomicAdd(&Dl[f * E + i], 1u);
+        for (int a = 0; a < KT; ++a) s[a] = e[a];
+        sort_ids<KT>(s);
+        bool fast = s[0] >= 0 && s[KT - 1] < E;
 #pragma unroll
-            for (int b = a + 1; b < (KT > 0 ? KT : 16); ++b) {
-                if (b >= kk) break;
-                const int j = e[b];
-                if ((unsigned)j >= (unsigned)E || j == i) continue;
-                if (SMEM) {
-                    const int lo = min(i, j), hi = max(i, j);
-                    atomicAdd(&hsm[f * tri + tri_index(lo, hi, E)], 1u);
-                } else {
-                    atomicAdd(&Cl[((size_t)f * E + i) * E + j], 1u);
-                    atomicAdd(&Cl[((size_t)f * E + j) * E + i], 1u);
+        for (int a = 0; a + 1 < KT; ++a) fast = fast && (s[a] != s[a + 1]);
+        if (fast) {
+#pragma unroll
+            for (int a = 0; a + 1 < KT; ++a) {
+                unsigned* rowp = hist + tri_row(s[a], E);
+#pragma unroll
+                for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b], 1u);
+            }
+            return;
+        }
+    }
+    slow_token<(KT > 0 ? KT : 16)>(e, KT > 0 ? KT : k, E, hist, corr);
+}
+
+// smem layout (words): [Fs][tri] pair bins | [Fs][E] corr | [Fs] ntok (layer 0 only) | pad to slot_words
+//                      | (filter mode) per-warp queues of token offsets
+template <int KT, bool FILTER>
+__global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParams p) {
+    extern __shared__ __align__(16) unsigned hsm[];
+    const int tid = threadIdx.x;
+    const int g = FILTER ? blockIdx.x / p.nfg : blockIdx.x;
+    const int fg = FILTER ? blockIdx.x % p.nfg : 0;
+    const long long lo = group_lo(g, p.T, p.groups), hi = group_lo(g + 1, p.T, p.groups);
+    if (lo >= hi) return;
+    unsigned* corr = hsm + (size_t)p.Fs * p.tri;
+    unsigned* sntok = corr + (size_t)p.Fs * p.E;
+    const int k = KT > 0 ? KT : p.k;
+    uint4* hsm4 = reinterpret_cast<uint4*>(hsm);
+    const int slot4 = p.slot_words / 4;
+    for (int i = tid; i < slot4; i += kThreads) hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
+    __syncthreads();
+
+    // filter mode: per-warp queue of matching token offsets (relative to the layer's token 0)
+    unsigned* wq = hsm + p.slot_words + (tid >> 5) * kQueue;
+    int qn = 0;                         // warp-uniform
+    const int lane = tid & 31;
+
+    int layer = (int)(lo / p.cps);
+    for (long long item = lo; item <= hi; ++item) {
+        const int l = item < hi ? (int)(item / p.cps) : -1;
+        if (l != layer) {
+            const int16_t* lbase = p.indices + (size_t)layer * (size_t)p.N * k;
+            if (FILTER) {               // drain the partial queue of this layer
+                if (lane < qn) count_token<KT>(lbase + (size_t)wq[lane] * k, k, p.E, hsm, corr);
+                qn = 0;
+            }
+            __syncthreads();
+            // flush this (group, layer) visit to its slot, then clear
+            uint4* dst = reinterpret_cast<uint4*>(p.scratch + ((size_t)(g + layer) * p.nfg + fg) * p.slot_words);
+            for (int i = tid; i < slot4; i += kThreads) {
+                dst[i] = hsm4[i];
+                hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
+            }
+            __syncthreads();
+            if (l < 0) break;
+            layer = l;
+        }
+        const long long t0 = (item - (long long)l * p.cps) * p.chunk;
+        const long long t1 = min(p.N, t0 + p.chunk);
+        const int16_t* lbase = p.indices + (size_t)l * (size_t)p.N * k;
+        if (!FILTER) {
+            for (long long t = t0 + tid; t < t1; t += kThreads) {
+                const int f = p.family[t];
+                if ((unsigned)f >= (unsigned)p.F) continue;     // padding token
+                if (l == 0) atomicAdd(&sntok[f], 1u);
+                count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm + (size_t)f * p.tri, corr + f * p.E);
+            }
+        } else {
+            // each thread scans 4 consecutive tokens per step; a warp covers 128
+            for (long long tb = t0 + (long long)(tid >> 5) * 128; tb < t1; tb += (long long)kWarps * 128) {
+                const long long ta = tb + lane * 4;
+                unsigned m = 0;
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (ta + u < t1 && (int)p.family[ta + u] == fg) m |= 1u << u;
+                const int c = __popc(m);
+                int inc = c;            // inclusive warp scan
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int v = __shfl_up_sync(0xffffffffu, inc, d);
+                    if (lane >= d) inc += v;
                 }
+                const int total = __shfl_sync(0xffffffffu, inc, 31);
+                int pos = qn + inc - c;
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (m & (1u << u)) wq[pos++] = (unsigned)(ta + u);
+                qn += total;
+                if (l == 0 && lane == 0 && total) atomicAdd(&sntok[0], (unsigned)total);
+                __syncwarp();
+                while (qn >= 32) {
+                    qn -= 32;
+                    const unsigned t = wq[qn + lane];
+                    count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm, corr);
+                }
+                __syncwarp();
             }
         }
     }
-    if (SMEM) {
-        __syncthreads();
-        for (int idx = threadIdx.x; idx < F * E; idx += blockDim.x) {
-            const unsigned v = hD[idx];
-            if (v) atomicAdd(&Dl[idx], v);
+}
+
+// One CTA per (layer, family).  Sums the scratch slots of the layer into shared memory, then writes
+// the symmetric C rows, D and (layer 0) ntok.  ZERO: overwrite instead of accumulate.
+template <bool ZERO>
+__global__ void __launch_bounds__(512) coact_finalize_kernel(const HistParams p, unsigned* __restrict__ D,
+                                                            unsigned* __restrict__ C,
+                                                            unsigned long long* __restrict__ ntok) {
+    extern __shared__ __align__(16) unsigned fsm[];      // [tri] pair sums | [E] corr sums | [E] row sums
+    const int l = blockIdx.x / p.F, f = blockIdx.x % p.F;
+    const int E = p.E, tri = p.tri;
+    const int fgi = p.nfg > 1 ? f : 0;                   // which CTA of a group holds family f
+    const int fs = p.nfg > 1 ? 0 : f;                    // family index inside a slot
+    const int g0 = group_of_item((long long)l * p.cps, p.T, p.groups);
+    const int g1 = group_of_item((long long)(l + 1) * p.cps - 1, p.T, p.groups);
+    unsigned* scorr = fsm + tri;
+    unsigned* srow = scorr + E;
+    const unsigned* slot0 = p.scratch + ((size_t)(g0 + l) * p.nfg + fgi) * p.slot_words;
+    const size_t gstride = (size_t)p.nfg * p.slot_words;
+    for (int i = threadIdx.x; i < tri; i += blockDim.x) {
+        unsigned acc = 0;
+        for (int g = g0; g <= g1; ++g) acc += slot0[(size_t)(g - g0) * gstride + (size_t)fs * tri + i];
+        fsm[i] = acc;
+    }
+    for (int i = threadIdx.x; i < E; i += blockDim.x) {
+        unsigned acc = 0;
+        for (int g = g0; g <= g1; ++g)
+            acc += slot0[(size_t)(g - g0) * gstride + (size_t)p.Fs * tri + (size_t)fs * E + i];
+        scorr[i] = acc;
+    }
+    if (l == 0 && threadIdx.x == 0) {
+        unsigned long long acc = 0;
+        for (int g = g0; g <= g1; ++g) acc += slot0[(size_t)(g - g0) * gstride + (size_t)p.Fs * (tri + E) + fs];
+        ntok[f] = ZERO ? acc : ntok[f] + acc;
+    }
+    __syncthreads();
+    unsigned* Cf = C + ((size_t)l * p.F + f) * E * E;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
+    for (int i = warp; i < E; i += nwarps) {
+        unsigned rs = 0;
+        const int ri = tri_row(i, E);
+        for (int j = lane; j < E; j += 32) {
+            unsigned v = 0;
+            if (j > i) v = fsm[ri + j];
+            else if (j < i) v = fsm[tri_row(j, E) + i];
+            rs += v;
+            const size_t o = (size_t)i * E + j;
+            if (ZERO) Cf[o] = v;                         // the diagonal is cleared with the rest
+            else if (j != i) Cf[o] += v;
         }
-        for (int idx = threadIdx.x; idx < F * E * E; idx += blockDim.x) {
-            const int f = idx / (E * E);
-            const int rem = idx - f * E * E;
-            const int i = rem / E, j = rem - i * E;
-            if (i == j) continue;
-            const unsigned v = hsm[f * tri + tri_index(min(i, j), max(i, j), E)];
-            if (v) atomicAdd(&Cl[idx], v);
-        }
+        rs = __reduce_add_sync(0xffffffffu, rs);
+        if (lane == 0) srow[i] = rs;
+    }
+    __syncthreads();
+    const unsigned km1 = (unsigned)max(p.k - 1, 1);
+    unsigned* Df = D + ((size_t)l * p.F + f) * E;
+    for (int i = threadIdx.x; i < E; i += blockDim.x) {
+        const unsigned d = (srow[i] + scorr[i]) / km1;
+        Df[i] = ZERO ? d : Df[i] + d;
     }
 }
 
-__global__ void family_count_kernel(const int8_t* __restrict__ family, long long N, int F,
-                                    unsigned long long* __restrict__ ntok) {
-    __shared__ unsigned cnt[8];
-    if (threadIdx.x < 8) cnt[threadIdx.x] = 0u;
-    __syncthreads();
-    unsigned mine[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < N; t += stride) {
-        const int f = family[t];
-#pragma unroll
-        for (int g = 0; g < 8; ++g) mine[g] += (f == g) ? 1u : 0u;
-    }
-#pragma unroll
-    for (int g = 0; g < 8; ++g) {
-        const unsigned s = __reduce_add_sync(0xffffffffu, mine[g]);
-        if ((threadIdx.x & 31) == 0 && s && g < F) atomicAdd(&cnt[g], s);
-    }
-    __syncthreads();
-    if (threadIdx.x < F && cnt[threadIdx.x]) atomicAdd(&ntok[threadIdx.x], (unsigned long long)cnt[threadIdx.x]);
-}
-
-// errword[0] = 1 + smallest bad record id, errword[1] = kind of some bad record.
-__global__ void validate_trace_kernel(const int16_t* __restrict__ indices, const int8_t* __restrict__ family,
-                                      long long N, int k, int L, int E, int F, unsigned long long* err) {
+// Fallback: global atomics on D and C (any E <= 512).  The caller zeroes and counts ntok.
+__global__ void __launch_bounds__(512)
+coact_global_kernel(const int16_t* __restrict__ indices, const int8_t* __restrict__ family, long long N, int k, int L,
+                    int E, int F, unsigned* __restrict__ D, unsigned* __restrict__ C) {
     const long long total = (long long)L * N;
     const long long stride = (long long)gridDim.x * blockDim.x;
     for (long long rec = (long long)blockIdx.x * blockDim.x + threadIdx.x; rec < total; rec += stride) {
-        const long long t = rec % N;
-        int kind = 0;
+        const long long l = rec / N, t = rec - l * N;
         const int f = family[t];
-        if (f >= F) kind = 3;                                   // family out of range (negative = padding)
+        if ((unsigned)f >= (unsigned)F) continue;
         const int16_t* row = indices + (size_t)rec * k;
-        for (int a = 0; a < k && !kind; ++a) {
+        unsigned* Dl = D + ((size_t)l * F + f) * E;
+        unsigned* Cl = C + ((size_t)l * F + f) * E * E;
+        for (int a = 0; a < k; ++a) {
             const int i = row[a];
-            if (i < 0) continue;                                // empty slot
-            if (i >= E) { kind = 1; break; }                    // id out of range
-            for (int b = a + 1; b < k; ++b)
-                if (row[b] == i) { kind = 2; break; }           // duplicate inside a token
-        }
-        if (kind) {
-            atomicMin(err, (unsigned long long)rec + 1ull);
-            err[1] = (unsigned long long)kind;
-        }
-    }
-}
-
-__global__ void validate_placement_kernel(int L, int E, int P, int capacity, const int8_t* __restrict__ primary,
-                                          const int8_t* __restrict__ replicas, int r, unsigned long long* err) {
-    // one CTA per layer
-    __shared__ int count[64];
-    const int l = blockIdx.x;
-    if (threadIdx.x < 64) count[threadIdx.x] = 0;
-    __syncthreads();
-    for (int e = threadIdx.x; e < E; e += blockDim.x) {
-        const int m = primary[(size_t)l * E + e];
-        int kind = 0;
-        if (m < 0 || m >= P) kind = 1;
-        else atomicAdd(&count[m], 1);
-        if (!kind && replicas) {
-            for (int a = 0; a < r && !kind; ++a) {
-                const int c = replicas[((size_t)l * E + e) * r + a];
-                if (c < -1 || c >= P) kind = 3;
-                else if (c >= 0) {
-                    if (c == m) kind = 4;
-                    for (int b = a + 1; b < r; ++b)
-                        if (replicas[((size_t)l * E + e) * r + b] == c) kind = 5;
-                }
+            if ((unsigned)i >= (unsigned)E) continue;
+            atomicAdd(&Dl[i], 1u);
+            for (int b = a + 1; b < k; ++b) {
+                const int j = row[b];
+                if ((unsigned)j >= (unsigned)E || j == i) continue;
+                atomicAdd(&Cl[(size_t)i * E + j], 1u);
+                atomicAdd(&Cl[(size_t)j * E + i], 1u);
             }
         }
-        if (kind) {
-            atomicMin(err, (unsigned long long)((size_t)l * E + e) + 1ull);
-            err[1] = (unsigned long long)kind;
-        }
-    }
-    __syncthreads();
-    if (threadIdx.x < P && count[threadIdx.x] > capacity) {
-        atomicMin(err, (unsigned long long)((size_t)l * E) + 1ull);
-        err[1] = 2ull;                                          // partition over capacity
     }
 }
 
-constexpr unsigned long long kNoError = ~0ull;
-
-__global__ void errword_begin(unsigned long long* err) { err[0] = kNoError; err[1] = 0; }
-__global__ void errword_end(unsigned long long* err) { if (err[0] == kNoError) err[0] = 0; }
-
-template <int KT>
-int launch_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k, int L, int E, int F,
-                uint32_t* D, uint32_t* C) {
-    const size_t tri = (size_t)E * (E - 1) / 2;
-    const size_t smem = sizeof(unsigned) * (size_t)F * (tri + E);
-    const bool use_smem = smem <= (size_t)ctx->smem_optin - 1024;
-    // CTAs: about two waves of one CTA per SM when the histogram is large, more when small
-    const int per_sm = use_smem ? (int)max((size_t)1, min((size_t)4, ((size_t)ctx->smem_optin) / (smem + 1024))) : 4;
-    int cpl = max(1, (ctx->sm_count * per_sm) / L);
-    const long long blocks = (N + kHistThreads - 1) / kHistThreads;
-    if ((long long)cpl > blocks) cpl = (int)max(1ll, blocks);
-    const int grid = L * cpl;
-    tacg_prof_scope prof(ctx, TACG_PROF_COACT);
-    if (use_smem) {
-        auto kern = coact_hist_kernel<KT, true>;
-        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kern<<<grid, kHistThreads, smem, ctx->stream>>>(indices, family, (long long)N, k, L, E, F, cpl, D, C);
-    } else {
-        coact_hist_kernel<KT, false><<<grid, kHistThreads, 0, ctx->stream>>>(indices, family, (long long)N, k, L, E,
-                                                                            F, cpl, D, C);
-    }
+template <int KT, bool FILTER>
+int launch_hist(tacg_ctx* ctx, const HistParams& p, size_t smem, int grid) {
+    auto kern = coact_hist_kernel<KT, FILTER>;
+    TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    kern<<<grid, kThreads, smem, ctx->stream>>>(p);
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
+}
+
+template <bool FILTER>
+int launch_hist_k(tacg_ctx* ctx, const HistParams& p, size_t smem, int grid) {
+    switch (tacg_pick_kt(p.k, p.indices)) {
+        case 2: return launch_hist<2, FILTER>(ctx, p, smem, grid);
+        case 4: return launch_hist<4, FILTER>(ctx, p, smem, grid);
+        case 6: return launch_hist<6, FILTER>(ctx, p, smem, grid);
+        case 8: return launch_hist<8, FILTER>(ctx, p, smem, grid);
+        default: return launch_hist<0, FILTER>(ctx, p, smem, grid);
+    }
 }
 
 }  // namespace
 
 int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k, int L,
-                           int E, int F, uint32_t* D, uint32_t* C) {
-    switch (tacg_pick_kt(k, indices)) {
-        case 2: return launch_hist<2>(ctx, indices, family, N, k, L, E, F, D, C);
-        case 4: return launch_hist<4>(ctx, indices, family, N, k, L, E, F, D, C);
-        case 6: return launch_hist<6>(ctx, indices, family, N, k, L, E, F, D, C);
-        case 8: return launch_hist<8>(ctx, indices, family, N, k, L, E, F, D, C);
-        default: return launch_hist<0>(ctx, indices, family, N, k, L, E, F, D, C);
+                           int E, int F, uint32_t* D, uint32_t* C, uint64_t* ntok, bool zero_first) {
+    HistParams p;
+    p.indices = indices; p.family = family; p.N = N; p.k = k; p.L = L; p.E = E; p.F = F;
+    p.tri = E * (E - 1) / 2;
+    const size_t limit = (size_t)ctx->smem_optin;
+    const size_t all_words = tacg_align_up((size_t)F * (p.tri + E + 1), 4);
+    const size_t one_words = tacg_align_up((size_t)(p.tri + E + 1), 4);
+    const size_t queue_bytes = sizeof(unsigned) * kWarps * kQueue;
+    bool filter;
+    if (all_words * 4 <= limit) filter = false;
+    else if (one_words * 4 + queue_bytes <= limit && N < (1ll << 32)) filter = true;
+    else {
+        // neither layout fits: global atomics
+        if (zero_first) {
+            TACG_CUDA_TRY(ctx, cudaMemsetAsync(D, 0, sizeof(uint32_t) * (size_t)L * F * E, ctx->stream));
+            TACG_CUDA_TRY(ctx, cudaMemsetAsync(C, 0, sizeof(uint32_t) * (size_t)L * F * E * E, ctx->stream));
+            TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
+        }
+        int rc = tacg_launch_family_count(ctx, family, N, F, ntok);
+        if (rc != TACG_OK) return rc;
+        tacg_prof_scope prof(ctx, TACG_PROF_COACT);
+        coact_global_kernel<<<ctx->sm_count * 4, 512, 0, ctx->stream>>>(indices, family, (long long)N, k, L, E, F, D, C);
+        TACG_LAUNCH_CHECK(ctx);
+        return TACG_OK;
     }
-}
-
-int tacg_launch_family_count(tacg_ctx* ctx, const int8_t* family, int64_t N, int F, uint64_t* ntok) {
-    const int threads = 256;
-    long long want = (N + threads * 16 - 1) / (threads * 16);
-    const int grid = (int)max(1ll, min(want, (long long)ctx->sm_count * 4));
-    family_count_kernel<<<grid, threads, 0, ctx->stream>>>(family, (long long)N, F,
-                                                           reinterpret_cast<unsigned long long*>(ntok));
-    TACG_LAUNCH_CHECK(ctx);
-    return TACG_OK;
-}
-
-int tacg_launch_validate_trace(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k, int L,
-                               int E, int F) {
-    errword_begin<<<1, 1, 0, ctx->stream>>>(ctx->errword);
-    TACG_LAUNCH_CHECK(ctx);
-    const long long total = (long long)L * N;
-    const int grid = (int)max(1ll, min((total + 255) / 256, (long long)ctx->sm_count * 8));
-    validate_trace_kernel<<<grid, 256, 0, ctx->stream>>>(indices, family, (long long)N, k, L, E, F, ctx->errword);
-    TACG_LAUNCH_CHECK(ctx);
-    errword_end<<<1, 1, 0, ctx->stream>>>(ctx->errword);
-    TACG_LAUNCH_CHECK(ctx);
-    return TACG_OK;
-}
-
-int tacg_launch_validate_placement(tacg_ctx* ctx, int L, int E, int P, int capacity, const int8_t* primary,
-                                   const int8_t* replicas, int r) {
-    errword_begin<<<1, 1, 0, ctx->stream>>>(ctx->errword);
-    TACG_LAUNCH_CHECK(ctx);
-    validate_placement_kernel<<<L, 128, 0, ctx->stream>>>(L, E, P, capacity, primary, replicas, r, ctx->errword);
-    TACG_LAUNCH_CHECK(ctx);
-    errword_end<<<1, 1, 0, ctx->stream>>>(ctx->errword);
+    p.nfg = filter ? F : 1;
+    p.Fs = filter ? 1 : F;
+    p.slot_words = (int)(filter ? one_words : all_words);
+    p.chunk = filter ? 4096 : 1024;
+    p.cps = (int)((N + p.chunk - 1) / p.chunk);
+    p.T = (long long)L * p.cps;
+    p.groups = (int)max(1ll, min((long long)(ctx->sm_count / p.nfg), p.T));
+    const size_t slots = (size_t)(p.groups + L - 1) * p.nfg;
+    p.scratch = static_cast<unsigned*>(tacg_scratch(ctx, slots * p.slot_words * sizeof(unsigned)));
+    if (!p.scratch) return TACG_ERR_CUDA;
+    const size_t smem = (size_t)p.slot_words * 4 + (filter ? queue_bytes : 0);
+    const int grid = p.groups * p.nfg;
+    tacg_prof_scope prof(ctx, TACG_PROF_COACT);
+    int rc = filter ? launch_hist_k<true>(ctx, p, smem, grid) : launch_hist_k<false>(ctx, p, smem, grid);
+    if (rc != TACG_OK) return rc;
+    const size_t fsmem = sizeof(unsigned) * ((size_t)p.tri + 2 * E);
+    unsigned long long* nt = reinterpret_cast<unsigned long long*>(ntok);
+    if (zero_first) {
+        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(coact_finalize_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem));
+        coact_finalize_kernel<true><<<L * F, 512, fsmem, ctx->stream>>>(p, D, C, nt);
+    } else {
+        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(coact_finalize_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem));
+        coact_finalize_kernel<false><<<L * F, 512, fsmem, ctx->stream>>>(p, D, C, nt);
+    }
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }

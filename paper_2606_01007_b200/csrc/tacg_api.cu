@@ -167,22 +167,23 @@ int tacg_coact_accumulate(tacg_ctx* ctx, const int16_t* indices, const int8_t* f
         rc = read_errword(ctx, TACG_ERR_BAD_INDEX, "coact validate (record = layer*N + token)");
         if (rc != TACG_OK) return rc;
     }
-    if (flags & TACG_ZERO_FIRST) {
+    // Path choice (DESIGN.md "Path choice"): the tensor path where it is supported, else the histogram.
+    const bool use_mma = N > 0 && ((path == TACG_PATH_MMA) || (path == TACG_PATH_AUTO && mma_ok));
+    const bool zero_first = (flags & TACG_ZERO_FIRST) != 0;
+    if (zero_first && (N == 0 || use_mma)) {
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(D, 0, sizeof(uint32_t) * (size_t)L * F * E, ctx->stream));
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(C, 0, sizeof(uint32_t) * (size_t)L * F * E * E, ctx->stream));
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
     }
     if (N == 0) return TACG_OK;
-    int rc = tacg_launch_family_count(ctx, family, N, F, ntok);
-    if (rc != TACG_OK) return rc;
-    // Path choice (DESIGN.md "Path choice"): the tensor path where it is supported, else the histogram.
-    const bool use_mma = (path == TACG_PATH_MMA) || (path == TACG_PATH_AUTO && mma_ok);
     if (use_mma) {
+        int rc = tacg_launch_family_count(ctx, family, N, F, ntok);
+        if (rc != TACG_OK) return rc;
         ctx->last_path = TACG_PATH_MMA;
         return tacg_launch_coact_mma(ctx, indices, family, N, k, L, E, F, D, C);
     }
     ctx->last_path = TACG_PATH_HIST;
-    return tacg_launch_coact_hist(ctx, indices, family, N, k, L, E, F, D, C);
+    return tacg_launch_coact_hist(ctx, indices, family, N, k, L, E, F, D, C, ntok, zero_first);
 }
 
 int tacg_affinity_swapgain(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L, int E,

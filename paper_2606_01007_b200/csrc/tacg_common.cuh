@@ -73,8 +73,9 @@ int tacg_launch_validate_trace(tacg_ctx* ctx, const int16_t* indices, const int8
                                int k, int L, int E, int F);
 int tacg_launch_validate_placement(tacg_ctx* ctx, int L, int E, int P, int capacity,
                                    const int8_t* primary, const int8_t* replicas, int r);
+// Counts D, C and ntok (all three); zero_first = overwrite instead of accumulate.
 int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k,
-                           int L, int E, int F, uint32_t* D, uint32_t* C);
+                           int L, int E, int F, uint32_t* D, uint32_t* C, uint64_t* ntok, bool zero_first);
 bool tacg_coact_mma_supported(int k, int E, int F);
 int tacg_launch_coact_mma(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k,
                           int L, int E, int F, uint32_t* D, uint32_t* C);
