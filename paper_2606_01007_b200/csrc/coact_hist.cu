@@ -24,6 +24,8 @@ namespace {
 
 constexpr int kThreads = 1024;           // one CTA per SM
 constexpr int kWarps = kThreads / 32;
+constexpr int kBatch = 4;                 // tokens per thread whose loads are issued together
+constexpr int kRun = 4;                   // items (of kThreads tokens) walked together
 constexpr int kQueue = 160;              // per-warp token queue of the family-filter mode (<= 31 + 128 entries)
 
 struct HistParams {
@@ -104,31 +106,62 @@ __device__ __forceinline__ void slow_token(const int (&e)[KMAX], int k, int E, u
     }
 }
 
-// One token of a family whose triangle starts at hist (corr = its correction counters).
+// Raw 32-bit words of one token row (two ids per word); KT in {2,4,6,8}, base 16-byte aligned.
+template <int KT>
+__device__ __forceinline__ void load_raw(const int16_t* __restrict__ row, unsigned (&w)[KT / 2]) {
+    if constexpr (KT == 8) {
+        const uint4 v = __ldg(reinterpret_cast<const uint4*>(row));
+        w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+    } else if constexpr (KT == 4) {
+        const uint2 v = __ldg(reinterpret_cast<const uint2*>(row));
+        w[0] = v.x; w[1] = v.y;
+    } else {
+#pragma unroll
+        for (int i = 0; i < KT / 2; ++i) w[i] = __ldg(reinterpret_cast<const unsigned*>(row) + i);
+    }
+}
+
+// One token (KT ids packed in w) of a family whose triangle starts at hist (corr = its correction counters).
+template <int KT>
+__device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E, unsigned* hist, unsigned* corr) {
+    int e[KT], s[KT];
+#pragma unroll
+    for (int i = 0; i < KT / 2; ++i) {
+        e[2 * i] = (int)(short)(w[i] & 0xffffu);
+        e[2 * i + 1] = (int)w[i] >> 16;
+    }
+#pragma unroll
+    for (int a = 0; a < KT; ++a) s[a] = e[a];
+    sort_ids<KT>(s);
+    bool fast = s[0] >= 0 && s[KT - 1] < E;
+#pragma unroll
+    for (int a = 0; a + 1 < KT; ++a) fast = fast && (s[a] != s[a + 1]);
+    if (fast) {
+#pragma unroll
+        for (int a = 0; a + 1 < KT; ++a) {
+            unsigned* rowp = hist + tri_row(s[a], E);
+#pragma unroll
+            for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b], 1u);
+        }
+        return;
+    }
+    slow_token<KT>(e, KT, E, hist, corr);
+}
+
+// One token, any k: compile-time KT uses the packed path, KT == 0 reads k ids one by one.
 template <int KT>
 __device__ __forceinline__ void count_token(const int16_t* __restrict__ row, int k, int E, unsigned* hist,
                                             unsigned* corr) {
-    int e[KT > 0 ? KT : 16];
-    tacg_load_ids<KT>(row, k, e);
     if constexpr (KT >= 2) {
-        int s[KT];
+        unsigned w[KT / 2];
+        load_raw<KT>(row, w);
+        count_packed<KT>(w, E, hist, corr);
+    } else {
+        int e[16];
 #pragma unroll
-        for (int a = 0; a < KT; ++a) s[a] = e[a];
-        sort_ids<KT>(s);
-        bool fast = s[0] >= 0 && s[KT - 1] < E;
-#pragma unroll
-        for (int a = 0; a + 1 < KT; ++a) fast = fast && (s[a] != s[a + 1]);
-        if (fast) {
-#pragma unroll
-            for (int a = 0; a + 1 < KT; ++a) {
-                unsigned* rowp = hist + tri_row(s[a], E);
-#pragma unroll
-                for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b], 1u);
-            }
-            return;
-        }
+        for (int j = 0; j < 16; ++j) e[j] = (j < k) ? (int)__ldg(row + j) : -1;
+        slow_token<16>(e, k, E, hist, corr);
     }
-    slow_token<(KT > 0 ? KT : 16)>(e, KT > 0 ? KT : k, E, hist, corr);
 }
 
 // smem layout (words): [Fs][tri] pair bins | [Fs][E] corr | [Fs] ntok (layer 0 only) | pad to slot_words
@@ -154,9 +187,15 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
     int qn = 0;                         // warp-uniform
     const int lane = tid & 31;
 
+    // Items are walked in runs of up to kRun consecutive items of one layer, so that a thread has
+    // kBatch tokens in flight while group boundaries stay at the finer item granularity.
     int layer = (int)(lo / p.cps);
-    for (long long item = lo; item <= hi; ++item) {
-        const int l = item < hi ? (int)(item / p.cps) : -1;
+    int ci = (int)(lo - (long long)layer * p.cps);          // item inside the layer
+    int l = layer;
+    long long item = lo;
+    for (;;) {
+        if (ci == p.cps) { ci = 0; ++l; }
+        if (item == hi) l = -1;
         if (l != layer) {
             const int16_t* lbase = p.indices + (size_t)layer * (size_t)p.N * k;
             if (FILTER) {               // drain the partial queue of this layer
@@ -174,15 +213,41 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             if (l < 0) break;
             layer = l;
         }
-        const long long t0 = (item - (long long)l * p.cps) * p.chunk;
-        const long long t1 = min(p.N, t0 + p.chunk);
+        const int run = (int)min((long long)min(kRun, p.cps - ci), hi - item);
+        const long long t0 = (long long)ci * p.chunk;
+        const long long t1 = min(p.N, t0 + (long long)run * p.chunk);
+        ci += run;
+        item += run;
         const int16_t* lbase = p.indices + (size_t)l * (size_t)p.N * k;
         if (!FILTER) {
-            for (long long t = t0 + tid; t < t1; t += kThreads) {
-                const int f = p.family[t];
-                if ((unsigned)f >= (unsigned)p.F) continue;     // padding token
-                if (l == 0) atomicAdd(&sntok[f], 1u);
-                count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm + (size_t)f * p.tri, corr + f * p.E);
+            if constexpr (KT >= 2) {
+                // kBatch tokens per thread with all their loads in flight before the first increment
+                for (long long tb = t0 + tid; tb < t1; tb += (long long)kThreads * kBatch) {
+                    int f[kBatch];
+                    unsigned w[kBatch][KT / 2];
+#pragma unroll
+                    for (int u = 0; u < kBatch; ++u) {
+                        const long long t = tb + (long long)u * kThreads;
+                        f[u] = -1;
+                        if (t < t1) {
+                            f[u] = p.family[t];
+                            load_raw<KT>(lbase + (size_t)t * KT, w[u]);
+                        }
+                    }
+#pragma unroll
+                    for (int u = 0; u < kBatch; ++u) {
+                        if ((unsigned)f[u] >= (unsigned)p.F) continue;      // padding token / past the end
+                        if (l == 0) atomicAdd(&sntok[f[u]], 1u);
+                        count_packed<KT>(w[u], p.E, hsm + (size_t)f[u] * p.tri, corr + f[u] * p.E);
+                    }
+                }
+            } else {
+                for (long long t = t0 + tid; t < t1; t += kThreads) {
+                    const int f = p.family[t];
+                    if ((unsigned)f >= (unsigned)p.F) continue;     // padding token
+                    if (l == 0) atomicAdd(&sntok[f], 1u);
+                    count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm + (size_t)f * p.tri, corr + f * p.E);
+                }
             }
         } else {
             // each thread scans 4 consecutive tokens per step; a warp covers 128
@@ -235,10 +300,19 @@ __global__ void __launch_bounds__(512) coact_finalize_kernel(const HistParams p,
     unsigned* srow = scorr + E;
     const unsigned* slot0 = p.scratch + ((size_t)(g0 + l) * p.nfg + fgi) * p.slot_words;
     const size_t gstride = (size_t)p.nfg * p.slot_words;
+    const int ng = g1 - g0 + 1;
     for (int i = threadIdx.x; i < tri; i += blockDim.x) {
-        unsigned acc = 0;
-        for (int g = g0; g <= g1; ++g) acc += slot0[(size_t)(g - g0) * gstride + (size_t)fs * tri + i];
-        fsm[i] = acc;
+        const unsigned* src = slot0 + (size_t)fs * tri + i;
+        unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0;
+        int g = 0;
+        for (; g + 4 <= ng; g += 4) {
+            a0 += src[(size_t)g * gstride];
+            a1 += src[(size_t)(g + 1) * gstride];
+            a2 += src[(size_t)(g + 2) * gstride];
+            a3 += src[(size_t)(g + 3) * gstride];
+        }
+        for (; g < ng; ++g) a0 += src[(size_t)g * gstride];
+        fsm[i] = (a0 + a1) + (a2 + a3);
     }
     for (int i = threadIdx.x; i < E; i += blockDim.x) {
         unsigned acc = 0;
@@ -356,7 +430,7 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     p.nfg = filter ? F : 1;
     p.Fs = filter ? 1 : F;
     p.slot_words = (int)(filter ? one_words : all_words);
-    p.chunk = filter ? 4096 : 1024;
+    p.chunk = kThreads;
     p.cps = (int)((N + p.chunk - 1) / p.chunk);
     p.T = (long long)L * p.cps;
     p.groups = (int)max(1ll, min((long long)(ctx->sm_count / p.nfg), p.T));
