@@ -10,93 +10,45 @@
 // applies Eq. 15 redundantly from the same integers (same fp64 operations => the same bits),
 // so no CTA ever reads another CTA's floating-point state.  The kernel is launched
 // cooperatively whenever CTAs wait on one another.
+//
+// The pick rule of Q17 orders candidates by (not local, snapshot load, candidate slot).  Only the
+// first key depends on the token, so once per micro-batch each replicated expert's feasible
+// candidates are sorted by (snapshot load, slot) into a small table; a token then takes the first
+// entry that is local to it (in its accessed set R or its home), else the first entry.  That is
+// the same argmin, with all fp64 comparisons hoisted out of the token loop.
 #include <cooperative_groups.h>
 
 #include "tacg_common.cuh"
 
 namespace {
 
-constexpr int kEvalThreads = 256;
+constexpr int kEvalThreads = 512;
+constexpr int kEvalBatch = 4;        // tokens per thread with their loads in flight together
+constexpr int kCandStride = 12;      // bytes per expert in the candidate table: [0] = count, [1..9] = partitions
+constexpr unsigned kRepFlag = 0x80u; // ptab bit: the expert has at least one replica
 
-struct LayerTables {        // per-layer lookup tables in shared memory
-    unsigned short* info;   // [E] low byte = primary partition, high byte = number of valid replicas
-    signed char* rep;       // [E*r] replica partitions, -1 = none
-    double* S;              // [64] load snapshot
-    unsigned long long feas;  // bit m = S[m] <= (1+theta)*mean(S)
+struct LayerTables {
+    unsigned char* ptab;   // [E] primary partition | kRepFlag
+    unsigned char* cand;   // [E][kCandStride] sorted feasible candidates of replicated experts
+    signed char* rep;      // [E*r] replica partitions as given, -1 = none
+    double* S;             // [64] load snapshot
 };
 
-// Step 4 of O10 for one token: serve[j] per slot (-1 = empty), returns the accessed set R.
-template <int KT>
-__device__ __forceinline__ unsigned long long
-select_token(const int (&e)[KT > 0 ? KT : 16], int k, int E, int r, int home, const unsigned short* __restrict__ info,
-             const signed char* __restrict__ rep, const double* __restrict__ S, unsigned long long feas,
-             int (&sv)[KT > 0 ? KT : 16]) {
-    constexpr int KM = KT > 0 ? KT : 16;
-    unsigned long long R = 0ull;
-    unsigned pending = 0u;
-    // pass 1: experts with a single candidate are served by their primary regardless (Q18)
-#pragma unroll
-    for (int j = 0; j < KM; ++j) {
-        sv[j] = -1;
-        if (j < k && (unsigned)e[j] < (unsigned)E) {
-            const unsigned in = info[e[j]];
-            if ((in >> 8) == 0u) {
-                sv[j] = (int)(in & 63u);
-                R |= 1ull << (in & 63u);
-            } else {
-                pending |= 1u << j;
-            }
-        }
-    }
-    // pass 2: replicated experts in slot order; key (not local, snapshot load, candidate slot) (Q17)
-    if (pending) {
-#pragma unroll
-        for (int j = 0; j < KM; ++j) {
-            if (!((pending >> j) & 1u)) continue;
-            const int ex = e[j];
-            const int c0 = (int)(info[ex] & 63u);
-            unsigned long long cmask = 1ull << c0;
-            for (int a = 0; a < r; ++a) {
-                const int c = rep[ex * r + a];
-                if (c >= 0) cmask |= 1ull << (c & 63);
-            }
-            const bool anyfeas = (cmask & feas) != 0ull;       // else: fallback to all candidates
-            int best = -1, bestloc = 0;
-            double bestS = 0.0;
-            for (int a = -1; a < r; ++a) {
-                const int c = a < 0 ? c0 : (int)rep[ex * r + a];
-                if (c < 0) continue;
-                const int cm = c & 63;
-                if (anyfeas && !((feas >> cm) & 1ull)) continue;
-                const int nonlocal = (((R >> cm) & 1ull) || cm == home) ? 0 : 1;
-                const double s = S[cm];
-                if (best < 0 || nonlocal < bestloc || (nonlocal == bestloc && s < bestS)) {
-                    best = cm; bestloc = nonlocal; bestS = s;
-                }
-            }
-            sv[j] = best;
-            R |= 1ull << best;
-        }
-    }
-    return R;
-}
-
 __device__ __forceinline__ void load_tables(int E, int r, const int8_t* __restrict__ pr,
-                                            const int8_t* __restrict__ rp, unsigned short* info, signed char* rep) {
+                                            const int8_t* __restrict__ rp, const LayerTables& T) {
     for (int e = threadIdx.x; e < E; e += blockDim.x) {
         unsigned n = 0;
         for (int a = 0; a < r; ++a) {
             const signed char c = rp[(size_t)e * r + a];
-            rep[e * r + a] = c;
+            T.rep[e * r + a] = c;
             n += (c >= 0) ? 1u : 0u;
         }
-        info[e] = (unsigned short)(((unsigned)pr[e] & 63u) | (n << 8));
+        T.ptab[e] = (unsigned char)(((unsigned)pr[e] & 63u) | (n ? kRepFlag : 0u));
     }
 }
 
 // feas from a snapshot: mean summed left to right in double (Q19), theta widened from float.
-__device__ __forceinline__ void load_guard(const double* S, int P, float theta, unsigned long long* feas_out) {
-    // called by one thread
+__device__ __forceinline__ unsigned long long load_guard(const double* S, int P, float theta) {
     double tot = 0.0;
     for (int m = 0; m < P; ++m) tot = __dadd_rn(tot, S[m]);
     const double Lbar = tot / (double)P;
@@ -104,7 +56,80 @@ __device__ __forceinline__ void load_guard(const double* S, int P, float theta, 
     unsigned long long fm = 0ull;
     for (int m = 0; m < P; ++m)
         if (S[m] <= thr) fm |= 1ull << m;
-    *feas_out = fm;
+    return fm;
+}
+
+// Candidate table of one snapshot: for every replicated expert the candidates (primary, then
+// replicas in slot order), restricted to the feasible ones unless none is (fallback,
+// PAPER.md:155), stably sorted by snapshot load (strict <, so ties keep slot order).
+__device__ __forceinline__ void build_candidates(int E, int r, const LayerTables& T, unsigned long long feas) {
+    for (int e = threadIdx.x; e < E; e += blockDim.x) {
+        const unsigned in = T.ptab[e];
+        if (!(in & kRepFlag)) continue;
+        int c[9];
+        int n = 0;
+        c[n++] = (int)(in & 63u);
+        for (int a = 0; a < r; ++a) {
+            const int v = T.rep[e * r + a];
+            if (v >= 0) c[n++] = v & 63;
+        }
+        unsigned long long cmask = 0ull;
+        for (int i = 0; i < n; ++i) cmask |= 1ull << c[i];
+        const bool anyfeas = (cmask & feas) != 0ull;
+        int m = 0;
+        unsigned char* out = T.cand + e * kCandStride;
+        for (int i = 0; i < n; ++i) {
+            if (anyfeas && !((feas >> c[i]) & 1ull)) continue;
+            // insertion: after every entry whose load is <= this one's
+            const double s = T.S[c[i]];
+            int pos = m;
+            while (pos > 0 && s < T.S[out[pos]]) { out[pos + 1] = out[pos]; --pos; }
+            out[pos + 1] = (unsigned char)c[i];
+            ++m;
+        }
+        out[0] = (unsigned char)m;
+    }
+}
+
+// Step 4 of O10 for one token: serve[j] per slot (-1 = empty), returns the accessed set R.
+template <int KM>
+__device__ __forceinline__ unsigned long long serve_token(const int (&e)[KM], int k, int E, int home,
+                                                          const LayerTables& T, int (&sv)[KM]) {
+    unsigned long long R = 0ull;
+    unsigned pending = 0u;
+    // pass 1: experts with a single candidate are served by their primary regardless (Q18)
+#pragma unroll
+    for (int j = 0; j < KM; ++j) {
+        sv[j] = -1;
+        if (j < k && (unsigned)e[j] < (unsigned)E) {
+            const unsigned in = T.ptab[e[j]];
+            if (!(in & kRepFlag)) {
+                sv[j] = (int)in;
+                R |= 1ull << in;
+            } else {
+                pending |= 1u << j;
+            }
+        }
+    }
+    // pass 2: replicated experts in slot order; first local candidate of the sorted table, else the first
+    if (pending) {
+        const unsigned long long hb = 1ull << home;
+#pragma unroll
+        for (int j = 0; j < KM; ++j) {
+            if (!((pending >> j) & 1u)) continue;
+            const unsigned char* c = T.cand + e[j] * kCandStride;
+            const int n = c[0];
+            int pick = c[1];
+            const unsigned long long loc = R | hb;
+            for (int i = 1; i <= n; ++i) {
+                const int v = c[i];
+                if ((loc >> v) & 1ull) { pick = v; break; }
+            }
+            sv[j] = pick;
+            R |= 1ull << pick;
+        }
+    }
+    return R;
 }
 
 struct EvalParams {
@@ -131,16 +156,56 @@ struct EvalParams {
     int groups;             // number of concurrent layer groups = gridDim.x / cpl
 };
 
+__host__ __device__ inline size_t eval_align16(size_t x) { return (x + 15) & ~(size_t)15; }
+
+// carves the per-layer tables out of dynamic shared memory; returns the bytes used
+__device__ __forceinline__ size_t carve_tables(unsigned char* base, int E, int r, LayerTables& T) {
+    size_t off = 0;
+    T.S = reinterpret_cast<double*>(base + off);            off += 64 * sizeof(double);
+    T.ptab = base + off;                                    off += eval_align16((size_t)E);
+    T.cand = base + off;                                    off += eval_align16((size_t)E * kCandStride);
+    T.rep = reinterpret_cast<signed char*>(base + off);     off += eval_align16((size_t)E * (r > 0 ? r : 1));
+    return off;
+}
+
+size_t tables_bytes(int E, int r) {
+    return 64 * sizeof(double) + eval_align16((size_t)E) + eval_align16((size_t)E * kCandStride) +
+           eval_align16((size_t)E * (r > 0 ? r : 1));
+}
+
 template <int KT>
-__global__ void __launch_bounds__(kEvalThreads)
+__device__ __forceinline__ void unpack_ids(const unsigned (&w)[KT / 2], int (&e)[KT]) {
+#pragma unroll
+    for (int i = 0; i < KT / 2; ++i) {
+        e[2 * i] = (int)(short)(w[i] & 0xffffu);
+        e[2 * i + 1] = (int)w[i] >> 16;
+    }
+}
+
+template <int KT>
+__device__ __forceinline__ void load_row_raw(const int16_t* __restrict__ row, unsigned (&w)[KT / 2]) {
+    if constexpr (KT == 8) {
+        const uint4 v = __ldg(reinterpret_cast<const uint4*>(row));
+        w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+    } else if constexpr (KT == 4) {
+        const uint2 v = __ldg(reinterpret_cast<const uint2*>(row));
+        w[0] = v.x; w[1] = v.y;
+    } else {
+#pragma unroll
+        for (int i = 0; i < KT / 2; ++i) w[i] = __ldg(reinterpret_cast<const unsigned*>(row) + i);
+    }
+}
+
+template <int KT>
+__global__ void __launch_bounds__(kEvalThreads, 2)
 eval_kernel(EvalParams p) {
-    extern __shared__ unsigned char esm[];
-    // layout: S[64] double | cnt[P][32] u32 | dsum[64] u64 | info[E] u16 | rep[E*r] i8
-    double* S = reinterpret_cast<double*>(esm);
-    unsigned* cnt = reinterpret_cast<unsigned*>(esm + 64 * sizeof(double));
-    unsigned long long* dsum = reinterpret_cast<unsigned long long*>(cnt + (size_t)p.P * 32);
-    unsigned short* info = reinterpret_cast<unsigned short*>(dsum + 64);
-    signed char* rep = reinterpret_cast<signed char*>(info + ((p.E + 3) & ~3));
+    extern __shared__ __align__(16) unsigned char esm[];
+    constexpr int KM = KT > 0 ? KT : 16;
+    constexpr int U = KT > 0 ? kEvalBatch : 1;
+    LayerTables T;
+    size_t off = carve_tables(esm, p.E, p.r, T);
+    unsigned long long* dsum = reinterpret_cast<unsigned long long*>(esm + off);   off += 64 * sizeof(unsigned long long);
+    unsigned* cnt = reinterpret_cast<unsigned*>(esm + off);                        // [P][32], lane-private columns
     __shared__ double Ls[64];              // EMA state of this layer
     __shared__ unsigned long long ltot[64];  // cumulative integer load of this layer
     __shared__ unsigned long long feas_s;
@@ -149,32 +214,51 @@ eval_kernel(EvalParams p) {
     const int group = blockIdx.x / p.cpl;
     const int part = blockIdx.x % p.cpl;
     if (group >= p.groups) return;
-    const int lane = threadIdx.x & 31;
-    const int P = p.P, k = p.k, E = p.E, F = p.F, r = p.r;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int P = p.P, k = KT > 0 ? KT : p.k, E = p.E, F = p.F, r = p.r;
+    const int stepP = kEvalThreads % P;
 
     for (int layer = group; layer < p.L; layer += p.groups) {
         __syncthreads();
-        load_tables(E, r, p.primary + (size_t)layer * E, p.replicas ? p.replicas + (size_t)layer * E * r : nullptr,
-                    info, rep);
-        for (int i = threadIdx.x; i < P * 32; i += blockDim.x) cnt[i] = 0u;
-        if (threadIdx.x < 64) {
-            Ls[threadIdx.x] = (p.load_state && threadIdx.x < P) ? p.load_state[(size_t)layer * P + threadIdx.x] : 0.0;
-            ltot[threadIdx.x] = 0ull;
+        load_tables(E, r, p.primary + (size_t)layer * E, p.replicas ? p.replicas + (size_t)layer * E * r : nullptr, T);
+        for (int i = tid; i < P * 32; i += kEvalThreads) cnt[i] = 0u;
+        if (tid < 64) {
+            Ls[tid] = (p.load_state && tid < P) ? p.load_state[(size_t)layer * P + tid] : 0.0;
+            ltot[tid] = 0ull;
         }
-        if (threadIdx.x < 16) comm_s[threadIdx.x] = 0ull;
+        if (tid < 16) comm_s[tid] = 0ull;
         __syncthreads();
-        unsigned long long span_acc[8], rem_acc[8];   // lane 0 of each warp accumulates per family
+        unsigned acc[8];                    // per family: sum of span | remote << 16 over this thread's tokens
 #pragma unroll
-        for (int f = 0; f < 8; ++f) { span_acc[f] = 0ull; rem_acc[f] = 0ull; }
+        for (int g = 0; g < 8; ++g) acc[g] = 0u;
+        int since = 0;                      // tokens added to acc since the last flush (uniform per warp)
+        auto flush_acc = [&]() {
+#pragma unroll
+            for (int g = 0; g < 8; ++g) {
+                if (g < F) {
+                    const unsigned s = __reduce_add_sync(0xffffffffu, acc[g] & 0xffffu);
+                    const unsigned q = __reduce_add_sync(0xffffffffu, acc[g] >> 16);
+                    if (lane == 0) {
+                        if (s) atomicAdd(&comm_s[g], (unsigned long long)s);
+                        if (q) atomicAdd(&comm_s[8 + g], (unsigned long long)q);
+                    }
+                    acc[g] = 0u;
+                }
+            }
+            since = 0;
+        };
         const int16_t* base = p.indices + (size_t)layer * (size_t)p.N * (size_t)k;
 
         for (long long mb = 0; mb < p.nmb; ++mb) {
-            // steps 1-3: snapshot and guard
-            if (threadIdx.x < 64) S[threadIdx.x] = Ls[threadIdx.x];
+            // steps 1-3: snapshot, guard, candidate tables
+            if (tid < 64) T.S[tid] = Ls[tid];
             __syncthreads();
-            if (threadIdx.x == 0) load_guard(S, P, p.theta, &feas_s);
-            __syncthreads();
-            const unsigned long long feas = feas_s;
+            if (r > 0) {
+                if (tid == 0) feas_s = load_guard(T.S, P, p.theta);
+                __syncthreads();
+                build_candidates(E, r, T, feas_s);
+                __syncthreads();
+            }
             // step 4: this CTA's slice of the micro-batch
             const long long mb_begin = mb * p.B;
             const long long mb_end = min(p.N, mb_begin + p.B);
@@ -182,47 +266,63 @@ eval_kernel(EvalParams p) {
             const long long per = ((len + p.cpl - 1) / p.cpl + 31) / 32 * 32;
             const long long t0 = mb_begin + (long long)part * per;
             const long long t1 = min(mb_end, t0 + per);
-            for (long long tb = t0; tb < t1; tb += kEvalThreads) {
-                const long long t = tb + threadIdx.x;
-                int f = -1;
-                if (t < t1) f = p.family[t];
-                const bool live = (unsigned)f < (unsigned)F;
-                int packed = 0;
-                if (live) {
-                    int e[KT > 0 ? KT : 16], sv[KT > 0 ? KT : 16];
-                    tacg_load_ids<KT>(base + (size_t)t * k, k, e);
-                    const int home = (int)((p.token_offset + t) % P);
-                    const unsigned long long R = select_token<KT>(e, k, E, r, home, info, rep, S, feas, sv);
+            int home = (int)((p.token_offset + t0 + tid) % P);
+            for (long long tb = t0; tb < t1; tb += (long long)kEvalThreads * U) {
+                int f[U];
+                unsigned w[U][KT > 0 ? KT / 2 : 1];
 #pragma unroll
-                    for (int j = 0; j < (KT > 0 ? KT : 16); ++j)
-                        if (j < k && sv[j] >= 0) atomicAdd(&cnt[sv[j] * 32 + lane], 1u);
-                    const int nR = __popcll(R);
-                    const int rem = __popcll(R & ~(1ull << home));
-                    packed = max(0, nR - 1) | (rem << 16);
-                    if (p.cost) p.cost[(size_t)layer * p.N + t] = (unsigned char)rem;
-                    if (p.serve) {
-#pragma unroll
-                        for (int j = 0; j < (KT > 0 ? KT : 16); ++j)
-                            if (j < k) p.serve[((size_t)layer * p.N + t) * k + j] = (signed char)sv[j];
-                    }
-                } else if (t < t1) {
-                    if (p.cost) p.cost[(size_t)layer * p.N + t] = 0;
-                    if (p.serve)
-                        for (int j = 0; j < k; ++j) p.serve[((size_t)layer * p.N + t) * k + j] = -1;
-                }
-                // per-family communication sums: one warp reduction per family (span | remote<<16)
-#pragma unroll
-                for (int g = 0; g < 8; ++g) {
-                    if (g < F) {
-                        const unsigned s = __reduce_add_sync(0xffffffffu, (unsigned)((live && f == g) ? packed : 0));
-                        span_acc[g] += s & 0xffffu;
-                        rem_acc[g] += s >> 16;
+                for (int u = 0; u < U; ++u) {
+                    const long long t = tb + (long long)u * kEvalThreads + tid;
+                    f[u] = -1;
+                    if (t < t1) {
+                        f[u] = p.family[t];
+                        if constexpr (KT > 0) load_row_raw<KT>(base + (size_t)t * KT, w[u]);
                     }
                 }
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const long long t = tb + (long long)u * kEvalThreads + tid;
+                    const bool live = (unsigned)f[u] < (unsigned)F;
+                    unsigned packed = 0;
+                    if (live) {
+                        int e[KM], sv[KM];
+                        if constexpr (KT > 0) {
+                            unpack_ids<KT>(w[u], e);
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < 16; ++j) e[j] = (j < k) ? (int)__ldg(base + (size_t)t * k + j) : -1;
+                        }
+                        const unsigned long long R = serve_token<KM>(e, k, E, home, T, sv);
+#pragma unroll
+                        for (int j = 0; j < KM; ++j)
+                            if (j < k && sv[j] >= 0) atomicAdd(&cnt[sv[j] * 32 + lane], 1u);
+                        const int nR = __popcll(R);
+                        const int rem = __popcll(R & ~(1ull << home));
+                        packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
+                        if (p.cost) p.cost[(size_t)layer * p.N + t] = (unsigned char)rem;
+                        if (p.serve) {
+#pragma unroll
+                            for (int j = 0; j < KM; ++j)
+                                if (j < k) p.serve[((size_t)layer * p.N + t) * k + j] = (signed char)sv[j];
+                        }
+                    } else if (t < t1) {
+                        if (p.cost) p.cost[(size_t)layer * p.N + t] = 0;
+                        if (p.serve)
+                            for (int j = 0; j < k; ++j) p.serve[((size_t)layer * p.N + t) * k + j] = -1;
+                    }
+#pragma unroll
+                    for (int g = 0; g < 8; ++g)
+                        if (g < F) acc[g] += (f[u] == g) ? packed : 0u;
+                    home += stepP;
+                    if (home >= P) home -= P;
+                }
+                since += U;
+                if (since >= 3800) flush_acc();
             }
+            flush_acc();
             // step 5: integer dispatch counts of the micro-batch, then Eq. 15
             __syncthreads();
-            for (int m = threadIdx.x >> 5; m < P; m += kEvalThreads / 32) {
+            for (int m = tid >> 5; m < P; m += kEvalThreads / 32) {
                 const unsigned s = __reduce_add_sync(0xffffffffu, cnt[m * 32 + lane]);
                 cnt[m * 32 + lane] = 0u;
                 if (lane == 0) dsum[m] = (unsigned long long)s;
@@ -230,10 +330,10 @@ eval_kernel(EvalParams p) {
             __syncthreads();
             if (p.cpl > 1) {
                 unsigned long long* dl = p.delta + ((size_t)layer * p.nmb + mb) * P;
-                if (threadIdx.x < P && dsum[threadIdx.x]) atomicAdd(&dl[threadIdx.x], dsum[threadIdx.x]);
+                if (tid < P && dsum[tid]) atomicAdd(&dl[tid], dsum[tid]);
                 __threadfence();
                 __syncthreads();
-                if (threadIdx.x == 0) {
+                if (tid == 0) {
                     atomicAdd(&p.barrier[layer], 1u);
                     const unsigned target = (unsigned)((mb + 1) * p.cpl);
                     volatile unsigned* bar = p.barrier + layer;
@@ -241,34 +341,24 @@ eval_kernel(EvalParams p) {
                     __threadfence();
                 }
                 __syncthreads();
-                if (threadIdx.x < P) dsum[threadIdx.x] = __ldcg(&dl[threadIdx.x]);
+                if (tid < P) dsum[tid] = __ldcg(&dl[tid]);
                 __syncthreads();
             }
-            if (threadIdx.x < P) {
-                const unsigned long long d = dsum[threadIdx.x];
-                Ls[threadIdx.x] = __dadd_rn(__dmul_rn(p.rho, Ls[threadIdx.x]), (double)d);   // no FMA (Q19)
-                ltot[threadIdx.x] += d;
+            if (tid < P) {
+                const unsigned long long d = dsum[tid];
+                Ls[tid] = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
+                ltot[tid] += d;
             }
             __syncthreads();
         }
         // layer epilogue: communication sums and, from part 0, loads and the final state
-        if (lane == 0) {
-#pragma unroll
-            for (int g = 0; g < 8; ++g) {
-                if (g < F) {
-                    if (span_acc[g]) atomicAdd(&comm_s[g], span_acc[g]);
-                    if (rem_acc[g]) atomicAdd(&comm_s[8 + g], rem_acc[g]);
-                }
-            }
+        if (tid < F) {
+            if (comm_s[tid]) atomicAdd(&p.comm_span[(size_t)layer * F + tid], comm_s[tid]);
+            if (comm_s[8 + tid]) atomicAdd(&p.comm_remote[(size_t)layer * F + tid], comm_s[8 + tid]);
         }
-        __syncthreads();
-        if (threadIdx.x < F) {
-            if (comm_s[threadIdx.x]) atomicAdd(&p.comm_span[(size_t)layer * F + threadIdx.x], comm_s[threadIdx.x]);
-            if (comm_s[8 + threadIdx.x]) atomicAdd(&p.comm_remote[(size_t)layer * F + threadIdx.x], comm_s[8 + threadIdx.x]);
-        }
-        if (part == 0 && threadIdx.x < P) {
-            p.load[(size_t)layer * P + threadIdx.x] = ltot[threadIdx.x];
-            if (p.load_state) p.load_state[(size_t)layer * P + threadIdx.x] = Ls[threadIdx.x];
+        if (part == 0 && tid < P) {
+            p.load[(size_t)layer * P + tid] = ltot[tid];
+            if (p.load_state) p.load_state[(size_t)layer * P + tid] = Ls[tid];
         }
     }
 }
@@ -312,25 +402,26 @@ __global__ void __launch_bounds__(kEvalThreads)
 select_kernel(const int16_t* __restrict__ indices, long long N, int k, int E, int P, int r,
               const int8_t* __restrict__ primary, const int8_t* __restrict__ replicas,
               const double* __restrict__ snapshot, float theta, long long token_offset, signed char* __restrict__ serve) {
-    extern __shared__ unsigned char ssm[];
-    double* S = reinterpret_cast<double*>(ssm);
-    unsigned short* info = reinterpret_cast<unsigned short*>(ssm + 64 * sizeof(double));
-    signed char* rep = reinterpret_cast<signed char*>(info + ((E + 3) & ~3));
+    extern __shared__ __align__(16) unsigned char ssm[];
+    constexpr int KM = KT > 0 ? KT : 16;
+    LayerTables T;
+    carve_tables(ssm, E, r, T);
     __shared__ unsigned long long feas_s;
     const int layer = blockIdx.y;
-    load_tables(E, r, primary + (size_t)layer * E, replicas ? replicas + (size_t)layer * E * r : nullptr, info, rep);
-    if (threadIdx.x < 64) S[threadIdx.x] = threadIdx.x < P ? snapshot[(size_t)layer * P + threadIdx.x] : 0.0;
+    load_tables(E, r, primary + (size_t)layer * E, replicas ? replicas + (size_t)layer * E * r : nullptr, T);
+    if (threadIdx.x < 64) T.S[threadIdx.x] = threadIdx.x < P ? snapshot[(size_t)layer * P + threadIdx.x] : 0.0;
     __syncthreads();
-    if (threadIdx.x == 0) load_guard(S, P, theta, &feas_s);
+    if (threadIdx.x == 0) feas_s = load_guard(T.S, P, theta);
     __syncthreads();
-    const unsigned long long feas = feas_s;
+    build_candidates(E, r, T, feas_s);
+    __syncthreads();
     const int16_t* base = indices + (size_t)layer * (size_t)N * (size_t)k;
     const long long stride = (long long)gridDim.x * kEvalThreads;
     for (long long t = (long long)blockIdx.x * kEvalThreads + threadIdx.x; t < N; t += stride) {
-        int e[KT > 0 ? KT : 16], sv[KT > 0 ? KT : 16];
+        int e[KM], sv[KM];
         tacg_load_ids<KT>(base + (size_t)t * k, k, e);
         const int home = (int)((token_offset + t) % P);
-        select_token<KT>(e, k, E, r, home, info, rep, S, feas, sv);
+        serve_token<KM>(e, k, E, home, T, sv);
         signed char* out = serve + ((size_t)layer * N + t) * k;
         if constexpr (KT == 8) {
             int2 v;
@@ -339,15 +430,14 @@ select_kernel(const int16_t* __restrict__ indices, long long N, int k, int E, in
             *reinterpret_cast<int2*>(out) = v;
         } else {
 #pragma unroll
-            for (int j = 0; j < (KT > 0 ? KT : 16); ++j)
+            for (int j = 0; j < KM; ++j)
                 if (j < k) out[j] = (signed char)sv[j];
         }
     }
 }
 
 size_t eval_smem_bytes(int E, int P, int r) {
-    return 64 * sizeof(double) + sizeof(unsigned) * (size_t)P * 32 + 64 * sizeof(unsigned long long) +
-           sizeof(unsigned short) * (size_t)((E + 3) & ~3) + (size_t)E * (r > 0 ? r : 1) + 16;
+    return tables_bytes(E, r) + 64 * sizeof(unsigned long long) + sizeof(unsigned) * (size_t)P * 32;
 }
 
 template <int KT>
@@ -391,8 +481,7 @@ template <int KT>
 int launch_select_t(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P,
                     const int8_t* primary, const int8_t* replicas, int r, const double* snapshot, float theta,
                     int64_t token_offset, int8_t* serve) {
-    const size_t smem = 64 * sizeof(double) + sizeof(unsigned short) * (size_t)((E + 3) & ~3) +
-                        (size_t)E * (r > 0 ? r : 1) + 16;
+    const size_t smem = tables_bytes(E, r);
     const long long blocks = (N + kEvalThreads - 1) / kEvalThreads;
     const int gx = (int)max(1ll, min(blocks, (long long)max(1, ctx->sm_count * 8 / L)));
     select_kernel<KT><<<dim3(gx, L), kEvalThreads, smem, ctx->stream>>>(
