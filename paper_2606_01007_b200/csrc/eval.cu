@@ -91,11 +91,58 @@ __device__ __forceinline__ void build_candidates(int E, int r, const LayerTables
     }
 }
 
+// Pass 2 of the selection: replicated experts (bits of `pending`) in slot order; each takes the first
+// local candidate of its sorted table, else the first, and joins R.
+template <int KM, typename M>
+__device__ __forceinline__ M serve_pending(const int (&e)[KM], unsigned pending, int home, M R, const LayerTables& T,
+                                           int (&sv)[KM]) {
+    const M hb = (M)1 << home;
+#pragma unroll
+    for (int j = 0; j < KM; ++j) {
+        if (!((pending >> j) & 1u)) continue;
+        const unsigned char* c = T.cand + e[j] * kCandStride;
+        const int n = c[0];
+        int pick = c[1];
+        const M loc = R | hb;
+        for (int i = 1; i <= n; ++i) {
+            const int v = c[i];
+            if ((loc >> v) & (M)1) { pick = v; break; }
+        }
+        sv[j] = pick;
+        R |= (M)1 << pick;
+    }
+    return R;
+}
+
+// All KM slots hold valid ids: pass 1 without branches.
+template <int KM, bool REP, typename M>
+__device__ __forceinline__ M serve_fast(const int (&e)[KM], int home, const LayerTables& T, int (&sv)[KM]) {
+    M R = 0;
+    unsigned pending = 0u;
+#pragma unroll
+    for (int j = 0; j < KM; ++j) {
+        const unsigned in = T.ptab[e[j]];
+        if constexpr (REP) {
+            const unsigned isrep = in >> 7;
+            sv[j] = (int)(in & 63u);
+            R |= (M)(isrep ^ 1u) << (in & 63u);
+            pending |= isrep << j;
+        } else {
+            sv[j] = (int)in;
+            R |= (M)1 << in;
+        }
+    }
+    if constexpr (REP) {
+        if (pending) R = serve_pending<KM, M>(e, pending, home, R, T, sv);
+    }
+    return R;
+}
+
 // Step 4 of O10 for one token: serve[j] per slot (-1 = empty), returns the accessed set R.
-template <int KM>
-__device__ __forceinline__ unsigned long long serve_token(const int (&e)[KM], int k, int E, int home,
-                                                          const LayerTables& T, int (&sv)[KM]) {
-    unsigned long long R = 0ull;
+template <int KM, typename M = unsigned long long>
+__device__ __forceinline__ M serve_token(const int (&e)[KM], int k, int E, int home, const LayerTables& T,
+                                         int (&sv)[KM]) {
+    M R = 0;
     unsigned pending = 0u;
     // pass 1: experts with a single candidate are served by their primary regardless (Q18)
 #pragma unroll
@@ -105,7 +152,7 @@ __device__ __forceinline__ unsigned long long serve_token(const int (&e)[KM], in
             const unsigned in = T.ptab[e[j]];
             if (!(in & kRepFlag)) {
                 sv[j] = (int)in;
-                R |= 1ull << in;
+                R |= (M)1 << in;
             } else {
                 pending |= 1u << j;
             }
@@ -113,21 +160,7 @@ __device__ __forceinline__ unsigned long long serve_token(const int (&e)[KM], in
     }
     // pass 2: replicated experts in slot order; first local candidate of the sorted table, else the first
     if (pending) {
-        const unsigned long long hb = 1ull << home;
-#pragma unroll
-        for (int j = 0; j < KM; ++j) {
-            if (!((pending >> j) & 1u)) continue;
-            const unsigned char* c = T.cand + e[j] * kCandStride;
-            const int n = c[0];
-            int pick = c[1];
-            const unsigned long long loc = R | hb;
-            for (int i = 1; i <= n; ++i) {
-                const int v = c[i];
-                if ((loc >> v) & 1ull) { pick = v; break; }
-            }
-            sv[j] = pick;
-            R |= 1ull << pick;
-        }
+        R = serve_pending<KM, M>(e, pending, home, R, T, sv);
     }
     return R;
 }
@@ -196,7 +229,9 @@ __device__ __forceinline__ void load_row_raw(const int16_t* __restrict__ row, un
     }
 }
 
-template <int KT>
+// KT: compile-time k (0 = generic), REP: a replica table is present, M: partition-set mask type
+// (unsigned for P <= 32, else unsigned long long).
+template <int KT, bool REP, typename M>
 __global__ void __launch_bounds__(kEvalThreads, 2)
 eval_kernel(EvalParams p) {
     extern __shared__ __align__(16) unsigned char esm[];
@@ -215,12 +250,13 @@ eval_kernel(EvalParams p) {
     const int part = blockIdx.x % p.cpl;
     if (group >= p.groups) return;
     const int tid = threadIdx.x, lane = tid & 31;
-    const int P = p.P, k = KT > 0 ? KT : p.k, E = p.E, F = p.F, r = p.r;
+    const int P = p.P, k = KT > 0 ? KT : p.k, E = p.E, F = p.F, r = REP ? p.r : 0;
     const int stepP = kEvalThreads % P;
+    unsigned* cnt_lane = cnt + lane;
 
     for (int layer = group; layer < p.L; layer += p.groups) {
         __syncthreads();
-        load_tables(E, r, p.primary + (size_t)layer * E, p.replicas ? p.replicas + (size_t)layer * E * r : nullptr, T);
+        load_tables(E, r, p.primary + (size_t)layer * E, REP ? p.replicas + (size_t)layer * E * r : nullptr, T);
         for (int i = tid; i < P * 32; i += kEvalThreads) cnt[i] = 0u;
         if (tid < 64) {
             Ls[tid] = (p.load_state && tid < P) ? p.load_state[(size_t)layer * P + tid] : 0.0;
@@ -248,12 +284,14 @@ eval_kernel(EvalParams p) {
             since = 0;
         };
         const int16_t* base = p.indices + (size_t)layer * (size_t)p.N * (size_t)k;
+        unsigned char* cost_l = p.cost ? p.cost + (size_t)layer * p.N : nullptr;
+        signed char* serve_l = p.serve ? p.serve + (size_t)layer * p.N * k : nullptr;
 
         for (long long mb = 0; mb < p.nmb; ++mb) {
             // steps 1-3: snapshot, guard, candidate tables
-            if (tid < 64) T.S[tid] = Ls[tid];
-            __syncthreads();
-            if (r > 0) {
+            if (REP) {
+                if (tid < 64) T.S[tid] = Ls[tid];
+                __syncthreads();
                 if (tid == 0) feas_s = load_guard(T.S, P, p.theta);
                 __syncthreads();
                 build_candidates(E, r, T, feas_s);
@@ -266,49 +304,77 @@ eval_kernel(EvalParams p) {
             const long long per = ((len + p.cpl - 1) / p.cpl + 31) / 32 * 32;
             const long long t0 = mb_begin + (long long)part * per;
             const long long t1 = min(mb_end, t0 + per);
+            const int n = t1 > t0 ? (int)(t1 - t0) : 0;            // tokens of the slice (per <= 2^31 checked on the host)
             int home = (int)((p.token_offset + t0 + tid) % P);
-            for (long long tb = t0; tb < t1; tb += (long long)kEvalThreads * U) {
+            const int8_t* fam0 = p.family + t0;
+            const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
+            for (int ob = tid; ob < n + tid; ob += kEvalThreads * U) {      // uniform trip count across the CTA
                 int f[U];
                 unsigned w[U][KT > 0 ? KT / 2 : 1];
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
-                    const long long t = tb + (long long)u * kEvalThreads + tid;
+                    const int o = ob + u * kEvalThreads;
                     f[u] = -1;
-                    if (t < t1) {
-                        f[u] = p.family[t];
-                        if constexpr (KT > 0) load_row_raw<KT>(base + (size_t)t * KT, w[u]);
+                    if (o < n) {
+                        f[u] = fam0[o];
+                        if constexpr (KT == 8) {
+                            const uint4 v = __ldg(reinterpret_cast<const uint4*>(rows0) + o);
+                            w[u][0] = v.x; w[u][1] = v.y; w[u][2] = v.z; w[u][3] = v.w;
+                        } else if constexpr (KT == 4) {
+                            const uint2 v = __ldg(reinterpret_cast<const uint2*>(rows0) + o);
+                            w[u][0] = v.x; w[u][1] = v.y;
+                        } else if constexpr (KT > 0) {
+#pragma unroll
+                            for (int i = 0; i < KT / 2; ++i) w[u][i] = __ldg(rows0 + o * (KT / 2) + i);
+                        }
                     }
                 }
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
-                    const long long t = tb + (long long)u * kEvalThreads + tid;
+                    const int o = ob + u * kEvalThreads;
                     const bool live = (unsigned)f[u] < (unsigned)F;
                     unsigned packed = 0;
                     if (live) {
                         int e[KM], sv[KM];
+                        M R;
+                        bool fast = false;
                         if constexpr (KT > 0) {
                             unpack_ids<KT>(w[u], e);
+                            int lo = e[0], hi = e[0];
+#pragma unroll
+                            for (int j = 1; j < KT; ++j) { lo = min(lo, e[j]); hi = max(hi, e[j]); }
+                            fast = lo >= 0 && hi < E;
                         } else {
 #pragma unroll
-                            for (int j = 0; j < 16; ++j) e[j] = (j < k) ? (int)__ldg(base + (size_t)t * k + j) : -1;
+                            for (int j = 0; j < 16; ++j)
+                                e[j] = (j < k) ? (int)__ldg(base + ((size_t)t0 + o) * k + j) : -1;
                         }
-                        const unsigned long long R = serve_token<KM>(e, k, E, home, T, sv);
+                        if (fast) {
+                            R = serve_fast<KM, REP, M>(e, home, T, sv);
 #pragma unroll
-                        for (int j = 0; j < KM; ++j)
-                            if (j < k && sv[j] >= 0) atomicAdd(&cnt[sv[j] * 32 + lane], 1u);
-                        const int nR = __popcll(R);
-                        const int rem = __popcll(R & ~(1ull << home));
-                        packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
-                        if (p.cost) p.cost[(size_t)layer * p.N + t] = (unsigned char)rem;
-                        if (p.serve) {
+                            for (int j = 0; j < KM; ++j) atomicAdd(cnt_lane + sv[j] * 32, 1u);
+                        } else {
+                            R = serve_token<KM, M>(e, k, E, home, T, sv);
 #pragma unroll
                             for (int j = 0; j < KM; ++j)
-                                if (j < k) p.serve[((size_t)layer * p.N + t) * k + j] = (signed char)sv[j];
+                                if (j < k && sv[j] >= 0) atomicAdd(cnt_lane + sv[j] * 32, 1u);
                         }
-                    } else if (t < t1) {
-                        if (p.cost) p.cost[(size_t)layer * p.N + t] = 0;
-                        if (p.serve)
-                            for (int j = 0; j < k; ++j) p.serve[((size_t)layer * p.N + t) * k + j] = -1;
+                        const M notHome = ~((M)1 << home);
+                        int nR, rem;
+                        if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
+                        else { nR = __popc(R); rem = __popc(R & notHome); }
+                        packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
+                        if (cost_l) cost_l[t0 + o] = (unsigned char)rem;
+                        if (serve_l) {
+                            signed char* out = serve_l + ((size_t)t0 + o) * k;
+#pragma unroll
+                            for (int j = 0; j < KM; ++j)
+                                if (j < k) out[j] = (signed char)sv[j];
+                        }
+                    } else if (o < n) {
+                        if (cost_l) cost_l[t0 + o] = 0;
+                        if (serve_l)
+                            for (int j = 0; j < k; ++j) serve_l[((size_t)t0 + o) * k + j] = -1;
                     }
 #pragma unroll
                     for (int g = 0; g < 8; ++g)
@@ -443,7 +509,10 @@ size_t eval_smem_bytes(int E, int P, int r) {
 template <int KT>
 int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     const size_t smem = eval_smem_bytes(p.E, p.P, p.r);
-    auto kern = eval_kernel<KT>;
+    const bool rep = p.replicas != nullptr && p.r > 0;
+    void (*kern)(EvalParams) =
+        p.P <= 32 ? (rep ? eval_kernel<KT, true, unsigned> : eval_kernel<KT, false, unsigned>)
+                  : (rep ? eval_kernel<KT, true, unsigned long long> : eval_kernel<KT, false, unsigned long long>);
     int occ = 0;
     TACG_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kEvalThreads, smem));
     if (occ < 1) occ = 1;
@@ -453,6 +522,10 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     const long long slices = max(1ll, (min(p.B, p.N) + 2 * kEvalThreads - 1) / (2 * kEvalThreads));
     if (cpl > slices) cpl = slices;
     p.cpl = (int)cpl;
+    if ((min(p.B, p.N) + cpl - 1) / cpl + 32 > 0x7fffffffll) {
+        snprintf(ctx->detail, sizeof(ctx->detail), "eval: more than 2^31 tokens per CTA slice");
+        return TACG_ERR_SHAPE;
+    }
     p.groups = (int)min((long long)p.L, (long long)max_grid / cpl);
     const int grid = p.groups * p.cpl;
     const bool waits = p.cpl > 1 && p.nmb > 1;     // CTAs of a group meet at a barrier per micro-batch
