@@ -111,6 +111,15 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic(config, path):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the co-activation kernel(s), per launch, from the
+    committed ncu --set full capture (profiles/traffic.json, written by hand from the .ncu-rep); None if absent."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))[f"config{config}_{path}"]["bytes"]
+    except Exception:
+        return None
+
+
 def coact_algorithmic_bytes(cfg):
     """indices read once + family once + D and C written once."""
     return cfg.L * cfg.N * cfg.k * 2 + cfg.N + cfg.L * cfg.F * (cfg.E * cfg.E + cfg.E) * 4
@@ -329,7 +338,7 @@ def main():
     used_path = {tacg.TACG_PATH_HIST: "hist", tacg.TACG_PATH_MMA: "mma"}.get(ctx.last_path(), "?")
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-        "traffic": None, "kernel": f"coact_{used_path}_kernel", "peak_source": peak_src,
+        "traffic": ncu_traffic(args.config, used_path), "kernel": f"coact_{used_path}_kernel", "peak_source": peak_src,
         "algorithmic_bytes_per_launch": abytes, "avg_launch_ms": co_avg_ms, "launches_timed": co_n,
         "coact_routed_tokens_per_s": cfg.L * cfg.N / (co_avg_ms * 1e-3) if co_avg_ms > 0 else 0.0,
         "other_kernels_avg_ms": {"affinity_swapgain(4 kernels)": af_ms / max(1, af_n), "eval_kernel": ev_ms / max(1, ev_n)},
@@ -368,10 +377,13 @@ def main():
         bi, bf, ei, ef = (x.cpu().numpy() for x in sets[0])
         Ls, threads = oracle_sample_layers(cbind, cfg, bi, bf, ei, ef, primary_np, replicas_np, 10.0)
         t0 = time.perf_counter()
-        units = oracle_step(cbind, cfg, bi, bf, ei, ef, primary_np, replicas_np, Ls)
+        units, reps = 0, 0
+        while reps == 0 or time.perf_counter() - t0 < 10.0:        # about 10 s of CPU work
+            units += oracle_step(cbind, cfg, bi, bf, ei, ef, primary_np, replicas_np, Ls)
+            reps += 1
         dt = time.perf_counter() - t0
         cpu_baseline = {"value": units / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-                        "sample": f"one step on the first {Ls} of {cfg.L} layers, all tokens ({dt:.1f} s)"}
+                        "sample": f"{reps} step(s) on the first {Ls} of {cfg.L} layers, all tokens ({dt:.1f} s)"}
 
     if rank == 0:
         line = {

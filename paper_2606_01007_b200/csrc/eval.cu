@@ -97,19 +97,46 @@ template <int KM, typename M>
 __device__ __forceinline__ M serve_pending(const int (&e)[KM], unsigned pending, int home, M R, const LayerTables& T,
                                            int (&sv)[KM]) {
     const M hb = (M)1 << home;
+    if constexpr (KM <= 8) {
+        // Each lane walks its own set bits (lowest first = slot order), so a warp runs for the
+        // largest number of replicated slots any of its tokens has, not for all KM slots.
+        unsigned long long picks = 0ull;
+        unsigned todo = pending;
+        while (todo) {
+            const int j = __ffs(todo) - 1;
+            todo &= todo - 1u;
+            int ex = e[0];
 #pragma unroll
-    for (int j = 0; j < KM; ++j) {
-        if (!((pending >> j) & 1u)) continue;
-        const unsigned char* c = T.cand + e[j] * kCandStride;
-        const int n = c[0];
-        int pick = c[1];
-        const M loc = R | hb;
-        for (int i = 1; i <= n; ++i) {
-            const int v = c[i];
-            if ((loc >> v) & (M)1) { pick = v; break; }
+            for (int q = 1; q < KM; ++q) ex = (j == q) ? e[q] : ex;
+            const unsigned char* c = T.cand + ex * kCandStride;
+            const int n = c[0];
+            int pick = c[1];
+            const M loc = R | hb;
+            for (int i = 1; i <= n; ++i) {
+                const int v = c[i];
+                if ((loc >> v) & (M)1) { pick = v; break; }
+            }
+            picks |= (unsigned long long)pick << (8 * j);
+            R |= (M)1 << pick;
         }
-        sv[j] = pick;
-        R |= (M)1 << pick;
+#pragma unroll
+        for (int j = 0; j < KM; ++j)
+            if ((pending >> j) & 1u) sv[j] = (int)((picks >> (8 * j)) & 0xffull);
+    } else {
+#pragma unroll
+        for (int j = 0; j < KM; ++j) {
+            if (!((pending >> j) & 1u)) continue;
+            const unsigned char* c = T.cand + e[j] * kCandStride;
+            const int n = c[0];
+            int pick = c[1];
+            const M loc = R | hb;
+            for (int i = 1; i <= n; ++i) {
+                const int v = c[i];
+                if ((loc >> v) & (M)1) { pick = v; break; }
+            }
+            sv[j] = pick;
+            R |= (M)1 << pick;
+        }
     }
     return R;
 }

@@ -1,0 +1,96 @@
+"""Parity at BASELINE.json's full per-layer sizes, in the launch configuration bench.py times
+(same flags, same micro-batch, traces generated on the device exactly as bench.py does).
+
+The C oracle finishes these in seconds, so every output is compared element by element:
+config 2 whole; configs 3 and 4 at the full token count per layer on a subset of layers (layers are
+independent problems, Q22, and the library's grid split changes with L, so two values of
+L are used for config 3); config 5 whole.  Invariants that hold at any size (north_star) are
+checked on the GPU result itself.
+"""
+import numpy as np
+import pytest
+import torch
+
+import tracegen
+from oracle import cbind
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def tacg():
+    import paper_2606_01007_b200 as t
+    return t
+
+
+@pytest.fixture(scope="module")
+def ctx(tacg):
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    c = tacg.Context(0)
+    yield c
+    c.close()
+
+
+def _u32(t):
+    return t.cpu().numpy().view(np.uint32)
+
+
+def _u64(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+def _device_trace(cfg_id, L, eval_trace):
+    cfg = tracegen.get_config(cfg_id)
+    cfg = tracegen.scaled(cfg, L=min(cfg.L, L))
+    params = tracegen.make_params(cfg)
+    idx, fam = tracegen.gen_trace(cfg, params, eval_trace=eval_trace, device="cuda", seed=cfg.seed + 17)
+    return cfg, idx, fam
+
+
+def _check_invariants(cfg, N, D, C, ntok):
+    """north_star: C symmetric with zero diagonal; sum_e D[f,:] = k*N_f; sum_{i<j} C = N k(k-1)/2."""
+    assert (C == C.transpose(0, 1, 3, 2)).all()
+    assert (np.diagonal(C, axis1=2, axis2=3) == 0).all()
+    assert int(ntok.sum()) == N
+    k = cfg.k
+    assert (D.sum(axis=2, dtype=np.uint64) == (k * ntok)[None, :]).all()
+    assert (C.sum(axis=(2, 3), dtype=np.uint64) == (k * (k - 1) * ntok)[None, :]).all()
+
+
+@pytest.mark.parametrize("cfg_id,L", [(2, 26), (3, 5), (3, 2), (4, 2), (5, 1)])
+def test_coact_full_size(tacg, ctx, cfg_id, L):
+    cfg, idx, fam = _device_trace(cfg_id, L, eval_trace=False)
+    out = tacg.tacg_coact_accumulate(ctx, idx, fam, cfg.E, cfg.F, flags=tacg.TACG_ZERO_FIRST | tacg.TACG_PATH_AUTO)
+    torch.cuda.synchronize()
+    D, C, ntok = _u32(out["D"]), _u32(out["C"]), _u64(out["ntok"])
+    _check_invariants(cfg, cfg.N, D, C, ntok)
+    wD, wC, wn = cbind.coact(idx.cpu().numpy(), fam.cpu().numpy(), cfg.E, cfg.F)
+    assert (ntok == wn).all()
+    assert (D == wD).all()
+    assert (C == wC).all()
+
+
+@pytest.mark.parametrize("cfg_id,L", [(2, 26), (3, 4), (4, 2), (5, 1)])
+def test_eval_full_size(tacg, ctx, cfg_id, L):
+    cfg, idx, fam = _device_trace(cfg_id, L, eval_trace=True)
+    primary = tracegen.random_placement(cfg.E, cfg.P, cfg.capacity, cfg.L, seed=cfg.seed)
+    replicas = tracegen.random_replicas(primary, cfg.P, cfg.r, cfg.n_rep, seed=cfg.seed + 1) if cfg.r else None
+    st = torch.zeros((cfg.L, cfg.P), dtype=torch.float64, device="cuda")
+    got = tacg.tacg_eval_placement(ctx, idx, fam, cfg.E, cfg.F, cfg.P, torch.from_numpy(primary).cuda(),
+                                   None if replicas is None else torch.from_numpy(replicas).cuda(), theta=0.15,
+                                   rho=0.995, microbatch=cfg.microbatch, load_state=st, want_cost=True)
+    torch.cuda.synchronize()
+    want = cbind.eval_placement(idx.cpu().numpy(), fam.cpu().numpy(), cfg.E, cfg.F, cfg.P, primary, replicas,
+                                theta=0.15, rho=0.995, microbatch=cfg.microbatch,
+                                load_state=np.zeros((cfg.L, cfg.P)), want_cost=True)
+    assert (_u64(got["load"]) == want["load"]).all()
+    assert (_u64(got["comm_span"]) == want["comm_span"]).all()
+    assert (_u64(got["comm_remote"]) == want["comm_remote"]).all()
+    assert (_u64(got["ntok"]) == want["ntok"]).all()
+    assert (got["cost"].cpu().numpy() == want["cost"]).all()
+    assert (st.cpu().numpy().view(np.uint64) == want["load_state"].view(np.uint64)).all()
+    assert np.allclose(got["fairness"].cpu().numpy().astype(np.float64), want["fairness"], rtol=1e-5, atol=1e-7)
+    # any size: every dispatch is served by exactly one partition; Jain in [1/P, 1]
+    assert (_u64(got["load"]).sum(axis=1) == np.uint64(cfg.N_eval * cfg.k)).all()
+    jain = got["fairness"][:, 0].cpu().numpy()
+    assert ((jain >= 1.0 / cfg.P - 1e-6) & (jain <= 1.0 + 1e-6)).all()
