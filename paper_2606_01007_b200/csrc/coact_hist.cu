@@ -44,17 +44,6 @@ struct HistParams {
     int slot_words;     // Fs*(tri+E+1) rounded up to 4
 };
 
-__host__ __device__ __forceinline__ long long group_lo(long long g, long long T, int groups) { return g * T / groups; }
-
-// the group that owns item x
-__device__ __forceinline__ int group_of_item(long long x, long long T, int groups) {
-    int g = (int)((x * groups) / T);
-    if (g >= groups) g = groups - 1;
-    while (g + 1 < groups && group_lo(g + 1, T, groups) <= x) ++g;
-    while (g > 0 && group_lo(g, T, groups) > x) --g;
-    return g;
-}
-
 // R(i) + j is the bin of the pair i < j in a row-major strict upper triangle of an E x E matrix:
 // R(i) = i(2E-1-i)/2 - i - 1 = i(2E-3-i)/2 - 1 (the product is always even).
 __device__ __forceinline__ int tri_row(int i, int E) { return ((i * (2 * E - 3 - i)) >> 1) - 1; }

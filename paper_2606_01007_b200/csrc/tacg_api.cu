@@ -159,7 +159,7 @@ int tacg_coact_accumulate(tacg_ctx* ctx, const int16_t* indices, const int8_t* f
     if (path == TACG_PATH_MASK) return fail(ctx, TACG_ERR_SHAPE, "coact: both TACG_PATH_HIST and TACG_PATH_MMA set");
     const bool mma_ok = tacg_coact_mma_supported(k, E, F) && (reinterpret_cast<uintptr_t>(indices) % 16) == 0;
     if (path == TACG_PATH_MMA && !mma_ok)
-        return fail(ctx, TACG_ERR_SHAPE, "coact: TACG_PATH_MMA needs E%16==0, E<=128, F*E<=512, 16-byte aligned indices");
+        return fail(ctx, TACG_ERR_SHAPE, "coact: TACG_PATH_MMA needs k in {2,4,6,8}, E<=128, F*Epad<=512 (Epad = 64 or 128), 16-byte aligned indices");
     TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     if ((flags & TACG_VALIDATE) && N > 0) {
         int rc = tacg_launch_validate_trace(ctx, indices, family, N, k, L, E, F);
@@ -170,17 +170,15 @@ int tacg_coact_accumulate(tacg_ctx* ctx, const int16_t* indices, const int8_t* f
     // Path choice: the tensor path where it is supported, else the histogram.
     const bool use_mma = N > 0 && ((path == TACG_PATH_MMA) || (path == TACG_PATH_AUTO && mma_ok));
     const bool zero_first = (flags & TACG_ZERO_FIRST) != 0;
-    if (zero_first && (N == 0 || use_mma)) {
+    if (zero_first && N == 0) {
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(D, 0, sizeof(uint32_t) * (size_t)L * F * E, ctx->stream));
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(C, 0, sizeof(uint32_t) * (size_t)L * F * E * E, ctx->stream));
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
     }
     if (N == 0) return TACG_OK;
     if (use_mma) {
-        int rc = tacg_launch_family_count(ctx, family, N, F, ntok);
-        if (rc != TACG_OK) return rc;
         ctx->last_path = TACG_PATH_MMA;
-        return tacg_launch_coact_mma(ctx, indices, family, N, k, L, E, F, D, C);
+        return tacg_launch_coact_mma(ctx, indices, family, N, k, L, E, F, D, C, ntok, zero_first);
     }
     ctx->last_path = TACG_PATH_HIST;
     return tacg_launch_coact_hist(ctx, indices, family, N, k, L, E, F, D, C, ntok, zero_first);

@@ -78,7 +78,7 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
                            int L, int E, int F, uint32_t* D, uint32_t* C, uint64_t* ntok, bool zero_first);
 bool tacg_coact_mma_supported(int k, int E, int F);
 int tacg_launch_coact_mma(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k,
-                          int L, int E, int F, uint32_t* D, uint32_t* C);
+                          int L, int E, int F, uint32_t* D, uint32_t* C, uint64_t* ntok, bool zero_first);
 int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L,
                          int E, int F, int P, const int8_t* primary, double alpha, double tau, double eps,
                          float* pref, float* W, float* aff, float* gain);
@@ -93,6 +93,20 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
 
 // ---- device helpers ----
 #ifdef __CUDACC__
+// Static work split of the co-activation kernels: T items (layer-major) over `groups` CTA groups;
+// group g owns items [g*T/groups, (g+1)*T/groups) and writes one scratch slot per layer it visits.
+__host__ __device__ __forceinline__ long long group_lo(long long g, long long T, int groups) { return g * T / groups; }
+
+// the group that owns item x
+__device__ __forceinline__ int group_of_item(long long x, long long T, int groups) {
+    int g = (int)((x * groups) / T);
+    if (g >= groups) g = groups - 1;
+    while (g + 1 < groups && group_lo(g + 1, T, groups) <= x) ++g;
+    while (g > 0 && group_lo(g, T, groups) > x) --g;
+    return g;
+}
+
+
 // Loads the KT expert ids of one token row.  KT in {2,4,6,8}: vector loads (the host
 // checked the base alignment); KT == 0: k runtime, 2-byte loads.
 template <int KT>
