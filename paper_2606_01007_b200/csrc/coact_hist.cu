@@ -78,7 +78,7 @@ __device__ __forceinline__ void sort_ids(int (&e)[K]) {
 // Any token: every slot is checked.  For each valid slot a, cnt = number of pair increments the
 // slot takes part in; the correction counter receives (k-1) - cnt so that
 // (pair bins touching e) + corr[e] = (k-1) * (valid slots holding e)   holds exactly.
-template <int KMAX>
+template <int KMAX, int CP = 1>
 __device__ __forceinline__ void slow_token(const int (&e)[KMAX], int k, int E, unsigned* hist, unsigned* corr) {
     const int km1 = max(k - 1, 1);
     for (int a = 0; a < k; ++a) {
@@ -89,7 +89,7 @@ __device__ __forceinline__ void slow_token(const int (&e)[KMAX], int k, int E, u
             const int j = e[b];
             if (b == a || (unsigned)j >= (unsigned)E || j == i) continue;
             ++cnt;
-            if (b > a) atomicAdd(&hist[tri_row(min(i, j), E) + max(i, j)], 1u);
+            if (b > a) atomicAdd(&hist[(tri_row(min(i, j), E) + max(i, j)) * CP], 1u);
         }
         if (km1 - cnt) atomicAdd(&corr[i], (unsigned)(km1 - cnt));
     }
@@ -111,7 +111,9 @@ __device__ __forceinline__ void load_raw(const int16_t* __restrict__ row, unsign
 }
 
 // One token (KT ids packed in w) of a family whose triangle starts at hist (corr = its correction counters).
-template <int KT>
+// CP > 1: the bins are interleaved CP-fold (word = bin * CP + copy) and hist already points at this
+// lane's copy, so lanes of different copies never share a bank.
+template <int KT, int CP = 1>
 __device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E, unsigned* hist, unsigned* corr) {
     int e[KT], s[KT];
 #pragma unroll
@@ -128,34 +130,35 @@ __device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E,
     if (fast) {
 #pragma unroll
         for (int a = 0; a + 1 < KT; ++a) {
-            unsigned* rowp = hist + tri_row(s[a], E);
+            unsigned* rowp = hist + tri_row(s[a], E) * CP;
 #pragma unroll
-            for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b], 1u);
+            for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b] * CP, 1u);
         }
         return;
     }
-    slow_token<KT>(e, KT, E, hist, corr);
+    slow_token<KT, CP>(e, KT, E, hist, corr);
 }
 
 // One token, any k: compile-time KT uses the packed path, KT == 0 reads k ids one by one.
-template <int KT>
+template <int KT, int CP = 1>
 __device__ __forceinline__ void count_token(const int16_t* __restrict__ row, int k, int E, unsigned* hist,
                                             unsigned* corr) {
     if constexpr (KT >= 2) {
         unsigned w[KT / 2];
         load_raw<KT>(row, w);
-        count_packed<KT>(w, E, hist, corr);
+        count_packed<KT, CP>(w, E, hist, corr);
     } else {
         int e[16];
 #pragma unroll
         for (int j = 0; j < 16; ++j) e[j] = (j < k) ? (int)__ldg(row + j) : -1;
-        slow_token<16>(e, k, E, hist, corr);
+        slow_token<16, CP>(e, k, E, hist, corr);
     }
 }
 
 // smem layout (words): [Fs][tri] pair bins | [Fs][E] corr | [Fs] ntok (layer 0 only) | pad to slot_words
 //                      | (filter mode) per-warp queues of token offsets
-template <int KT, bool FILTER>
+// CP (non-filter mode only): bank-spread copies of the pair bins, one per quarter warp.
+template <int KT, bool FILTER, int CP>
 __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParams p) {
     extern __shared__ __align__(16) unsigned hsm[];
     const int tid = threadIdx.x;
@@ -163,13 +166,16 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
     const int fg = FILTER ? blockIdx.x % p.nfg : 0;
     const long long lo = group_lo(g, p.T, p.groups), hi = group_lo(g + 1, p.T, p.groups);
     if (lo >= hi) return;
-    unsigned* corr = hsm + (size_t)p.Fs * p.tri;
+    const int nbins = p.Fs * p.tri;                       // pair bins of a slot
+    unsigned* corr = hsm + (size_t)nbins * CP;
     unsigned* sntok = corr + (size_t)p.Fs * p.E;
     const int k = KT > 0 ? KT : p.k;
     uint4* hsm4 = reinterpret_cast<uint4*>(hsm);
-    const int slot4 = p.slot_words / 4;
-    for (int i = tid; i < slot4; i += kThreads) hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
+    const int tail = p.slot_words - nbins;                 // corr + ntok + padding words
+    const int smem4 = (nbins * CP + tail + 3) / 4;
+    for (int i = tid; i < smem4; i += kThreads) hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
+    unsigned* hist_lane = hsm + (CP > 1 ? ((tid & 31) >> 3) % CP : 0);
 
     // filter mode: per-warp queue of matching token offsets (relative to the layer's token 0)
     unsigned* wq = hsm + p.slot_words + (tid >> 5) * kQueue;
@@ -193,10 +199,24 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             }
             __syncthreads();
             // flush this (group, layer) visit to its slot, then clear
-            uint4* dst = reinterpret_cast<uint4*>(p.scratch + ((size_t)(g + layer) * p.nfg + fg) * p.slot_words);
-            for (int i = tid; i < slot4; i += kThreads) {
-                dst[i] = hsm4[i];
-                hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
+            unsigned* dst = p.scratch + ((size_t)(g + layer) * p.nfg + fg) * p.slot_words;
+            if constexpr (CP == 1) {
+                uint4* dst4 = reinterpret_cast<uint4*>(dst);
+                for (int i = tid; i < smem4; i += kThreads) {
+                    dst4[i] = hsm4[i];
+                    hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
+                }
+            } else {
+                static_assert(CP == 1 || CP == 4, "copies are summed with one 16-byte load");
+                for (int i = tid; i < nbins; i += kThreads) {
+                    const uint4 v = hsm4[i];
+                    dst[i] = (v.x + v.y) + (v.z + v.w);
+                    hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
+                }
+                for (int i = tid; i < tail; i += kThreads) {
+                    dst[nbins + i] = corr[i];
+                    corr[i] = 0u;
+                }
             }
             __syncthreads();
             if (l < 0) break;
@@ -227,7 +247,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
                     for (int u = 0; u < kBatch; ++u) {
                         if ((unsigned)f[u] >= (unsigned)p.F) continue;      // padding token / past the end
                         if (l == 0) atomicAdd(&sntok[f[u]], 1u);
-                        count_packed<KT>(w[u], p.E, hsm + (size_t)f[u] * p.tri, corr + f[u] * p.E);
+                        count_packed<KT, CP>(w[u], p.E, hist_lane + (size_t)f[u] * p.tri * CP, corr + f[u] * p.E);
                     }
                 }
             } else {
@@ -235,7 +255,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
                     const int f = p.family[t];
                     if ((unsigned)f >= (unsigned)p.F) continue;     // padding token
                     if (l == 0) atomicAdd(&sntok[f], 1u);
-                    count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm + (size_t)f * p.tri, corr + f * p.E);
+                    count_token<KT, CP>(lbase + (size_t)t * k, k, p.E, hist_lane + (size_t)f * p.tri * CP, corr + f * p.E);
                 }
             }
         } else {
@@ -368,23 +388,23 @@ coact_global_kernel(const int16_t* __restrict__ indices, const int8_t* __restric
     }
 }
 
-template <int KT, bool FILTER>
+template <int KT, bool FILTER, int CP>
 int launch_hist(tacg_ctx* ctx, const HistParams& p, size_t smem, int grid) {
-    auto kern = coact_hist_kernel<KT, FILTER>;
+    auto kern = coact_hist_kernel<KT, FILTER, CP>;
     TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     kern<<<grid, kThreads, smem, ctx->stream>>>(p);
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
 
-template <bool FILTER>
+template <bool FILTER, int CP>
 int launch_hist_k(tacg_ctx* ctx, const HistParams& p, size_t smem, int grid) {
     switch (tacg_pick_kt(p.k, p.indices)) {
-        case 2: return launch_hist<2, FILTER>(ctx, p, smem, grid);
-        case 4: return launch_hist<4, FILTER>(ctx, p, smem, grid);
-        case 6: return launch_hist<6, FILTER>(ctx, p, smem, grid);
-        case 8: return launch_hist<8, FILTER>(ctx, p, smem, grid);
-        default: return launch_hist<0, FILTER>(ctx, p, smem, grid);
+        case 2: return launch_hist<2, FILTER, CP>(ctx, p, smem, grid);
+        case 4: return launch_hist<4, FILTER, CP>(ctx, p, smem, grid);
+        case 6: return launch_hist<6, FILTER, CP>(ctx, p, smem, grid);
+        case 8: return launch_hist<8, FILTER, CP>(ctx, p, smem, grid);
+        default: return launch_hist<0, FILTER, CP>(ctx, p, smem, grid);
     }
 }
 
@@ -426,10 +446,14 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     const size_t slots = (size_t)(p.groups + L - 1) * p.nfg;
     p.scratch = static_cast<unsigned*>(tacg_scratch(ctx, slots * p.slot_words * sizeof(unsigned)));
     if (!p.scratch) return TACG_ERR_CUDA;
-    const size_t smem = (size_t)p.slot_words * 4 + (filter ? queue_bytes : 0);
+    // four bank-spread copies of the pair bins when they fit (non-filter mode)
+    const size_t bins_bytes = sizeof(unsigned) * (size_t)p.Fs * p.tri;
+    const bool copies = !filter && (size_t)p.slot_words * 4 + 3 * bins_bytes + 16 <= limit;
+    const size_t smem = (size_t)p.slot_words * 4 + (filter ? queue_bytes : 0) + (copies ? 3 * bins_bytes + 16 : 0);
     const int grid = p.groups * p.nfg;
     tacg_prof_scope prof(ctx, TACG_PROF_COACT);
-    int rc = filter ? launch_hist_k<true>(ctx, p, smem, grid) : launch_hist_k<false>(ctx, p, smem, grid);
+    int rc = filter ? launch_hist_k<true, 1>(ctx, p, smem, grid)
+                    : (copies ? launch_hist_k<false, 4>(ctx, p, smem, grid) : launch_hist_k<false, 1>(ctx, p, smem, grid));
     if (rc != TACG_OK) return rc;
     const size_t fsmem = sizeof(unsigned) * ((size_t)p.tri + 2 * E);
     unsigned long long* nt = reinterpret_cast<unsigned long long*>(ntok);

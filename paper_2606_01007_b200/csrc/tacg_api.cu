@@ -167,8 +167,9 @@ int tacg_coact_accumulate(tacg_ctx* ctx, const int16_t* indices, const int8_t* f
         rc = read_errword(ctx, TACG_ERR_BAD_INDEX, "coact validate (record = layer*N + token)");
         if (rc != TACG_OK) return rc;
     }
-    // Path choice: the tensor path where it is supported, else the histogram.
-    const bool use_mma = N > 0 && ((path == TACG_PATH_MMA) || (path == TACG_PATH_AUTO && mma_ok));
+    // Path choice: measured on B200 the histogram kernel is faster than the
+    // tensor path at every supported shape, so AUTO takes the histogram; TACG_PATH_MMA forces tcgen05.
+    const bool use_mma = N > 0 && path == TACG_PATH_MMA;
     const bool zero_first = (flags & TACG_ZERO_FIRST) != 0;
     if (zero_first && N == 0) {
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(D, 0, sizeof(uint32_t) * (size_t)L * F * E, ctx->stream));

@@ -57,10 +57,12 @@ def _check_invariants(cfg, N, D, C, ntok):
     assert (C.sum(axis=(2, 3), dtype=np.uint64) == (k * (k - 1) * ntok)[None, :]).all()
 
 
-@pytest.mark.parametrize("cfg_id,L", [(2, 26), (3, 5), (3, 2), (4, 2), (5, 1)])
-def test_coact_full_size(tacg, ctx, cfg_id, L):
+@pytest.mark.parametrize("cfg_id,L,path", [(2, 26, "auto"), (3, 5, "auto"), (3, 2, "auto"), (4, 2, "auto"), (5, 1, "auto"),
+                                           (2, 26, "mma"), (3, 3, "mma")])
+def test_coact_full_size(tacg, ctx, cfg_id, L, path):
     cfg, idx, fam = _device_trace(cfg_id, L, eval_trace=False)
-    out = tacg.tacg_coact_accumulate(ctx, idx, fam, cfg.E, cfg.F, flags=tacg.TACG_ZERO_FIRST | tacg.TACG_PATH_AUTO)
+    flag = tacg.TACG_PATH_MMA if path == "mma" else tacg.TACG_PATH_AUTO
+    out = tacg.tacg_coact_accumulate(ctx, idx, fam, cfg.E, cfg.F, flags=tacg.TACG_ZERO_FIRST | flag)
     torch.cuda.synchronize()
     D, C, ntok = _u32(out["D"]), _u32(out["C"]), _u64(out["ntok"])
     _check_invariants(cfg, cfg.N, D, C, ntok)

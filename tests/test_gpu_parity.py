@@ -50,12 +50,17 @@ COACT_CASES = [
 ]
 
 
-@pytest.mark.parametrize("path", ["hist", "auto"])
+PATH_FLAG = {"hist": 0x10, "auto": 0x00, "mma": 0x20}
+
+
+@pytest.mark.parametrize("path", ["hist", "auto", "mma"])
 @pytest.mark.parametrize("cfg_id,N,L", COACT_CASES)
 def test_coact_counts_bit_exact(tacg, ctx, cfg_id, N, L, path):
     cfg, idx, fam = _trace(cfg_id, N, L)
+    if path == "mma" and cfg.E > 128:
+        pytest.skip("tcgen05 path: E <= 128 (one accumulator tile per family in 512 TMEM columns)")
     D, C, ntok = cbind.coact(idx.numpy(), fam.numpy(), cfg.E, cfg.F)
-    flags = tacg.TACG_ZERO_FIRST | (tacg.TACG_PATH_HIST if path == "hist" else tacg.TACG_PATH_AUTO)
+    flags = tacg.TACG_ZERO_FIRST | PATH_FLAG[path]
     out = tacg.tacg_coact_accumulate(ctx, idx.cuda(), fam.cuda(), cfg.E, cfg.F, flags=flags)
     torch.cuda.synchronize()
     assert (_u32(out["D"]) == D).all()
@@ -69,7 +74,7 @@ def test_coact_counts_bit_exact(tacg, ctx, cfg_id, N, L, path):
     assert (_u64(out2["ntok"]) == 2 * ntok).all()
 
 
-@pytest.mark.parametrize("path", ["hist", "auto"])
+@pytest.mark.parametrize("path", ["hist", "auto", "mma"])
 def test_coact_skip_rules_and_generic_k(tacg, ctx, path):
     """Negative ids = empty slots, negative family = padding; odd k and unaligned views use the generic loader."""
     rng = np.random.default_rng(5)
@@ -78,8 +83,10 @@ def test_coact_skip_rules_and_generic_k(tacg, ctx, path):
         idx[rng.random(idx.shape) < 0.1] = -1
         fam = rng.integers(0, F, size=N).astype(np.int8)
         fam[rng.random(N) < 0.05] = -1
+        if path == "mma" and k % 2:
+            continue                                    # tcgen05 path: even k only (vector row loads)
         D, C, ntok = cbind.coact(idx, fam, E, F)
-        flags = tacg.TACG_ZERO_FIRST | (tacg.TACG_PATH_HIST if path == "hist" else 0)
+        flags = tacg.TACG_ZERO_FIRST | PATH_FLAG[path]
         out = tacg.tacg_coact_accumulate(ctx, torch.from_numpy(idx).cuda(), torch.from_numpy(fam).cuda(), E, F,
                                          flags=flags)
         torch.cuda.synchronize()
