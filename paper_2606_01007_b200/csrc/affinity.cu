@@ -36,16 +36,19 @@ __device__ __forceinline__ double warp_max(double v) {
     return v;
 }
 
-// Abar[i,j] = (1/F) sum_f C[f,i,j] / max(1,ntok[f])   (readings Q2, Q4)
-__device__ __forceinline__ double abar_entry(const unsigned* __restrict__ Cl, const double* nf, int F, int E, int i, int j) {
+// Abar[i,j] = (1/F) sum_f C[f,i,j] / max(1,ntok[f])   (readings Q2, Q4).
+// inf[f] = 1 / (F * max(1,ntok[f])): one fp64 reciprocal per family instead of a division per entry;
+// the result differs from the divided form by a few fp64 ulps, far inside the fp32 tolerance (Q14).
+__device__ __forceinline__ double abar_entry(const unsigned* __restrict__ Cl, const double* inf, int F, int E, int i, int j) {
     double s = 0.0;
-    for (int f = 0; f < F; ++f) s += (double)__ldg(&Cl[((size_t)f * E + i) * E + j]) / nf[f];
-    return s / (double)F;
+    for (int f = 0; f < F; ++f) s += (double)__ldg(&Cl[((size_t)f * E + i) * E + j]) * inf[f];
+    return s;
 }
 
 // W[i,j] of Eq. 8 from Abar, max Abar and the preference rows of i and j (Eq. 7).
-__device__ __forceinline__ double w_entry(double abar, double amax, const double* pi, const double* pj, int F, double alpha) {
-    const double ah = amax > 0.0 ? abar / amax : 0.0;
+// iamax = 1/max Abar (0 when the maximum is 0, Q8).
+__device__ __forceinline__ double w_entry(double abar, double iamax, const double* pi, const double* pj, int F, double alpha) {
+    const double ah = abar * iamax;
     double at = 0.0;
     for (int f = 0; f < F; ++f) at += pi[f] * pj[f];
     return (1.0 - alpha) * ah + alpha * (at * ah);
@@ -58,7 +61,7 @@ rowstats_kernel(const unsigned* __restrict__ C, const unsigned long long* __rest
     const int lane = threadIdx.x & 31;
     if (i >= E) return;
     double nf[8];
-    for (int f = 0; f < F; ++f) nf[f] = (double)max(1ull, ntok[f]);
+    for (int f = 0; f < F; ++f) nf[f] = 1.0 / ((double)F * (double)max(1ull, ntok[f]));
     const unsigned* Cl = C + (size_t)l * F * E * E;
     double rmax = 0.0;
     for (int j = lane; j < E; j += 32) rmax = fmax(rmax, abar_entry(Cl, nf, F, E, i, j));
@@ -73,14 +76,15 @@ rowstats_kernel(const unsigned* __restrict__ C, const unsigned long long* __rest
     if (lane == 0) s.rowmax[(size_t)l * E + i] = rmax;
 }
 
-__device__ double block_sum(double v, double* red) {
-    v = warp_sum(v);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
-    __syncthreads();
-    double t = 0.0;
-    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
-    return t;
+// relative advantage of family f at one expert: x^f - mean of the other families (Eq. 2-3, Q5)
+__device__ __forceinline__ double rel_adv(const double* x, int E, int F, int f, int e) {
+    double other = 0.0;
+    if (F > 1) {
+        for (int g = 0; g < F; ++g)
+            if (g != f) other += x[g * E + e];
+        other /= (double)(F - 1);
+    }
+    return x[f * E + e] - other;
 }
 
 // One CTA per layer.  Dynamic smem: u[F][E], c[F][E], sc[F][E] doubles.
@@ -88,61 +92,42 @@ __global__ void __launch_bounds__(256)
 pref_kernel(const unsigned* __restrict__ D, const unsigned long long* __restrict__ ntok, int E, int F, double tau,
             double eps, AffScratch s, float* __restrict__ pref_out) {
     extern __shared__ double psm[];
-    __shared__ double red[8];
+    __shared__ double red[64];
     double* u = psm;
     double* c = psm + (size_t)F * E;
     double* sc = psm + (size_t)2 * F * E;
     const int l = blockIdx.x;
     const unsigned* Dl = D + (size_t)l * F * E;
+    // Warp f owns family f (F <= 8 = warps of the CTA): every sum over experts is a warp reduction,
+    // so the only CTA-wide barriers are the two below.
+    const int f = threadIdx.x >> 5, lane = threadIdx.x & 31;
     // O2: u = D / sum D (Q1), c = rowsum(C)/N_f (Eq. 2 right; counts >= 0 so |.| is the identity, Q3)
-    for (int f = 0; f < F; ++f) {
+    if (f < F) {
         double part = 0.0;
-        for (int e = threadIdx.x; e < E; e += blockDim.x) part += (double)Dl[f * E + e];   // exact: integers < 2^53
-        const double tot = fmax(1.0, block_sum(part, red));
+        for (int e = lane; e < E; e += 32) part += (double)Dl[f * E + e];          // exact: integers < 2^53
+        const double tot = fmax(1.0, warp_sum(part));
         const double nf = (double)max(1ull, ntok[f]);
-        for (int e = threadIdx.x; e < E; e += blockDim.x) {
+        for (int e = lane; e < E; e += 32) {
             u[f * E + e] = (double)Dl[f * E + e] / tot;
             c[f * E + e] = (double)s.rowsum[((size_t)l * F + f) * E + e] / nf;
-            sc[f * E + e] = 0.0;
         }
     }
     __syncthreads();
     // O3, O4: relative advantage (Eq. 2-3) and z-score over experts (Eq. 4), summed into s (Eq. 5)
-    for (int pass = 0; pass < 2; ++pass) {
-        const double* x = pass == 0 ? u : c;
-        for (int f = 0; f < F; ++f) {
+    if (f < F) {
+        for (int e = lane; e < E; e += 32) sc[f * E + e] = 0.0;
+        for (int pass = 0; pass < 2; ++pass) {
+            const double* x = pass == 0 ? u : c;
             double part = 0.0;
-            for (int e = threadIdx.x; e < E; e += blockDim.x) {
-                double other = 0.0;
-                if (F > 1) {
-                    for (int g = 0; g < F; ++g)
-                        if (g != f) other += x[g * E + e];
-                    other /= (double)(F - 1);
-                }
-                part += x[f * E + e] - other;
-            }
-            const double mu = block_sum(part, red) / (double)E;
+            for (int e = lane; e < E; e += 32) part += rel_adv(x, E, F, f, e);
+            const double mu = warp_sum(part) / (double)E;
             double vpart = 0.0;
-            for (int e = threadIdx.x; e < E; e += blockDim.x) {
-                double other = 0.0;
-                if (F > 1) {
-                    for (int g = 0; g < F; ++g)
-                        if (g != f) other += x[g * E + e];
-                    other /= (double)(F - 1);
-                }
-                const double d = (x[f * E + e] - other) - mu;
+            for (int e = lane; e < E; e += 32) {
+                const double d = rel_adv(x, E, F, f, e) - mu;
                 vpart += d * d;
             }
-            const double sigma = sqrt(block_sum(vpart, red) / (double)E);
-            for (int e = threadIdx.x; e < E; e += blockDim.x) {
-                double other = 0.0;
-                if (F > 1) {
-                    for (int g = 0; g < F; ++g)
-                        if (g != f) other += x[g * E + e];
-                    other /= (double)(F - 1);
-                }
-                sc[f * E + e] += ((x[f * E + e] - other) - mu) / (sigma + eps);
-            }
+            const double sigma = sqrt(warp_sum(vpart) / (double)E);
+            for (int e = lane; e < E; e += 32) sc[f * E + e] += (rel_adv(x, E, F, f, e) - mu) / (sigma + eps);
         }
     }
     __syncthreads();
@@ -213,11 +198,11 @@ graph_aff_kernel(const unsigned* __restrict__ C, const unsigned long long* __res
     if (i >= E) return;
     double nf[8], pi[8];
     for (int f = 0; f < F; ++f) {
-        nf[f] = (double)max(1ull, ntok[f]);
+        nf[f] = 1.0 / ((double)F * (double)max(1ull, ntok[f]));
         pi[f] = s.pref64[((size_t)l * E + i) * F + f];
     }
     const unsigned* Cl = C + (size_t)l * F * E * E;
-    const double amax = s.amax[l];
+    const double amax = s.amax[l] > 0.0 ? 1.0 / s.amax[l] : 0.0;
     double* wr = wrow + (size_t)warp * E;
     for (int j = lane; j < E; j += 32) {
         const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), amax, pi, s.pref64 + ((size_t)l * E + j) * F, F, alpha);
@@ -246,11 +231,11 @@ gain_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict
     const int8_t* pr = primary + (size_t)l * E;
     double nf[8], pi[8];
     for (int f = 0; f < F; ++f) {
-        nf[f] = (double)max(1ull, ntok[f]);
+        nf[f] = 1.0 / ((double)F * (double)max(1ull, ntok[f]));
         pi[f] = s.pref64[((size_t)l * E + i) * F + f];
     }
     const unsigned* Cl = C + (size_t)l * F * E * E;
-    const double amax = s.amax[l];
+    const double amax = s.amax[l] > 0.0 ? 1.0 / s.amax[l] : 0.0;
     const double* affl = s.aff64 + (size_t)l * E * P;
     const int a = pr[i] & 63;
     for (int j = lane; j < E; j += 32) {

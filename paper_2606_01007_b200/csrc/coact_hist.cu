@@ -292,71 +292,61 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
     }
 }
 
-// One CTA per (layer, family).  Sums the scratch slots of the layer into shared memory, then writes
-// the symmetric C rows, D and (layer 0) ntok.  ZERO: overwrite instead of accumulate.
+// One warp per output row: grid (ceil(E/8), L*F), 8 rows per CTA.  Each lane sums the slots' bins of its
+// (i,j) elements straight from scratch (L2 resident; the eight neighbouring rows of a CTA share the
+// sectors of the column part), writes the symmetric C row, and the warp reduces the row sum for D.
+// ZERO: overwrite instead of accumulate (the diagonal is then cleared with the rest).
 template <bool ZERO>
-__global__ void __launch_bounds__(512) coact_finalize_kernel(const HistParams p, unsigned* __restrict__ D,
+__global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p, unsigned* __restrict__ D,
                                                             unsigned* __restrict__ C,
                                                             unsigned long long* __restrict__ ntok) {
-    extern __shared__ __align__(16) unsigned fsm[];      // [tri] pair sums | [E] corr sums | [E] row sums
-    const int l = blockIdx.x / p.F, f = blockIdx.x % p.F;
+    const int lf = blockIdx.y;
+    const int l = lf / p.F, f = lf % p.F;
     const int E = p.E, tri = p.tri;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = blockIdx.x * 8 + warp;
     const int fgi = p.nfg > 1 ? f : 0;                   // which CTA of a group holds family f
     const int fs = p.nfg > 1 ? 0 : f;                    // family index inside a slot
     const int g0 = group_of_item((long long)l * p.cps, p.T, p.groups);
     const int g1 = group_of_item((long long)(l + 1) * p.cps - 1, p.T, p.groups);
-    unsigned* scorr = fsm + tri;
-    unsigned* srow = scorr + E;
+    const int ng = g1 - g0 + 1;
     const unsigned* slot0 = p.scratch + ((size_t)(g0 + l) * p.nfg + fgi) * p.slot_words;
     const size_t gstride = (size_t)p.nfg * p.slot_words;
-    const int ng = g1 - g0 + 1;
-    for (int i = threadIdx.x; i < tri; i += blockDim.x) {
-        const unsigned* src = slot0 + (size_t)fs * tri + i;
-        unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0;
-        int g = 0;
-        for (; g + 4 <= ng; g += 4) {
-            a0 += src[(size_t)g * gstride];
-            a1 += src[(size_t)(g + 1) * gstride];
-            a2 += src[(size_t)(g + 2) * gstride];
-            a3 += src[(size_t)(g + 3) * gstride];
-        }
-        for (; g < ng; ++g) a0 += src[(size_t)g * gstride];
-        fsm[i] = (a0 + a1) + (a2 + a3);
-    }
-    for (int i = threadIdx.x; i < E; i += blockDim.x) {
-        unsigned acc = 0;
-        for (int g = g0; g <= g1; ++g)
-            acc += slot0[(size_t)(g - g0) * gstride + (size_t)p.Fs * tri + (size_t)fs * E + i];
-        scorr[i] = acc;
-    }
-    if (l == 0 && threadIdx.x == 0) {
+    if (l == 0 && blockIdx.x == 0 && threadIdx.x == 0) {
         unsigned long long acc = 0;
-        for (int g = g0; g <= g1; ++g) acc += slot0[(size_t)(g - g0) * gstride + (size_t)p.Fs * (tri + E) + fs];
+        for (int g = 0; g < ng; ++g) acc += slot0[(size_t)g * gstride + (size_t)p.Fs * (tri + E) + fs];
         ntok[f] = ZERO ? acc : ntok[f] + acc;
     }
-    __syncthreads();
-    unsigned* Cf = C + ((size_t)l * p.F + f) * E * E;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-    for (int i = warp; i < E; i += nwarps) {
-        unsigned rs = 0;
-        const int ri = tri_row(i, E);
-        for (int j = lane; j < E; j += 32) {
-            unsigned v = 0;
-            if (j > i) v = fsm[ri + j];
-            else if (j < i) v = fsm[tri_row(j, E) + i];
-            rs += v;
-            const size_t o = (size_t)i * E + j;
-            if (ZERO) Cf[o] = v;                         // the diagonal is cleared with the rest
-            else if (j != i) Cf[o] += v;
+    if (i >= E) return;
+    unsigned* Cf = C + ((size_t)l * p.F + f) * E * E + (size_t)i * E;
+    const unsigned* bins = slot0 + (size_t)fs * tri;
+    const int ri = tri_row(i, E);
+    unsigned rs = 0;
+    for (int j = lane; j < E; j += 32) {
+        unsigned v = 0;
+        if (j != i) {
+            const unsigned* src = bins + (j > i ? ri + j : tri_row(j, E) + i);
+            unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0;
+            int g = 0;
+            for (; g + 4 <= ng; g += 4) {
+                a0 += src[(size_t)g * gstride];
+                a1 += src[(size_t)(g + 1) * gstride];
+                a2 += src[(size_t)(g + 2) * gstride];
+                a3 += src[(size_t)(g + 3) * gstride];
+            }
+            for (; g < ng; ++g) a0 += src[(size_t)g * gstride];
+            v = (a0 + a1) + (a2 + a3);
         }
-        rs = __reduce_add_sync(0xffffffffu, rs);
-        if (lane == 0) srow[i] = rs;
+        rs += v;
+        if (ZERO) Cf[j] = v;
+        else if (j != i) Cf[j] += v;
     }
-    __syncthreads();
-    const unsigned km1 = (unsigned)max(p.k - 1, 1);
-    unsigned* Df = D + ((size_t)l * p.F + f) * E;
-    for (int i = threadIdx.x; i < E; i += blockDim.x) {
-        const unsigned d = (srow[i] + scorr[i]) / km1;
+    rs = __reduce_add_sync(0xffffffffu, rs);
+    if (lane == 0) {
+        unsigned corr = 0;
+        for (int g = 0; g < ng; ++g) corr += slot0[(size_t)g * gstride + (size_t)p.Fs * tri + (size_t)fs * E + i];
+        const unsigned d = (rs + corr) / (unsigned)max(p.k - 1, 1);
+        unsigned* Df = D + ((size_t)l * p.F + f) * E;
         Df[i] = ZERO ? d : Df[i] + d;
     }
 }
@@ -455,15 +445,10 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     int rc = filter ? launch_hist_k<true, 1>(ctx, p, smem, grid)
                     : (copies ? launch_hist_k<false, 4>(ctx, p, smem, grid) : launch_hist_k<false, 1>(ctx, p, smem, grid));
     if (rc != TACG_OK) return rc;
-    const size_t fsmem = sizeof(unsigned) * ((size_t)p.tri + 2 * E);
     unsigned long long* nt = reinterpret_cast<unsigned long long*>(ntok);
-    if (zero_first) {
-        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(coact_finalize_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem));
-        coact_finalize_kernel<true><<<L * F, 512, fsmem, ctx->stream>>>(p, D, C, nt);
-    } else {
-        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(coact_finalize_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsmem));
-        coact_finalize_kernel<false><<<L * F, 512, fsmem, ctx->stream>>>(p, D, C, nt);
-    }
+    const dim3 fgrid((E + 7) / 8, L * F);
+    if (zero_first) coact_finalize_kernel<true><<<fgrid, 256, 0, ctx->stream>>>(p, D, C, nt);
+    else coact_finalize_kernel<false><<<fgrid, 256, 0, ctx->stream>>>(p, D, C, nt);
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
