@@ -312,16 +312,20 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
     const int ng = g1 - g0 + 1;
     const unsigned* slot0 = p.scratch + ((size_t)(g0 + l) * p.nfg + fgi) * p.slot_words;
     const size_t gstride = (size_t)p.nfg * p.slot_words;
-    if (l == 0 && blockIdx.x == 0 && threadIdx.x == 0) {
-        unsigned long long acc = 0;
-        for (int g = 0; g < ng; ++g) acc += slot0[(size_t)g * gstride + (size_t)p.Fs * (tri + E) + fs];
-        ntok[f] = ZERO ? acc : ntok[f] + acc;
+    if (l == 0 && blockIdx.x == 0 && warp == 0) {         // slots are read one per lane, then reduced
+        unsigned acc = 0;
+        for (int g = lane; g < ng; g += 32) acc += slot0[(size_t)g * gstride + (size_t)p.Fs * (tri + E) + fs];
+        acc = __reduce_add_sync(0xffffffffu, acc);
+        if (lane == 0) ntok[f] = ZERO ? (unsigned long long)acc : ntok[f] + acc;
     }
     if (i >= E) return;
     unsigned* Cf = C + ((size_t)l * p.F + f) * E * E + (size_t)i * E;
     const unsigned* bins = slot0 + (size_t)fs * tri;
     const int ri = tri_row(i, E);
     unsigned rs = 0;
+    unsigned corr = 0;
+    for (int g = lane; g < ng; g += 32) corr += slot0[(size_t)g * gstride + (size_t)p.Fs * tri + (size_t)fs * E + i];
+#pragma unroll 2
     for (int j = lane; j < E; j += 32) {
         unsigned v = 0;
         if (j != i) {
@@ -341,11 +345,9 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
         if (ZERO) Cf[j] = v;
         else if (j != i) Cf[j] += v;
     }
-    rs = __reduce_add_sync(0xffffffffu, rs);
+    rs = __reduce_add_sync(0xffffffffu, rs + corr);
     if (lane == 0) {
-        unsigned corr = 0;
-        for (int g = 0; g < ng; ++g) corr += slot0[(size_t)g * gstride + (size_t)p.Fs * tri + (size_t)fs * E + i];
-        const unsigned d = (rs + corr) / (unsigned)max(p.k - 1, 1);
+        const unsigned d = rs / (unsigned)max(p.k - 1, 1);
         unsigned* Df = D + ((size_t)l * p.F + f) * E;
         Df[i] = ZERO ? d : Df[i] + d;
     }

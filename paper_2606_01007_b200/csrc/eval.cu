@@ -208,6 +208,7 @@ struct EvalParams {
     unsigned long long* load;          // [L,P] out
     unsigned long long* comm_span;     // [L,F] out (zeroed before launch, reduced atomically)
     unsigned long long* comm_remote;   // [L,F]
+    unsigned long long* ntok;          // [F] out (zeroed before launch; counted by the CTAs of layer 0)
     unsigned char* cost;    // [L,N] or null
     signed char* serve;     // [L,N,k] or null
     unsigned long long* delta;   // scratch [L,nmb,P], zeroed before launch (only used when cpl > 1)
@@ -272,6 +273,7 @@ eval_kernel(EvalParams p) {
     __shared__ unsigned long long ltot[64];  // cumulative integer load of this layer
     __shared__ unsigned long long feas_s;
     __shared__ unsigned long long comm_s[16];
+    __shared__ unsigned fam_s[8];          // tokens per family seen by this CTA (layer 0 only)
 
     const int group = blockIdx.x / p.cpl;
     const int part = blockIdx.x % p.cpl;
@@ -290,12 +292,24 @@ eval_kernel(EvalParams p) {
             ltot[tid] = 0ull;
         }
         if (tid < 16) comm_s[tid] = 0ull;
+        if (tid < 8) fam_s[tid] = 0u;
         __syncthreads();
         unsigned acc[8];                    // per family: sum of span | remote << 16 over this thread's tokens
 #pragma unroll
         for (int g = 0; g < 8; ++g) acc[g] = 0u;
         int since = 0;                      // tokens added to acc since the last flush (uniform per warp)
+        unsigned long long famc = 0ull;     // layer 0: tokens per family of this thread, 8-bit fields
         auto flush_acc = [&]() {
+            if (layer == 0) {
+#pragma unroll
+                for (int g = 0; g < 8; ++g) {
+                    if (g < F) {
+                        const unsigned c = __reduce_add_sync(0xffffffffu, (unsigned)(famc >> (8 * g)) & 0xffu);
+                        if (lane == 0 && c) atomicAdd(&fam_s[g], c);
+                    }
+                }
+                famc = 0ull;
+            }
 #pragma unroll
             for (int g = 0; g < 8; ++g) {
                 if (g < F) {
@@ -406,11 +420,12 @@ eval_kernel(EvalParams p) {
 #pragma unroll
                     for (int g = 0; g < 8; ++g)
                         if (g < F) acc[g] += (f[u] == g) ? packed : 0u;
+                    if (layer == 0 && live) famc += 1ull << (8 * f[u]);
                     home += stepP;
                     if (home >= P) home -= P;
                 }
                 since += U;
-                if (since >= 3800) flush_acc();
+                if (since >= (layer == 0 ? 252 : 3800)) flush_acc();   // 8-bit / 16-bit fields must not overflow
             }
             flush_acc();
             // step 5: integer dispatch counts of the micro-batch, then Eq. 15
@@ -445,6 +460,7 @@ eval_kernel(EvalParams p) {
             __syncthreads();
         }
         // layer epilogue: communication sums and, from part 0, loads and the final state
+        if (layer == 0 && tid < F && fam_s[tid]) atomicAdd(&p.ntok[tid], (unsigned long long)fam_s[tid]);
         if (tid < F) {
             if (comm_s[tid]) atomicAdd(&p.comm_span[(size_t)layer * F + tid], comm_s[tid]);
             if (comm_s[8 + tid]) atomicAdd(&p.comm_remote[(size_t)layer * F + tid], comm_s[8 + tid]);
@@ -457,27 +473,37 @@ eval_kernel(EvalParams p) {
 }
 
 // O11: (jain, maxvio, cv) per layer and for the loads summed over layers, fp64 -> fp32.
-__global__ void fairness_kernel(const unsigned long long* __restrict__ load, int L, int P, float* __restrict__ out) {
-    for (int row = blockIdx.x * blockDim.x + threadIdx.x; row <= L; row += gridDim.x * blockDim.x) {
+// One CTA per output row (row L = loads summed over layers), 64 x 16 threads: thread (m, q) adds the
+// layers q, q+16, ... of partition m, so no thread walks more than L/16 dependent loads; the
+// statistics are then computed by one thread from the P sums in the fixed order m = 0..P-1.
+__global__ void __launch_bounds__(1024) fairness_kernel(const unsigned long long* __restrict__ load, int L, int P,
+                                                       float* __restrict__ out) {
+    __shared__ unsigned long long part[16][64];
+    __shared__ double x[64];
+    const int row = blockIdx.x;
+    const int m = threadIdx.x & 63, q = threadIdx.x >> 6;
+    unsigned long long v = 0;
+    if (m < P) {
+        if (row < L) { if (q == 0) v = load[(size_t)row * P + m]; }
+        else for (int l = q; l < L; l += 16) v += load[(size_t)l * P + m];
+    }
+    part[q][m] = v;
+    __syncthreads();
+    if (q == 0) {
+        unsigned long long t = 0;
+#pragma unroll
+        for (int z = 0; z < 16; ++z) t += part[z][m];
+        x[m] = (double)t;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
         double tot = 0.0, sq = 0.0, mx = 0.0;
-        for (int m = 0; m < P; ++m) {
-            unsigned long long v = 0;
-            if (row < L) v = load[(size_t)row * P + m];
-            else for (int l = 0; l < L; ++l) v += load[(size_t)l * P + m];
-            const double x = (double)v;
-            tot += x; sq += x * x; mx = fmax(mx, x);
-        }
+        for (int z = 0; z < P; ++z) { tot += x[z]; sq += x[z] * x[z]; mx = fmax(mx, x[z]); }
         double jain = 1.0, maxvio = 0.0, cv = 0.0;
         if (tot != 0.0) {
             const double mean = tot / (double)P;
             double var = 0.0;
-            for (int m = 0; m < P; ++m) {
-                unsigned long long v = 0;
-                if (row < L) v = load[(size_t)row * P + m];
-                else for (int l = 0; l < L; ++l) v += load[(size_t)l * P + m];
-                const double x = (double)v;
-                var += (x - mean) * (x - mean);
-            }
+            for (int z = 0; z < P; ++z) var += (x[z] - mean) * (x[z] - mean);
             var /= (double)P;
             jain = (tot * tot) / ((double)P * sq);
             maxvio = (mx - mean) / mean;
@@ -529,6 +555,19 @@ select_kernel(const int16_t* __restrict__ indices, long long N, int k, int E, in
     }
 }
 
+// clears the accumulated outputs and the barrier scratch in one launch
+__global__ void eval_zero_kernel(unsigned long long* a, size_t na, unsigned long long* b, size_t nb,
+                                 unsigned long long* c, size_t nc, unsigned long long* d, size_t nd,
+                                 unsigned long long* s, size_t ns) {
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (size_t i = i0; i < na; i += stride) a[i] = 0ull;
+    for (size_t i = i0; i < nb; i += stride) b[i] = 0ull;
+    for (size_t i = i0; i < nc; i += stride) c[i] = 0ull;
+    for (size_t i = i0; i < nd; i += stride) d[i] = 0ull;
+    for (size_t i = i0; i < ns; i += stride) s[i] = 0ull;
+}
+
 size_t eval_smem_bytes(int E, int P, int r) {
     return tables_bytes(E, r) + 64 * sizeof(unsigned long long) + sizeof(unsigned) * (size_t)P * 32;
 }
@@ -563,7 +602,14 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     if (!base) return TACG_ERR_CUDA;
     p.delta = reinterpret_cast<unsigned long long*>(base + o_delta);
     p.barrier = reinterpret_cast<unsigned*>(base + o_bar);
-    if (p.cpl > 1) TACG_CUDA_TRY(ctx, cudaMemsetAsync(base, 0, off, ctx->stream));
+    {
+        const size_t ns = p.cpl > 1 ? off / sizeof(unsigned long long) : 0;
+        const int zgrid = (int)max((size_t)1, min((size_t)ctx->sm_count, (ns + 1023) / 1024));
+        eval_zero_kernel<<<zgrid, 1024, 0, ctx->stream>>>(p.comm_span, (size_t)p.L * p.F, p.comm_remote, (size_t)p.L * p.F,
+                                                          p.load, (size_t)p.L * p.P, p.ntok, (size_t)p.F,
+                                                          reinterpret_cast<unsigned long long*>(base), ns);
+        TACG_LAUNCH_CHECK(ctx);
+    }
     tacg_prof_scope prof(ctx, TACG_PROF_EVAL);
     if (waits) {
         void* args[] = {&p};
@@ -610,11 +656,14 @@ int tacg_launch_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, 
 int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k, int L, int E,
                      int F, int P, const int8_t* primary, const int8_t* replicas, int r, float theta, double rho,
                      int64_t microbatch, int64_t token_offset, double* load_state, uint64_t* load,
-                     uint64_t* comm_span, uint64_t* comm_remote, float* fairness, uint8_t* cost_per_token,
-                     int8_t* serve) {
-    TACG_CUDA_TRY(ctx, cudaMemsetAsync(comm_span, 0, sizeof(uint64_t) * (size_t)L * F, ctx->stream));
-    TACG_CUDA_TRY(ctx, cudaMemsetAsync(comm_remote, 0, sizeof(uint64_t) * (size_t)L * F, ctx->stream));
-    TACG_CUDA_TRY(ctx, cudaMemsetAsync(load, 0, sizeof(uint64_t) * (size_t)L * P, ctx->stream));
+                     uint64_t* comm_span, uint64_t* comm_remote, uint64_t* ntok, float* fairness,
+                     uint8_t* cost_per_token, int8_t* serve) {
+    if (N == 0) {
+        TACG_CUDA_TRY(ctx, cudaMemsetAsync(comm_span, 0, sizeof(uint64_t) * (size_t)L * F, ctx->stream));
+        TACG_CUDA_TRY(ctx, cudaMemsetAsync(comm_remote, 0, sizeof(uint64_t) * (size_t)L * F, ctx->stream));
+        TACG_CUDA_TRY(ctx, cudaMemsetAsync(load, 0, sizeof(uint64_t) * (size_t)L * P, ctx->stream));
+        TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
+    }
     if (N > 0) {
         EvalParams p;
         p.indices = indices; p.family = family; p.N = N; p.k = k; p.L = L; p.E = E; p.F = F; p.P = P; p.r = r;
@@ -627,6 +676,7 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         p.load = reinterpret_cast<unsigned long long*>(load);
         p.comm_span = reinterpret_cast<unsigned long long*>(comm_span);
         p.comm_remote = reinterpret_cast<unsigned long long*>(comm_remote);
+        p.ntok = reinterpret_cast<unsigned long long*>(ntok);
         p.cost = cost_per_token;
         p.serve = reinterpret_cast<signed char*>(serve);
         p.delta = nullptr; p.barrier = nullptr; p.cpl = 1; p.groups = 1;
@@ -640,7 +690,7 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         }
         if (rc != TACG_OK) return rc;
     }
-    fairness_kernel<<<1, 64, 0, ctx->stream>>>(reinterpret_cast<const unsigned long long*>(load), L, P, fairness);
+    fairness_kernel<<<L + 1, 1024, 0, ctx->stream>>>(reinterpret_cast<const unsigned long long*>(load), L, P, fairness);
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }

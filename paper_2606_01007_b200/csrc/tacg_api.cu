@@ -241,13 +241,8 @@ int tacg_eval_placement(tacg_ctx* ctx, const int16_t* indices, const int8_t* fam
         rc = read_errword(ctx, TACG_ERR_PLACEMENT, "eval validate (record = layer*E + expert)");
         if (rc != TACG_OK) return rc;
     }
-    TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
-    if (N > 0) {
-        int rc = tacg_launch_family_count(ctx, family, N, F, ntok);
-        if (rc != TACG_OK) return rc;
-    }
     return tacg_launch_eval(ctx, indices, family, N, k, L, E, F, P, primary, r ? replicas : nullptr, r, theta, rho,
-                            microbatch, token_offset, load_state, load, comm_span, comm_remote, fairness,
+                            microbatch, token_offset, load_state, load, comm_span, comm_remote, ntok, fairness,
                             cost_per_token, serve);
 }
 

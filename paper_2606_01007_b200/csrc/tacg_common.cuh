@@ -88,18 +88,21 @@ int tacg_launch_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, 
 int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k, int L,
                      int E, int F, int P, const int8_t* primary, const int8_t* replicas, int r, float theta,
                      double rho, int64_t microbatch, int64_t token_offset, double* load_state,
-                     uint64_t* load, uint64_t* comm_span, uint64_t* comm_remote, float* fairness,
+                     uint64_t* load, uint64_t* comm_span, uint64_t* comm_remote, uint64_t* ntok, float* fairness,
                      uint8_t* cost_per_token, int8_t* serve);
 
 // ---- device helpers ----
 #ifdef __CUDACC__
 // Static work split of the co-activation kernels: T items (layer-major) over `groups` CTA groups;
 // group g owns items [g*T/groups, (g+1)*T/groups) and writes one scratch slot per layer it visits.
-__host__ __device__ __forceinline__ long long group_lo(long long g, long long T, int groups) { return g * T / groups; }
+__host__ __device__ __forceinline__ long long group_lo(long long g, long long T, int groups) {
+    if (T < (1ll << 24) && groups < 256) return (long long)(((unsigned)g * (unsigned)T) / (unsigned)groups);   // 32-bit divide
+    return g * T / groups;
+}
 
 // the group that owns item x
 __device__ __forceinline__ int group_of_item(long long x, long long T, int groups) {
-    int g = (int)((x * groups) / T);
+    int g = (T < (1ll << 24) && groups < 256) ? (int)(((unsigned)x * (unsigned)groups) / (unsigned)T) : (int)((x * groups) / T);
     if (g >= groups) g = groups - 1;
     while (g + 1 < groups && group_lo(g + 1, T, groups) <= x) ++g;
     while (g > 0 && group_lo(g, T, groups) > x) --g;
