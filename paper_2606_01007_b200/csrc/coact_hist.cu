@@ -42,6 +42,8 @@ struct HistParams {
     int groups;         // CTAs / nfg; group g owns items [g*T/groups, (g+1)*T/groups)
     unsigned* scratch;  // [(groups+L-1)*nfg][slot_words]
     int slot_words;     // Fs*(tri+E+1) rounded up to 4
+    int memo_off;       // byte offset of the token-set table in shared memory, 0 = no table
+    int memo_ts;        // table entries per family (power of two)
 };
 
 // R(i) + j is the bin of the pair i < j in a row-major strict upper triangle of an E x E matrix:
@@ -113,8 +115,19 @@ __device__ __forceinline__ void load_raw(const int16_t* __restrict__ row, unsign
 // One token (KT ids packed in w) of a family whose triangle starts at hist (corr = its correction counters).
 // CP > 1: the bins are interleaved CP-fold (word = bin * CP + copy) and hist already points at this
 // lane's copy, so lanes of different copies never share a bank.
+// Token-set table (one region per family): a token whose sorted ids are already a key of the table
+// costs one 64-bit CAS and one increment instead of k(k-1)/2 bin increments; the entries are expanded
+// into the bins (count x every pair) when the CTA leaves the layer.  Exact for any input; it pays
+// when expert sets repeat (planted groups, popular sets) and costs one failed CAS otherwise.
+struct MemoTable {
+    unsigned long long* keys;   // nullptr = disabled; 0 = empty entry (never a key: ids are distinct, k >= 2)
+    unsigned* cnt;
+    unsigned mask;              // entries - 1
+};
+
 template <int KT, int CP = 1>
-__device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E, unsigned* hist, unsigned* corr) {
+__device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E, unsigned* hist, unsigned* corr,
+                                             const MemoTable memo = MemoTable{nullptr, nullptr, 0u}) {
     int e[KT], s[KT];
 #pragma unroll
     for (int i = 0; i < KT / 2; ++i) {
@@ -128,6 +141,17 @@ __device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E,
 #pragma unroll
     for (int a = 0; a + 1 < KT; ++a) fast = fast && (s[a] != s[a + 1]);
     if (fast) {
+        if (memo.keys) {
+            unsigned long long key = 0ull;
+#pragma unroll
+            for (int a = 0; a < KT; ++a) key |= (unsigned long long)(unsigned)s[a] << (8 * a);
+            const unsigned h = (unsigned)((key * 0x9E3779B97F4A7C15ull) >> 40) & memo.mask;
+            const unsigned long long prev = atomicCAS(memo.keys + h, 0ull, key);
+            if (prev == 0ull || prev == key) {
+                atomicAdd(memo.cnt + h, 1u);
+                return;
+            }
+        }
 #pragma unroll
         for (int a = 0; a + 1 < KT; ++a) {
             unsigned* rowp = hist + tri_row(s[a], E) * CP;
@@ -142,11 +166,11 @@ __device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E,
 // One token, any k: compile-time KT uses the packed path, KT == 0 reads k ids one by one.
 template <int KT, int CP = 1>
 __device__ __forceinline__ void count_token(const int16_t* __restrict__ row, int k, int E, unsigned* hist,
-                                            unsigned* corr) {
+                                            unsigned* corr, const MemoTable memo = MemoTable{nullptr, nullptr, 0u}) {
     if constexpr (KT >= 2) {
         unsigned w[KT / 2];
         load_raw<KT>(row, w);
-        count_packed<KT, CP>(w, E, hist, corr);
+        count_packed<KT, CP>(w, E, hist, corr, memo);
     } else {
         int e[16];
 #pragma unroll
@@ -176,6 +200,19 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
     for (int i = tid; i < smem4; i += kThreads) hsm4[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
     unsigned* hist_lane = hsm + (CP > 1 ? ((tid & 31) >> 3) % CP : 0);
+    // token-set table: [Fs][memo_ts] keys, then [Fs][memo_ts] counts
+    const int mentries = (KT >= 2 && p.memo_off) ? p.Fs * p.memo_ts : 0;
+    unsigned long long* mkeys = reinterpret_cast<unsigned long long*>(reinterpret_cast<unsigned char*>(hsm) + p.memo_off);
+    unsigned* mcnt = reinterpret_cast<unsigned*>(mkeys + mentries);
+    for (int i = tid; i < mentries; i += kThreads) { mkeys[i] = 0ull; mcnt[i] = 0u; }
+    auto memo_of = [&](int fl) {
+        MemoTable m;
+        m.keys = mentries ? mkeys + (size_t)fl * p.memo_ts : nullptr;
+        m.cnt = mcnt + (size_t)fl * p.memo_ts;
+        m.mask = (unsigned)(p.memo_ts - 1);
+        return m;
+    };
+    __syncthreads();
 
     // filter mode: per-warp queue of matching token offsets (relative to the layer's token 0)
     unsigned* wq = hsm + p.slot_words + (tid >> 5) * kQueue;
@@ -194,10 +231,32 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
         if (l != layer) {
             const int16_t* lbase = p.indices + (size_t)layer * (size_t)p.N * k;
             if (FILTER) {               // drain the partial queue of this layer
-                if (lane < qn) count_token<KT>(lbase + (size_t)wq[lane] * k, k, p.E, hsm, corr);
+                if (lane < qn) count_token<KT>(lbase + (size_t)wq[lane] * k, k, p.E, hsm, corr, memo_of(0));
                 qn = 0;
             }
             __syncthreads();
+            if constexpr (KT >= 2) {
+                // expand the token-set table: count x every pair of the key
+                for (int i = tid; i < mentries; i += kThreads) {
+                    const unsigned c = mcnt[i];
+                    if (c) {
+                        const unsigned long long key = mkeys[i];
+                        unsigned* hf = hsm + (size_t)(i / p.memo_ts) * p.tri * CP + (CP > 1 ? (tid & (CP - 1)) : 0);
+                        int s[KT];
+#pragma unroll
+                        for (int a = 0; a < KT; ++a) s[a] = (int)((key >> (8 * a)) & 0xffull);
+#pragma unroll
+                        for (int a = 0; a + 1 < KT; ++a) {
+                            unsigned* rowp = hf + tri_row(s[a], p.E) * CP;
+#pragma unroll
+                            for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b] * CP, c);
+                        }
+                        mkeys[i] = 0ull;
+                        mcnt[i] = 0u;
+                    }
+                }
+                if (mentries) __syncthreads();
+            }
             // flush this (group, layer) visit to its slot, then clear
             unsigned* dst = p.scratch + ((size_t)(g + layer) * p.nfg + fg) * p.slot_words;
             if constexpr (CP == 1) {
@@ -247,7 +306,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
                     for (int u = 0; u < kBatch; ++u) {
                         if ((unsigned)f[u] >= (unsigned)p.F) continue;      // padding token / past the end
                         if (l == 0) atomicAdd(&sntok[f[u]], 1u);
-                        count_packed<KT, CP>(w[u], p.E, hist_lane + (size_t)f[u] * p.tri * CP, corr + f[u] * p.E);
+                        count_packed<KT, CP>(w[u], p.E, hist_lane + (size_t)f[u] * p.tri * CP, corr + f[u] * p.E, memo_of(f[u]));
                     }
                 }
             } else {
@@ -284,7 +343,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
                 while (qn >= 32) {
                     qn -= 32;
                     const unsigned t = wq[qn + lane];
-                    count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm, corr);
+                    count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm, corr, memo_of(0));
                 }
                 __syncwarp();
             }
@@ -441,7 +500,20 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     // four bank-spread copies of the pair bins when they fit (non-filter mode)
     const size_t bins_bytes = sizeof(unsigned) * (size_t)p.Fs * p.tri;
     const bool copies = !filter && (size_t)p.slot_words * 4 + 3 * bins_bytes + 16 <= limit;
-    const size_t smem = (size_t)p.slot_words * 4 + (filter ? queue_bytes : 0) + (copies ? 3 * bins_bytes + 16 : 0);
+    size_t smem = (size_t)p.slot_words * 4 + (filter ? queue_bytes : 0) + (copies ? 3 * bins_bytes + 16 : 0);
+    // token-set table: ids as bytes (E <= 256), packed loaders, 1024 entries per family.  Measured on
+    // B200: it pays at k = 8 (28 increments saved per hit: config 3 706 -> 555 us) and loses at k = 6
+    // (15 saved, the 64-bit CAS and the key packing cost more: config 2 71 -> 77 us), so k = 8 only.
+    p.memo_off = 0;
+    p.memo_ts = 1024;
+    if (E <= 256 && tacg_pick_kt(k, indices) == 8) {
+        const size_t off = tacg_align_up(smem, 16);
+        const size_t need = (size_t)p.Fs * p.memo_ts * (sizeof(unsigned long long) + sizeof(unsigned));
+        if (off + need <= limit) {
+            p.memo_off = (int)off;
+            smem = off + need;
+        }
+    }
     const int grid = p.groups * p.nfg;
     tacg_prof_scope prof(ctx, TACG_PROF_COACT);
     int rc = filter ? launch_hist_k<true, 1>(ctx, p, smem, grid)
