@@ -130,7 +130,7 @@ def make_sets(cfg, n_sets, rank, device):
     params = tracegen.make_params(cfg)
     sets = []
     for s in range(n_sets):
-        seed = cfg.seed + 17 * s + 1009 * rank
+        seed = rank_seed(cfg.seed, s, rank)
         bi, bf = tracegen.gen_trace(cfg, params, eval_trace=False, device=device, seed=seed)
         ei, ef = tracegen.gen_trace(cfg, params, eval_trace=True, device=device, seed=seed)
         sets.append((bi, bf, ei, ef))
@@ -190,6 +190,25 @@ def run_reference(args, cfg, rank):
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
+
+
+def rank_seed(cfg_seed, set_index, rank):
+    """Seed of trace set `set_index` on `rank`: every replica draws its own traces (replicas only)."""
+    return cfg_seed + 17 * set_index + 1009 * rank
+
+
+def max_over_ranks(ms, dist, device):
+    """The only data exchanged between ranks: the elapsed time of the timed region, reduced with MAX."""
+    if dist is None:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(units_per_step, steps, world, ms_total):
+    """Aggregate throughput of `world` independent replicas that each did units_per_step * steps units."""
+    return world * units_per_step * steps / (ms_total * 1e-3)
 
 
 def workload_config(cfg, n_sets, l2_note):
@@ -307,11 +326,7 @@ def main():
         e1.record()
         barrier()
         ctx.profile_enable(False)
-        ms = e0.elapsed_time(e1)
-        if dist is not None:
-            t = torch.tensor([ms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(e0.elapsed_time(e1), dist, dev)
         return ms, ctx.launch_count() - l0
 
     # ---- device-resident throughput (the headline `value`), clocks sampled during it
@@ -324,7 +339,7 @@ def main():
     sampler.stop()
     clocks = sampler.summary()
     units_per_step = cfg.L * (cfg.N + cfg.N_eval)
-    value = world * units_per_step * args.steps / (ms_total * 1e-3)
+    value = whole_job_value(units_per_step, args.steps, world, ms_total)
 
     # ---- roofline of the dominant kernel: same steps again with the library's event brackets on
     _, _ = timed(dev_fn, args.steps, 0, profile=True)
