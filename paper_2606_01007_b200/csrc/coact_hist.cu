@@ -146,7 +146,9 @@ __device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E,
 #pragma unroll
             for (int a = 0; a < KT; ++a) key |= (unsigned long long)(unsigned)s[a] << (8 * a);
             const unsigned h = (unsigned)((key * 0x9E3779B97F4A7C15ull) >> 40) & memo.mask;
-            const unsigned long long prev = atomicCAS(memo.keys + h, 0ull, key);
+            // plain read first: once a set is in the table a hit costs one load and one increment
+            unsigned long long prev = *reinterpret_cast<volatile unsigned long long*>(memo.keys + h);
+            if (prev == 0ull) prev = atomicCAS(memo.keys + h, 0ull, key);
             if (prev == 0ull || prev == key) {
                 atomicAdd(memo.cnt + h, 1u);
                 return;
@@ -502,7 +504,7 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     const bool copies = !filter && (size_t)p.slot_words * 4 + 3 * bins_bytes + 16 <= limit;
     size_t smem = (size_t)p.slot_words * 4 + (filter ? queue_bytes : 0) + (copies ? 3 * bins_bytes + 16 : 0);
     // token-set table: ids as bytes (E <= 256), packed loaders, 1024 entries per family.  Measured on
-    // B200: it pays at k = 8 (28 increments saved per hit: config 3 706 -> 555 us) and loses at k = 6
+    // B200: it pays at k = 8 (28 increments saved per hit: config 3 706 -> 516 us) and loses at k = 6
     // (15 saved, the 64-bit CAS and the key packing cost more: config 2 71 -> 77 us), so k = 8 only.
     p.memo_off = 0;
     p.memo_ts = 1024;
