@@ -26,6 +26,8 @@ constexpr int kEvalThreads = 512;
 constexpr int kEvalBatch = 4;        // tokens per thread with their loads in flight together
 constexpr int kCandStride = 12;      // bytes per expert in the candidate table: [0] = count, [1..9] = partitions
 constexpr unsigned kRepFlag = 0x80u; // ptab bit: the expert has at least one replica
+constexpr int kDeferCap = 64;        // deferred tokens per warp (at most 31 left over + 32 pushed)
+constexpr int kDeferWords = 9;       // ids (<= 4 words), serve bytes (2), R, pending|home|family, token offset; odd stride
 
 struct LayerTables {
     unsigned char* ptab;   // [E] primary partition | kRepFlag
@@ -137,6 +139,32 @@ __device__ __forceinline__ M serve_pending(const int (&e)[KM], unsigned pending,
             sv[j] = pick;
             R |= (M)1 << pick;
         }
+    }
+    return R;
+}
+
+// Pass 2 on packed serve bytes (KM <= 8): svp byte j = serving partition of slot j.
+template <int KM, typename M>
+__device__ __forceinline__ M serve_pending_packed(const int (&e)[KM], unsigned pending, int home, M R,
+                                                  const LayerTables& T, unsigned long long& svp) {
+    const M hb = (M)1 << home;
+    unsigned todo = pending;
+    while (todo) {
+        const int j = __ffs(todo) - 1;
+        todo &= todo - 1u;
+        int ex = e[0];
+#pragma unroll
+        for (int q = 1; q < KM; ++q) ex = (j == q) ? e[q] : ex;
+        const unsigned char* c = T.cand + ex * kCandStride;
+        const int n = c[0];
+        int pick = c[1];
+        const M loc = R | hb;
+        for (int i = 1; i <= n; ++i) {
+            const int v = c[i];
+            if ((loc >> v) & (M)1) { pick = v; break; }
+        }
+        svp = (svp & ~(0xffull << (8 * j))) | ((unsigned long long)pick << (8 * j));
+        R |= (M)1 << pick;
     }
     return R;
 }
@@ -269,6 +297,10 @@ eval_kernel(EvalParams p) {
     size_t off = carve_tables(esm, p.E, p.r, T);
     unsigned long long* dsum = reinterpret_cast<unsigned long long*>(esm + off);   off += 64 * sizeof(unsigned long long);
     unsigned* cnt = reinterpret_cast<unsigned*>(esm + off);                        // [P][32], lane-private columns
+    off += sizeof(unsigned) * (size_t)p.P * 32;
+    // deferred-token queue of each warp (replicated slots are resolved 32 tokens at a time)
+    constexpr bool kQueued = REP && KT > 0 && sizeof(M) == 4;
+    unsigned* wqueue = reinterpret_cast<unsigned*>(esm + off) + (threadIdx.x >> 5) * (kDeferCap * kDeferWords);
     __shared__ double Ls[64];              // EMA state of this layer
     __shared__ unsigned long long ltot[64];  // cumulative integer load of this layer
     __shared__ unsigned long long feas_s;
@@ -327,6 +359,49 @@ eval_kernel(EvalParams p) {
         const int16_t* base = p.indices + (size_t)layer * (size_t)p.N * (size_t)k;
         unsigned char* cost_l = p.cost ? p.cost + (size_t)layer * p.N : nullptr;
         signed char* serve_l = p.serve ? p.serve + (size_t)layer * p.N * k : nullptr;
+        long long slice0 = 0;               // first token of the slice being processed (for the queued outputs)
+        int qn = 0;                         // tokens waiting in this warp's queue (warp-uniform)
+        // loads, communication cost and outputs of one token whose serve bytes are final; returns span | remote << 16
+        auto finish_packed = [&](unsigned long long svp, M R, int hm, int o) -> unsigned {
+#pragma unroll
+            for (int j = 0; j < KM; ++j)
+                if (j < 8) atomicAdd(cnt_lane + (unsigned)((svp >> (8 * j)) & 0xffull) * 32, 1u);
+            const M notHome = ~((M)1 << hm);
+            int nR, rem;
+            if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
+            else { nR = __popc(R); rem = __popc(R & notHome); }
+            if (cost_l) cost_l[slice0 + o] = (unsigned char)rem;
+            if (serve_l) {
+                signed char* out = serve_l + ((size_t)slice0 + o) * k;
+#pragma unroll
+                for (int j = 0; j < KM; ++j)
+                    if (j < 8) out[j] = (signed char)((svp >> (8 * j)) & 0xffull);
+            }
+            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
+        };
+        // resolves the replicated slots of the last `nact` queued tokens, one token per lane
+        auto drain = [&](int nact) {
+            __syncwarp();
+            if (lane < nact) {
+                const unsigned* q = wqueue + (qn - nact + lane) * kDeferWords;
+                unsigned ww[KT > 0 ? KT / 2 : 1];
+#pragma unroll
+                for (int i = 0; i < (KT > 0 ? KT / 2 : 1); ++i) ww[i] = q[i];
+                int e[KM];
+                if constexpr (KT > 0) unpack_ids<KT>(ww, e);
+                unsigned long long svp = (unsigned long long)q[4] | ((unsigned long long)q[5] << 32);
+                const unsigned meta = q[7];
+                const int hm = (int)((meta >> 8) & 0xffu), fq = (int)(meta >> 16);
+                M R = (M)q[6];
+                if constexpr (KM <= 8) R = serve_pending_packed<KM, M>(e, meta & 0xffu, hm, R, T, svp);
+                const unsigned packed = finish_packed(svp, R, hm, (int)q[8]);
+#pragma unroll
+                for (int g = 0; g < 8; ++g)
+                    if (g < F) acc[g] += (fq == g) ? packed : 0u;
+            }
+            qn -= nact;
+            __syncwarp();
+        };
 
         for (long long mb = 0; mb < p.nmb; ++mb) {
             // steps 1-3: snapshot, guard, candidate tables
@@ -346,6 +421,7 @@ eval_kernel(EvalParams p) {
             const long long t0 = mb_begin + (long long)part * per;
             const long long t1 = min(mb_end, t0 + per);
             const int n = t1 > t0 ? (int)(t1 - t0) : 0;            // tokens of the slice (per <= 2^31 checked on the host)
+            slice0 = t0;
             int home = (int)((p.token_offset + t0 + tid) % P);
             const int8_t* fam0 = p.family + t0;
             const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
@@ -375,6 +451,10 @@ eval_kernel(EvalParams p) {
                     const int o = ob + u * kEvalThreads;
                     const bool live = (unsigned)f[u] < (unsigned)F;
                     unsigned packed = 0;
+                    bool defer = false;
+                    unsigned long long svp = 0ull;
+                    unsigned pend = 0u;
+                    M Rq = 0;
                     if (live) {
                         int e[KM], sv[KM];
                         M R;
@@ -390,27 +470,46 @@ eval_kernel(EvalParams p) {
                             for (int j = 0; j < 16; ++j)
                                 e[j] = (j < k) ? (int)__ldg(base + ((size_t)t0 + o) * k + j) : -1;
                         }
-                        if (fast) {
-                            R = serve_fast<KM, REP, M>(e, home, T, sv);
+                        bool done = true;
+                        if constexpr (kQueued) {
+                            if (fast) {
+                                // pass 1 on packed bytes; tokens with replicated slots wait in the warp's queue
 #pragma unroll
-                            for (int j = 0; j < KM; ++j) atomicAdd(cnt_lane + sv[j] * 32, 1u);
-                        } else {
-                            R = serve_token<KM, M>(e, k, E, home, T, sv);
-#pragma unroll
-                            for (int j = 0; j < KM; ++j)
-                                if (j < k && sv[j] >= 0) atomicAdd(cnt_lane + sv[j] * 32, 1u);
+                                for (int j = 0; j < KM; ++j) {
+                                    const unsigned in = T.ptab[e[j]];
+                                    const unsigned isrep = in >> 7;
+                                    svp |= (unsigned long long)(in & 63u) << (8 * j);
+                                    Rq |= (M)(isrep ^ 1u) << (in & 63u);
+                                    pend |= isrep << j;
+                                }
+                                defer = pend != 0u;
+                                done = false;
+                                if (!defer) packed = finish_packed(svp, Rq, home, o);
+                            }
                         }
-                        const M notHome = ~((M)1 << home);
-                        int nR, rem;
-                        if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
-                        else { nR = __popc(R); rem = __popc(R & notHome); }
-                        packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
-                        if (cost_l) cost_l[t0 + o] = (unsigned char)rem;
-                        if (serve_l) {
-                            signed char* out = serve_l + ((size_t)t0 + o) * k;
+                        if (done) {
+                            if (fast) {
+                                R = serve_fast<KM, REP, M>(e, home, T, sv);
 #pragma unroll
-                            for (int j = 0; j < KM; ++j)
-                                if (j < k) out[j] = (signed char)sv[j];
+                                for (int j = 0; j < KM; ++j) atomicAdd(cnt_lane + sv[j] * 32, 1u);
+                            } else {
+                                R = serve_token<KM, M>(e, k, E, home, T, sv);
+#pragma unroll
+                                for (int j = 0; j < KM; ++j)
+                                    if (j < k && sv[j] >= 0) atomicAdd(cnt_lane + sv[j] * 32, 1u);
+                            }
+                            const M notHome = ~((M)1 << home);
+                            int nR, rem;
+                            if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
+                            else { nR = __popc(R); rem = __popc(R & notHome); }
+                            packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
+                            if (cost_l) cost_l[t0 + o] = (unsigned char)rem;
+                            if (serve_l) {
+                                signed char* out = serve_l + ((size_t)t0 + o) * k;
+#pragma unroll
+                                for (int j = 0; j < KM; ++j)
+                                    if (j < k) out[j] = (signed char)sv[j];
+                            }
                         }
                     } else if (o < n) {
                         if (cost_l) cost_l[t0 + o] = 0;
@@ -421,11 +520,29 @@ eval_kernel(EvalParams p) {
                     for (int g = 0; g < 8; ++g)
                         if (g < F) acc[g] += (f[u] == g) ? packed : 0u;
                     if (layer == 0 && live) famc += 1ull << (8 * f[u]);
+                    if constexpr (kQueued) {
+                        const unsigned dm = __ballot_sync(0xffffffffu, defer);
+                        if (defer) {
+                            unsigned* q = wqueue + (qn + __popc(dm & ((1u << lane) - 1u))) * kDeferWords;
+#pragma unroll
+                            for (int i = 0; i < KT / 2; ++i) q[i] = w[u][i];
+                            q[4] = (unsigned)svp;
+                            q[5] = (unsigned)(svp >> 32);
+                            q[6] = (unsigned)Rq;
+                            q[7] = pend | ((unsigned)home << 8) | ((unsigned)f[u] << 16);
+                            q[8] = (unsigned)o;
+                        }
+                        qn += __popc(dm);
+                        if (qn >= 32) drain(32);
+                    }
                     home += stepP;
                     if (home >= P) home -= P;
                 }
-                since += U;
+                since += kQueued ? 2 * U : U;     // a queued token adds to acc when it is drained
                 if (since >= (layer == 0 ? 252 : 3800)) flush_acc();   // 8-bit / 16-bit fields must not overflow
+            }
+            if constexpr (kQueued) {
+                while (qn > 0) drain(min(qn, 32));
             }
             flush_acc();
             // step 5: integer dispatch counts of the micro-batch, then Eq. 15
@@ -569,7 +686,8 @@ __global__ void eval_zero_kernel(unsigned long long* a, size_t na, unsigned long
 }
 
 size_t eval_smem_bytes(int E, int P, int r) {
-    return tables_bytes(E, r) + 64 * sizeof(unsigned long long) + sizeof(unsigned) * (size_t)P * 32;
+    return tables_bytes(E, r) + 64 * sizeof(unsigned long long) + sizeof(unsigned) * (size_t)P * 32 +
+           (r > 0 ? sizeof(unsigned) * (size_t)(kEvalThreads / 32) * kDeferCap * kDeferWords : 0);
 }
 
 template <int KT>
