@@ -33,15 +33,19 @@ struct MmaParams {
     int cps;            // items per layer
     long long T;        // L * cps
     int groups;
-    unsigned* scratch;  // [groups+L-1][slot_words]
-    int slot_words;     // F*E*E + F, rounded up to 4
+    int nfg;            // 1: a CTA accumulates all F families; F: CTA c accumulates family c % F only
+    int Fl;             // families per CTA (F or 1)
+    unsigned* scratch;  // [(groups+L-1)*nfg][slot_words]
+    int slot_words;     // Fl*E*E + Fl, rounded up to 4
 };
 
 template <int EP>
 struct MmaGeom {
-    static constexpr int kItem = EP == 64 ? 1024 : 512;          // tokens per item
-    static constexpr int kTPT = kItem / kProducers;               // tokens per producer thread
-    static constexpr int kMaxFam = EP == 64 ? 8 : 4;              // F * EP <= 512 TMEM columns
+    static constexpr int kItem = EP == 64 ? 1024 : (EP == 128 ? 512 : 256);   // tokens scanned per item
+    static constexpr int kTPT = kItem >= kProducers ? kItem / kProducers : 1;  // tokens per producer thread
+    static constexpr int kMaxFam = EP == 64 ? 8 : (EP == 128 ? 4 : 1);         // families per CTA (TMEM columns)
+    static constexpr int kTile = EP < 128 ? EP : 128;             // M = N of one tcgen05.mma
+    static constexpr int kTiles = EP == 256 ? 3 : 1;              // EP = 256: tiles (0,0), (0,1), (1,1) of the symmetric product
     static constexpr int kChunks = kItem / 32 + kMaxFam;          // worst case chunks per item
     static constexpr int kChunkBytes = EP * 32;                   // [EP/16][32][16]
     static constexpr int kBufBytes = (kChunks + 1) * kChunkBytes; // + one all-zero chunk
@@ -114,9 +118,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) coact_mma_kernel(const MmaPara
     __shared__ uint32_t tmem_base_s;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int g = blockIdx.x;
+    const int g = blockIdx.x / p.nfg;
+    const int fsel = blockIdx.x % p.nfg;      // filter mode (nfg > 1): the one family this CTA accumulates
     const long long lo = group_lo(g, p.T, p.groups), hi = group_lo(g + 1, p.T, p.groups);
-    const int F = p.F, E = p.E;
+    const int F = p.Fl, E = p.E;              // F = families accumulated by this CTA
     constexpr uint32_t kTmemCols = 512;       // F * EP <= 512; one CTA per SM owns all of TMEM
 
     if (tid == 0) {
@@ -154,11 +159,14 @@ __global__ void __launch_bounds__(kMmaThreads, 1) coact_mma_kernel(const MmaPara
             const int16_t* lbase = p.indices + (size_t)l * (size_t)p.N * KT;
 #pragma unroll
             for (int u = 0; u < G::kTPT; ++u) {
-                const long long t = t0 + tid + u * kProducers;
+                const int ot = tid + u * kProducers;
+                const long long t = t0 + ot;
                 fam[slot][u] = -1;
-                if (t < p.N) {
-                    fam[slot][u] = p.family[t];
-                    load_words<KT>(lbase + (size_t)t * KT, w[slot][u]);
+                if (ot < G::kItem && t < p.N) {
+                    int f = p.family[t];
+                    if (p.nfg > 1) f = (f == fsel) ? 0 : -1;        // filter mode: local family 0 or skipped
+                    fam[slot][u] = f;
+                    if (f >= 0) load_words<KT>(lbase + (size_t)t * KT, w[slot][u]);
                 }
             }
         };
@@ -231,19 +239,26 @@ __global__ void __launch_bounds__(kMmaThreads, 1) coact_mma_kernel(const MmaPara
                 if (warp < 4) {
                     umma::mbar_wait(&empty_bar[cur], use & 1u);     // every MMA issued so far has completed
                     umma::tc_fence_after();
-                    unsigned* slot = p.scratch + (size_t)(g + layer) * p.slot_words;
-                    const int row = EP == 128 ? warp * 32 + lane : warp * 16 + lane;
-                    const bool row_ok = (EP == 128 || lane < 16) && row < E;
+                    unsigned* slot = p.scratch + ((size_t)(g + layer) * p.nfg + fsel) * p.slot_words;
+                    const int lrow = EP == 64 ? warp * 16 + lane : warp * 32 + lane;   // row inside a tile
+                    const bool lane_ok = EP != 64 || lane < 16;                       // M = 64: lanes 0-15 of a sub-partition
                     for (int f = 0; f < F; ++f) {
-                        for (int col = 0; col < E; col += 16) {
-                            uint32_t v[16];
-                            umma::tmem_ld_32x32b_x16(tmem + ((uint32_t)(warp * 32) << 16) + (uint32_t)(f * EP + col), v);
-                            umma::tmem_ld_wait();
-                            if (row_ok) {
-                                unsigned* dst = slot + ((size_t)f * E + row) * E + col;
 #pragma unroll
-                                for (int j = 0; j < 16; ++j)
-                                    if (col + j < E) dst[j] = v[j];
+                        for (int tile = 0; tile < G::kTiles; ++tile) {
+                            const int mi = tile == 2 ? 1 : 0, ni = tile == 0 ? 0 : 1;
+                            const int row = mi * 128 + lrow;
+                            const bool row_ok = lane_ok && row < E;
+                            for (int col = 0; col < G::kTile && ni * 128 + col < E; col += 16) {
+                                uint32_t v[16];
+                                umma::tmem_ld_32x32b_x16(tmem + ((uint32_t)(warp * 32) << 16) +
+                                                             (uint32_t)(f * EP + tile * 128 * (EP == 256) + col), v);
+                                umma::tmem_ld_wait();
+                                if (row_ok) {
+                                    unsigned* dst = slot + ((size_t)f * E + row) * E + ni * 128 + col;
+#pragma unroll
+                                    for (int j = 0; j < 16; ++j)
+                                        if (ni * 128 + col + j < E) dst[j] = v[j];
+                                }
                             }
                         }
                     }
@@ -259,7 +274,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) coact_mma_kernel(const MmaPara
         }
     } else {
         // ================================ MMA warp ================================
-        const uint32_t idesc = umma::idesc_u8_mn(EP, EP);
+        const uint32_t idesc = umma::idesc_u8_mn(G::kTile, G::kTile);
         int ci = nitems > 0 ? (int)(lo - (lo / p.cps) * p.cps) : 0;
         bool first = true;            // first item of a (CTA, layer) visit: accumulators start from zero
         uint32_t visits = 0;
@@ -289,17 +304,22 @@ __global__ void __launch_bounds__(kMmaThreads, 1) coact_mma_kernel(const MmaPara
                 for (int q = 0; q < kMaxF; ++q) {
                     if (q < F) {
                         const unsigned nch = (n[q] + 31u) >> 5;
-                        for (unsigned c = 0; c < nch; ++c) {
-                            const uint64_t d = umma::smem_desc_mn_interleave(buf + (off + c) * G::kChunkBytes, 128, 512);
-                            umma::mma_i8_ss(tmem + (uint32_t)(q * EP), d, d, idesc, (accmask >> q) & 1u);
+                        // chunk c == nch is the all-zero chunk: it clears the accumulators of a family that has no token yet
+                        const unsigned nrun = (first && nch == 0) ? 1u : nch;
+                        for (unsigned c = 0; c < nrun; ++c) {
+                            const uint32_t chunk = buf + (nch ? off + c : (unsigned)G::kChunks) * G::kChunkBytes;
+#pragma unroll
+                            for (int tile = 0; tile < G::kTiles; ++tile) {
+                                const int mi = tile == 2 ? 1 : 0, ni = tile == 0 ? 0 : 1;
+                                // a tile's 128 experts are 8 column blocks of 512 bytes
+                                const uint64_t da = umma::smem_desc_mn_interleave(chunk + mi * 4096 * (EP == 256), 128, 512);
+                                const uint64_t db = umma::smem_desc_mn_interleave(chunk + ni * 4096 * (EP == 256), 128, 512);
+                                umma::mma_i8_ss(tmem + (uint32_t)(q * EP + tile * 128 * (EP == 256)), da, db, idesc,
+                                                (accmask >> q) & 1u);
+                            }
                             accmask |= 1u << q;
                         }
                         off += nch;
-                        if (first && nch == 0) {            // no token of this family yet: clear its accumulator
-                            const uint64_t d = umma::smem_desc_mn_interleave(buf + G::kChunks * G::kChunkBytes, 128, 512);
-                            umma::mma_i8_ss(tmem + (uint32_t)(q * EP), d, d, idesc, 0u);
-                            accmask |= 1u << q;
-                        }
                     }
                 }
                 umma::mma_commit(&empty_bar[cur]);
@@ -328,12 +348,17 @@ __global__ void __launch_bounds__(512) coact_mma_finalize_kernel(const MmaParams
     const int g0 = group_of_item((long long)l * p.cps, p.T, p.groups);
     const int g1 = group_of_item((long long)(l + 1) * p.cps - 1, p.T, p.groups);
     const int ng = g1 - g0 + 1;
-    const unsigned* slot0 = p.scratch + (size_t)(g0 + l) * p.slot_words;
-    const size_t gs = (size_t)p.slot_words;
+    const int fgi = p.nfg > 1 ? f : 0;                   // which CTA of a group holds family f
+    const int fs = p.nfg > 1 ? 0 : f;                    // family index inside a slot
+    const unsigned* slot0 = p.scratch + ((size_t)(g0 + l) * p.nfg + fgi) * p.slot_words;
+    const size_t gs = (size_t)p.nfg * p.slot_words;
     unsigned* Cf = C + ((size_t)l * p.F + f) * E * E;
     unsigned* Df = D + ((size_t)l * p.F + f) * E;
     for (int idx = threadIdx.x; idx < E * E; idx += blockDim.x) {
-        const unsigned* src = slot0 + (size_t)f * E * E + idx;
+        // E > 128: the (rows >= 128, columns < 128) block is not computed; read its mirror image
+        const int ii = idx / E, jj = idx - ii * E;
+        const int sidx = (ii >= 128 && jj < 128) ? jj * E + ii : idx;
+        const unsigned* src = slot0 + (size_t)fs * E * E + sidx;
         unsigned a0 = 0, a1 = 0;
         int g = 0;
         for (; g + 2 <= ng; g += 2) {
@@ -352,7 +377,7 @@ __global__ void __launch_bounds__(512) coact_mma_finalize_kernel(const MmaParams
     }
     if (l == 0 && threadIdx.x == 0) {
         unsigned long long acc = 0;
-        for (int g = 0; g < ng; ++g) acc += slot0[(size_t)g * gs + (size_t)p.F * E * E + f];
+        for (int g = 0; g < ng; ++g) acc += slot0[(size_t)g * gs + (size_t)p.Fl * E * E + fs];
         ntok[f] = ZERO ? acc : ntok[f] + acc;
     }
 }
@@ -363,7 +388,7 @@ int launch_mma(tacg_ctx* ctx, const MmaParams& p) {
     const size_t smem = 2 * (size_t)G::kBufBytes;
     auto kern = coact_mma_kernel<EP, KT>;
     TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<p.groups, kMmaThreads, smem, ctx->stream>>>(p);
+    kern<<<p.groups * p.nfg, kMmaThreads, smem, ctx->stream>>>(p);
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
@@ -378,16 +403,16 @@ int launch_mma_k(tacg_ctx* ctx, const MmaParams& p) {
     }
 }
 
-int padded_E(int E) { return E <= 64 ? 64 : 128; }
+int padded_E(int E) { return E <= 64 ? 64 : (E <= 128 ? 128 : 256); }
 
 }  // namespace
 
-// k even and <= 8 (vector row loads), E <= 128 (one M = N = Epad accumulator tile per family),
-// F * Epad <= 512 TMEM columns.  The caller also checks the 16-byte alignment of `indices`.
+// k even and <= 8 (vector row loads), E <= 256.  All F families share a CTA when F * Epad <= 512 TMEM
+// columns and Epad <= 128; otherwise each CTA accumulates one family (Epad = 256: three 128 x 128
+// tiles of the symmetric product).  The caller also checks the 16-byte alignment of `indices`.
 bool tacg_coact_mma_supported(int k, int E, int F) {
     if (!(k == 2 || k == 4 || k == 6 || k == 8)) return false;
-    if (E < 1 || E > 128) return false;
-    return F * padded_E(E) <= 512;
+    return E >= 1 && E <= 256 && F >= 1;
 }
 
 int tacg_launch_coact_mma(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k, int L,
@@ -399,16 +424,19 @@ int tacg_launch_coact_mma(tacg_ctx* ctx, const int16_t* indices, const int8_t* f
     const int EP = padded_E(E);
     MmaParams p;
     p.indices = indices; p.family = family; p.N = N; p.k = k; p.L = L; p.E = E; p.F = F;
-    const int item = EP == 64 ? MmaGeom<64>::kItem : MmaGeom<128>::kItem;
+    const int item = EP == 64 ? MmaGeom<64>::kItem : (EP == 128 ? MmaGeom<128>::kItem : MmaGeom<256>::kItem);
+    const bool filter = EP == 256 || F * EP > 512;
+    p.nfg = filter ? F : 1;
+    p.Fl = filter ? 1 : F;
     p.cps = (int)((N + item - 1) / item);
     p.T = (long long)L * p.cps;
-    p.groups = (int)max(1ll, min((long long)ctx->sm_count, p.T));
-    p.slot_words = (int)tacg_align_up((size_t)F * E * E + F, 4);
-    const size_t slots = (size_t)p.groups + L - 1;
+    p.groups = (int)max(1ll, min((long long)(ctx->sm_count / p.nfg), p.T));
+    p.slot_words = (int)tacg_align_up((size_t)p.Fl * E * E + p.Fl, 4);
+    const size_t slots = ((size_t)p.groups + L - 1) * p.nfg;
     p.scratch = static_cast<unsigned*>(tacg_scratch(ctx, slots * p.slot_words * sizeof(unsigned)));
     if (!p.scratch) return TACG_ERR_CUDA;
     tacg_prof_scope prof(ctx, TACG_PROF_COACT);
-    int rc = EP == 64 ? launch_mma_k<64>(ctx, p) : launch_mma_k<128>(ctx, p);
+    int rc = EP == 64 ? launch_mma_k<64>(ctx, p) : (EP == 128 ? launch_mma_k<128>(ctx, p) : launch_mma_k<256>(ctx, p));
     if (rc != TACG_OK) return rc;
     unsigned long long* nt = reinterpret_cast<unsigned long long*>(ntok);
     if (zero_first) coact_mma_finalize_kernel<true><<<L * F, 512, 0, ctx->stream>>>(p, D, C, nt);

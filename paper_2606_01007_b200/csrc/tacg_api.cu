@@ -159,7 +159,7 @@ int tacg_coact_accumulate(tacg_ctx* ctx, const int16_t* indices, const int8_t* f
     if (path == TACG_PATH_MASK) return fail(ctx, TACG_ERR_SHAPE, "coact: both TACG_PATH_HIST and TACG_PATH_MMA set");
     const bool mma_ok = tacg_coact_mma_supported(k, E, F) && (reinterpret_cast<uintptr_t>(indices) % 16) == 0;
     if (path == TACG_PATH_MMA && !mma_ok)
-        return fail(ctx, TACG_ERR_SHAPE, "coact: TACG_PATH_MMA needs k in {2,4,6,8}, E<=128, F*Epad<=512 (Epad = 64 or 128), 16-byte aligned indices");
+        return fail(ctx, TACG_ERR_SHAPE, "coact: TACG_PATH_MMA needs k in {2,4,6,8}, E <= 256 and 16-byte aligned indices");
     TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     if ((flags & TACG_VALIDATE) && N > 0) {
         int rc = tacg_launch_validate_trace(ctx, indices, family, N, k, L, E, F);

@@ -58,7 +58,7 @@ def _check_invariants(cfg, N, D, C, ntok):
 
 
 @pytest.mark.parametrize("cfg_id,L,path", [(2, 26, "auto"), (3, 5, "auto"), (3, 2, "auto"), (4, 2, "auto"), (5, 1, "auto"),
-                                           (2, 26, "mma"), (3, 3, "mma")])
+                                           (2, 26, "mma"), (3, 3, "mma"), (4, 2, "mma"), (5, 1, "mma")])
 def test_coact_full_size(tacg, ctx, cfg_id, L, path):
     cfg, idx, fam = _device_trace(cfg_id, L, eval_trace=False)
     flag = tacg.TACG_PATH_MMA if path == "mma" else tacg.TACG_PATH_AUTO

@@ -57,8 +57,6 @@ PATH_FLAG = {"hist": 0x10, "auto": 0x00, "mma": 0x20}
 @pytest.mark.parametrize("cfg_id,N,L", COACT_CASES)
 def test_coact_counts_bit_exact(tacg, ctx, cfg_id, N, L, path):
     cfg, idx, fam = _trace(cfg_id, N, L)
-    if path == "mma" and cfg.E > 128:
-        pytest.skip("tcgen05 path: E <= 128 (one accumulator tile per family in 512 TMEM columns)")
     D, C, ntok = cbind.coact(idx.numpy(), fam.numpy(), cfg.E, cfg.F)
     flags = tacg.TACG_ZERO_FIRST | PATH_FLAG[path]
     out = tacg.tacg_coact_accumulate(ctx, idx.cuda(), fam.cuda(), cfg.E, cfg.F, flags=flags)
