@@ -27,7 +27,7 @@ constexpr int kEvalBatch = 4;        // tokens per thread with their loads in fl
 constexpr int kCandStride = 12;      // bytes per expert in the candidate table: [0] = count, [1..9] = partitions
 constexpr unsigned kRepFlag = 0x80u; // ptab bit: the expert has at least one replica
 constexpr int kDeferCap = 64;        // deferred tokens per warp (at most 31 left over + 32 pushed)
-constexpr int kDeferWords = 9;       // ids (<= 4 words), serve bytes (2), R, pending|home|family, token offset; odd stride
+constexpr int kDeferWords = 7;       // ids (<= 4 words), home | family << 8, token offset, pad; odd stride
 
 struct LayerTables {
     unsigned char* ptab;   // [E] primary partition | kRepFlag
@@ -379,6 +379,24 @@ eval_kernel(EvalParams p) {
             }
             return (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
         };
+        // same for a token whose serving partitions are in registers (no replicated slot)
+        auto finish_sv = [&](const int (&sv)[KM], M R, int hm, int o) -> unsigned {
+#pragma unroll
+            for (int j = 0; j < KM; ++j)
+                if (j < k) atomicAdd(cnt_lane + sv[j] * 32, 1u);
+            const M notHome = ~((M)1 << hm);
+            int nR, rem;
+            if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
+            else { nR = __popc(R); rem = __popc(R & notHome); }
+            if (cost_l) cost_l[slice0 + o] = (unsigned char)rem;
+            if (serve_l) {
+                signed char* out = serve_l + ((size_t)slice0 + o) * k;
+#pragma unroll
+                for (int j = 0; j < KM; ++j)
+                    if (j < k) out[j] = (signed char)sv[j];
+            }
+            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
+        };
         // resolves the replicated slots of the last `nact` queued tokens, one token per lane
         auto drain = [&](int nact) {
             __syncwarp();
@@ -389,15 +407,29 @@ eval_kernel(EvalParams p) {
                 for (int i = 0; i < (KT > 0 ? KT / 2 : 1); ++i) ww[i] = q[i];
                 int e[KM];
                 if constexpr (KT > 0) unpack_ids<KT>(ww, e);
-                unsigned long long svp = (unsigned long long)q[4] | ((unsigned long long)q[5] << 32);
-                const unsigned meta = q[7];
-                const int hm = (int)((meta >> 8) & 0xffu), fq = (int)(meta >> 16);
-                M R = (M)q[6];
-                if constexpr (KM <= 8) R = serve_pending_packed<KM, M>(e, meta & 0xffu, hm, R, T, svp);
-                const unsigned packed = finish_packed(svp, R, hm, (int)q[8]);
+                const unsigned meta = q[4];
+                const int hm = (int)(meta & 0xffu), fq = (int)(meta >> 8);
+                unsigned long long svp = 0ull;
+                unsigned pend = 0u;
+                M R = 0;
+                if constexpr (KM <= 8) {
 #pragma unroll
-                for (int g = 0; g < 8; ++g)
-                    if (g < F) acc[g] += (fq == g) ? packed : 0u;
+                    for (int j = 0; j < KM; ++j) {          // pass 1 again, on packed serve bytes
+                        const unsigned in = T.ptab[e[j]];
+                        const unsigned isrep = in >> 7;
+                        svp |= (unsigned long long)(in & 63u) << (8 * j);
+                        R |= (M)(isrep ^ 1u) << (in & 63u);
+                        pend |= isrep << j;
+                    }
+                    R = serve_pending_packed<KM, M>(e, pend, hm, R, T, svp);
+                }
+                const unsigned packed = finish_packed(svp, R, hm, (int)q[5]);
+#pragma unroll
+                for (int g = 0; g < 4; ++g) acc[g] += (fq == g) ? packed : 0u;
+                if (F > 4) {
+#pragma unroll
+                    for (int g = 4; g < 8; ++g) acc[g] += (fq == g) ? packed : 0u;
+                }
             }
             qn -= nact;
             __syncwarp();
@@ -452,9 +484,7 @@ eval_kernel(EvalParams p) {
                     const bool live = (unsigned)f[u] < (unsigned)F;
                     unsigned packed = 0;
                     bool defer = false;
-                    unsigned long long svp = 0ull;
                     unsigned pend = 0u;
-                    M Rq = 0;
                     if (live) {
                         int e[KM], sv[KM];
                         M R;
@@ -473,18 +503,19 @@ eval_kernel(EvalParams p) {
                         bool done = true;
                         if constexpr (kQueued) {
                             if (fast) {
-                                // pass 1 on packed bytes; tokens with replicated slots wait in the warp's queue
+                                // pass 1; a token with replicated slots waits in the warp's queue (only its ids are kept)
+                                M R1 = 0;
 #pragma unroll
                                 for (int j = 0; j < KM; ++j) {
                                     const unsigned in = T.ptab[e[j]];
                                     const unsigned isrep = in >> 7;
-                                    svp |= (unsigned long long)(in & 63u) << (8 * j);
-                                    Rq |= (M)(isrep ^ 1u) << (in & 63u);
-                                    pend |= isrep << j;
+                                    sv[j] = (int)(in & 63u);
+                                    R1 |= (M)(isrep ^ 1u) << (in & 63u);
+                                    pend |= isrep;
                                 }
                                 defer = pend != 0u;
                                 done = false;
-                                if (!defer) packed = finish_packed(svp, Rq, home, o);
+                                if (!defer) packed = finish_sv(sv, R1, home, o);
                             }
                         }
                         if (done) {
@@ -516,9 +547,13 @@ eval_kernel(EvalParams p) {
                         if (serve_l)
                             for (int j = 0; j < k; ++j) serve_l[((size_t)t0 + o) * k + j] = -1;
                     }
+                    // packed is 0 unless f[u] is a family < F, so no bound check on g is needed
 #pragma unroll
-                    for (int g = 0; g < 8; ++g)
-                        if (g < F) acc[g] += (f[u] == g) ? packed : 0u;
+                    for (int g = 0; g < 4; ++g) acc[g] += (f[u] == g) ? packed : 0u;
+                    if (F > 4) {
+#pragma unroll
+                        for (int g = 4; g < 8; ++g) acc[g] += (f[u] == g) ? packed : 0u;
+                    }
                     if (layer == 0 && live) famc += 1ull << (8 * f[u]);
                     if constexpr (kQueued) {
                         const unsigned dm = __ballot_sync(0xffffffffu, defer);
@@ -526,11 +561,8 @@ eval_kernel(EvalParams p) {
                             unsigned* q = wqueue + (qn + __popc(dm & ((1u << lane) - 1u))) * kDeferWords;
 #pragma unroll
                             for (int i = 0; i < KT / 2; ++i) q[i] = w[u][i];
-                            q[4] = (unsigned)svp;
-                            q[5] = (unsigned)(svp >> 32);
-                            q[6] = (unsigned)Rq;
-                            q[7] = pend | ((unsigned)home << 8) | ((unsigned)f[u] << 16);
-                            q[8] = (unsigned)o;
+                            q[4] = (unsigned)home | ((unsigned)f[u] << 8);
+                            q[5] = (unsigned)o;
                         }
                         qn += __popc(dm);
                         if (qn >= 32) drain(32);
