@@ -473,8 +473,9 @@ eval_kernel(EvalParams p) {
                             const uint2 v = __ldg(reinterpret_cast<const uint2*>(rows0) + o);
                             w[u][0] = v.x; w[u][1] = v.y;
                         } else if constexpr (KT > 0) {
+                            const unsigned* rp = rows0 + (size_t)o * (KT / 2);
 #pragma unroll
-                            for (int i = 0; i < KT / 2; ++i) w[u][i] = __ldg(rows0 + o * (KT / 2) + i);
+                            for (int i = 0; i < KT / 2; ++i) w[u][i] = __ldg(rp + i);
                         }
                     }
                 }
@@ -491,10 +492,10 @@ eval_kernel(EvalParams p) {
                         bool fast = false;
                         if constexpr (KT > 0) {
                             unpack_ids<KT>(w[u], e);
-                            int lo = e[0], hi = e[0];
+                            unsigned hi = (unsigned)e[0];       // a negative id is a huge unsigned value
 #pragma unroll
-                            for (int j = 1; j < KT; ++j) { lo = min(lo, e[j]); hi = max(hi, e[j]); }
-                            fast = lo >= 0 && hi < E;
+                            for (int j = 1; j < KT; ++j) hi = max(hi, (unsigned)e[j]);
+                            fast = hi < (unsigned)E;
                         } else {
 #pragma unroll
                             for (int j = 0; j < 16; ++j)
@@ -554,7 +555,9 @@ eval_kernel(EvalParams p) {
 #pragma unroll
                         for (int g = 4; g < 8; ++g) acc[g] += (f[u] == g) ? packed : 0u;
                     }
-                    if (layer == 0 && live) famc += 1ull << (8 * f[u]);
+                    if (layer == 0) {                   // uniform branch: only the CTAs of layer 0 count families
+                        if (live) famc += 1ull << (8 * f[u]);
+                    }
                     if constexpr (kQueued) {
                         const unsigned dm = __ballot_sync(0xffffffffu, defer);
                         if (defer) {
