@@ -87,7 +87,7 @@ __device__ __forceinline__ double rel_adv(const double* x, int E, int F, int f, 
     return x[f * E + e] - other;
 }
 
-// One CTA per layer.  Dynamic smem: u[F][E], c[F][E], sc[F][E] doubles.
+// One CTA per layer.  Dynamic smem: u[F][E], c[F][E], sc[F][E], dv[F][E] doubles.
 __global__ void __launch_bounds__(256)
 pref_kernel(const unsigned* __restrict__ D, const unsigned long long* __restrict__ ntok, int E, int F, double tau,
             double eps, AffScratch s, float* __restrict__ pref_out) {
@@ -96,6 +96,7 @@ pref_kernel(const unsigned* __restrict__ D, const unsigned long long* __restrict
     double* u = psm;
     double* c = psm + (size_t)F * E;
     double* sc = psm + (size_t)2 * F * E;
+    double* dv = psm + (size_t)3 * F * E;
     const int l = blockIdx.x;
     const unsigned* Dl = D + (size_t)l * F * E;
     // Warp f owns family f (F <= 8 = warps of the CTA): every sum over experts is a warp reduction,
@@ -113,21 +114,26 @@ pref_kernel(const unsigned* __restrict__ D, const unsigned long long* __restrict
         }
     }
     __syncthreads();
-    // O3, O4: relative advantage (Eq. 2-3) and z-score over experts (Eq. 4), summed into s (Eq. 5)
+    // O3, O4: relative advantage (Eq. 2-3) and z-score over experts (Eq. 4), summed into s (Eq. 5).
+    // The relative advantages of a pass are computed once into dv (owned by warp f) and reused.
     if (f < F) {
         for (int e = lane; e < E; e += 32) sc[f * E + e] = 0.0;
         for (int pass = 0; pass < 2; ++pass) {
             const double* x = pass == 0 ? u : c;
             double part = 0.0;
-            for (int e = lane; e < E; e += 32) part += rel_adv(x, E, F, f, e);
+            for (int e = lane; e < E; e += 32) {
+                const double d = rel_adv(x, E, F, f, e);
+                dv[f * E + e] = d;
+                part += d;
+            }
             const double mu = warp_sum(part) / (double)E;
             double vpart = 0.0;
             for (int e = lane; e < E; e += 32) {
-                const double d = rel_adv(x, E, F, f, e) - mu;
+                const double d = dv[f * E + e] - mu;
                 vpart += d * d;
             }
             const double sigma = sqrt(warp_sum(vpart) / (double)E);
-            for (int e = lane; e < E; e += 32) sc[f * E + e] += (rel_adv(x, E, F, f, e) - mu) / (sigma + eps);
+            for (int e = lane; e < E; e += 32) sc[f * E + e] += (dv[f * E + e] - mu) / (sigma + eps);
         }
     }
     __syncthreads();
@@ -273,7 +279,7 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     tacg_prof_scope prof(ctx, TACG_PROF_AFFINITY);
     rowstats_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, s);
     TACG_LAUNCH_CHECK(ctx);
-    const size_t psm = sizeof(double) * (size_t)3 * F * E;
+    const size_t psm = sizeof(double) * (size_t)4 * F * E;
     TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(pref_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
     pref_kernel<<<L, 256, psm, ctx->stream>>>(D, nt, E, F, tau, eps, s, pref);
     TACG_LAUNCH_CHECK(ctx);

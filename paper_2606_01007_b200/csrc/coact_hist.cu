@@ -368,9 +368,14 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
     const int i = blockIdx.x * 8 + warp;
     const int fgi = p.nfg > 1 ? f : 0;                   // which CTA of a group holds family f
     const int fs = p.nfg > 1 ? 0 : f;                    // family index inside a slot
-    const int g0 = group_of_item((long long)l * p.cps, p.T, p.groups);
-    const int g1 = group_of_item((long long)(l + 1) * p.cps - 1, p.T, p.groups);
-    const int ng = g1 - g0 + 1;
+    __shared__ int g01[2];                               // first and last group that visited the layer
+    if (threadIdx.x == 0) {
+        g01[0] = group_of_item((long long)l * p.cps, p.T, p.groups);
+        g01[1] = group_of_item((long long)(l + 1) * p.cps - 1, p.T, p.groups);
+    }
+    __syncthreads();
+    const int g0 = g01[0];
+    const int ng = g01[1] - g0 + 1;
     const unsigned* slot0 = p.scratch + ((size_t)(g0 + l) * p.nfg + fgi) * p.slot_words;
     const size_t gstride = (size_t)p.nfg * p.slot_words;
     if (l == 0 && blockIdx.x == 0 && warp == 0) {         // slots are read one per lane, then reduced
@@ -391,15 +396,16 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
         unsigned v = 0;
         if (j != i) {
             const unsigned* src = bins + (j > i ? ri + j : tri_row(j, E) + i);
+            // eight predicated, independent loads per round: every slot of a typical layer is in flight at once
             unsigned a0 = 0, a1 = 0, a2 = 0, a3 = 0;
-            int g = 0;
-            for (; g + 4 <= ng; g += 4) {
-                a0 += src[(size_t)g * gstride];
-                a1 += src[(size_t)(g + 1) * gstride];
-                a2 += src[(size_t)(g + 2) * gstride];
-                a3 += src[(size_t)(g + 3) * gstride];
+            for (int g = 0; g < ng; g += 8) {
+                const unsigned* s8 = src + (size_t)g * gstride;
+                const int left = ng - g;
+                unsigned x[8];
+#pragma unroll
+                for (int q = 0; q < 8; ++q) x[q] = q < left ? s8[(size_t)q * gstride] : 0u;
+                a0 += x[0] + x[4]; a1 += x[1] + x[5]; a2 += x[2] + x[6]; a3 += x[3] + x[7];
             }
-            for (; g < ng; ++g) a0 += src[(size_t)g * gstride];
             v = (a0 + a1) + (a2 + a3);
         }
         rs += v;
