@@ -49,7 +49,6 @@ struct MmaGeom {
     static constexpr int kChunks = kItem / 32 + kMaxFam;          // worst case chunks per item
     static constexpr int kChunkBytes = EP * 32;                   // [EP/16][32][16]
     static constexpr int kBufBytes = (kChunks + 1) * kChunkBytes; // + one all-zero chunk
-    static constexpr int kWords = EP / 32;                        // mask words per token
 };
 
 __device__ __forceinline__ void producer_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(kProducers) : "memory"); }

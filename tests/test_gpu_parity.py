@@ -127,6 +127,15 @@ def test_coact_empty_and_errors(tacg, ctx):
     idx2 = torch.tensor([[[0, 1], [2, 9]]], dtype=torch.int16, device=dev)
     assert ctx.tacg_coact_accumulate(idx2, fam[:2].contiguous(), 2, 2, 1, 4, 1, D, Cm, nt, tacg.TACG_VALIDATE) == -3
     assert "record 1" in ctx.detail()
+    # the tensor path refuses what it cannot do (odd k, E > 256) before touching the outputs
+    big = torch.zeros((1, 8, 2), dtype=torch.int16, device=dev)
+    Db = torch.zeros((1, 1, 300), dtype=torch.int32, device=dev)
+    Cb = torch.zeros((1, 1, 300, 300), dtype=torch.int32, device=dev)
+    assert ctx.tacg_coact_accumulate(big, fam, 8, 2, 1, 300, 1, Db, Cb, nt, tacg.TACG_PATH_MMA) == -2
+    odd = torch.zeros((1, 8, 3), dtype=torch.int16, device=dev)
+    assert ctx.tacg_coact_accumulate(odd, fam, 8, 3, 1, 4, 1, D, Cm, nt, tacg.TACG_PATH_MMA) == -2
+    assert ctx.tacg_coact_accumulate(idx, fam, 8, 2, 1, 4, 1, D, Cm, nt,
+                                     tacg.TACG_PATH_MMA | tacg.TACG_PATH_HIST) == -2          # both paths forced
     idx3 = torch.tensor([[[0, 1], [2, 3]]], dtype=torch.int16, device=dev)
     assert ctx.tacg_coact_accumulate(idx3, fam[:2].contiguous(), 2, 2, 1, 4, 1, D, Cm, nt, tacg.TACG_VALIDATE) == 0
 
