@@ -287,7 +287,8 @@ __device__ __forceinline__ void load_row_raw(const int16_t* __restrict__ row, un
 
 // KT: compile-time k (0 = generic), REP: a replica table is present, M: partition-set mask type
 // (unsigned for P <= 32, else unsigned long long).
-template <int KT, bool REP, typename M>
+// OUT: per-token outputs (cost_per_token / serve) were requested.
+template <int KT, bool REP, typename M, bool OUT>
 __global__ void __launch_bounds__(kEvalThreads, 2)
 eval_kernel(EvalParams p) {
     extern __shared__ __align__(16) unsigned char esm[];
@@ -326,30 +327,24 @@ eval_kernel(EvalParams p) {
         if (tid < 16) comm_s[tid] = 0ull;
         if (tid < 8) fam_s[tid] = 0u;
         __syncthreads();
-        unsigned acc[8];                    // per family: sum of span | remote << 16 over this thread's tokens
+        // per family, over this thread's tokens: span (bits 0-10) | remote (11-21) | token count (22-31)
+        unsigned acc[8];
 #pragma unroll
         for (int g = 0; g < 8; ++g) acc[g] = 0u;
         int since = 0;                      // tokens added to acc since the last flush (uniform per warp)
-        unsigned long long famc = 0ull;     // layer 0: tokens per family of this thread, 8-bit fields
         auto flush_acc = [&]() {
-            if (layer == 0) {
-#pragma unroll
-                for (int g = 0; g < 8; ++g) {
-                    if (g < F) {
-                        const unsigned c = __reduce_add_sync(0xffffffffu, (unsigned)(famc >> (8 * g)) & 0xffu);
-                        if (lane == 0 && c) atomicAdd(&fam_s[g], c);
-                    }
-                }
-                famc = 0ull;
-            }
 #pragma unroll
             for (int g = 0; g < 8; ++g) {
                 if (g < F) {
-                    const unsigned s = __reduce_add_sync(0xffffffffu, acc[g] & 0xffffu);
-                    const unsigned q = __reduce_add_sync(0xffffffffu, acc[g] >> 16);
+                    const unsigned s = __reduce_add_sync(0xffffffffu, acc[g] & 0x7ffu);
+                    const unsigned q = __reduce_add_sync(0xffffffffu, (acc[g] >> 11) & 0x7ffu);
                     if (lane == 0) {
                         if (s) atomicAdd(&comm_s[g], (unsigned long long)s);
                         if (q) atomicAdd(&comm_s[8 + g], (unsigned long long)q);
+                    }
+                    if (layer == 0) {               // tokens per family, counted once (family is shared by all layers)
+                        const unsigned c = __reduce_add_sync(0xffffffffu, acc[g] >> 22);
+                        if (lane == 0 && c) atomicAdd(&fam_s[g], c);
                     }
                     acc[g] = 0u;
                 }
@@ -357,11 +352,11 @@ eval_kernel(EvalParams p) {
             since = 0;
         };
         const int16_t* base = p.indices + (size_t)layer * (size_t)p.N * (size_t)k;
-        unsigned char* cost_l = p.cost ? p.cost + (size_t)layer * p.N : nullptr;
-        signed char* serve_l = p.serve ? p.serve + (size_t)layer * p.N * k : nullptr;
+        unsigned char* cost_l = (OUT && p.cost) ? p.cost + (size_t)layer * p.N : nullptr;
+        signed char* serve_l = (OUT && p.serve) ? p.serve + (size_t)layer * p.N * k : nullptr;
         long long slice0 = 0;               // first token of the slice being processed (for the queued outputs)
         int qn = 0;                         // tokens waiting in this warp's queue (warp-uniform)
-        // loads, communication cost and outputs of one token whose serve bytes are final; returns span | remote << 16
+        // loads, communication cost and outputs of one token whose serve bytes are final; returns span | remote << 11 | 1 << 22
         auto finish_packed = [&](unsigned long long svp, M R, int hm, int o) -> unsigned {
 #pragma unroll
             for (int j = 0; j < KM; ++j)
@@ -370,14 +365,14 @@ eval_kernel(EvalParams p) {
             int nR, rem;
             if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
             else { nR = __popc(R); rem = __popc(R & notHome); }
-            if (cost_l) cost_l[slice0 + o] = (unsigned char)rem;
-            if (serve_l) {
+            if (OUT && cost_l) cost_l[slice0 + o] = (unsigned char)rem;
+            if (OUT && serve_l) {
                 signed char* out = serve_l + ((size_t)slice0 + o) * k;
 #pragma unroll
                 for (int j = 0; j < KM; ++j)
                     if (j < 8) out[j] = (signed char)((svp >> (8 * j)) & 0xffull);
             }
-            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
+            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 11) | (1u << 22);
         };
         // same for a token whose serving partitions are in registers (no replicated slot)
         auto finish_sv = [&](const int (&sv)[KM], M R, int hm, int o) -> unsigned {
@@ -388,14 +383,14 @@ eval_kernel(EvalParams p) {
             int nR, rem;
             if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
             else { nR = __popc(R); rem = __popc(R & notHome); }
-            if (cost_l) cost_l[slice0 + o] = (unsigned char)rem;
-            if (serve_l) {
+            if (OUT && cost_l) cost_l[slice0 + o] = (unsigned char)rem;
+            if (OUT && serve_l) {
                 signed char* out = serve_l + ((size_t)slice0 + o) * k;
 #pragma unroll
                 for (int j = 0; j < KM; ++j)
                     if (j < k) out[j] = (signed char)sv[j];
             }
-            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
+            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 11) | (1u << 22);
         };
         // resolves the replicated slots of the last `nact` queued tokens, one token per lane
         auto drain = [&](int nact) {
@@ -534,9 +529,9 @@ eval_kernel(EvalParams p) {
                             int nR, rem;
                             if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
                             else { nR = __popc(R); rem = __popc(R & notHome); }
-                            packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 16);
-                            if (cost_l) cost_l[t0 + o] = (unsigned char)rem;
-                            if (serve_l) {
+                            packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 11) | (1u << 22);
+                            if (OUT && cost_l) cost_l[t0 + o] = (unsigned char)rem;
+                            if (OUT && serve_l) {
                                 signed char* out = serve_l + ((size_t)t0 + o) * k;
 #pragma unroll
                                 for (int j = 0; j < KM; ++j)
@@ -544,8 +539,8 @@ eval_kernel(EvalParams p) {
                             }
                         }
                     } else if (o < n) {
-                        if (cost_l) cost_l[t0 + o] = 0;
-                        if (serve_l)
+                        if (OUT && cost_l) cost_l[t0 + o] = 0;
+                        if (OUT && serve_l)
                             for (int j = 0; j < k; ++j) serve_l[((size_t)t0 + o) * k + j] = -1;
                     }
                     // packed is 0 unless f[u] is a family < F, so no bound check on g is needed
@@ -554,9 +549,6 @@ eval_kernel(EvalParams p) {
                     if (F > 4) {
 #pragma unroll
                         for (int g = 4; g < 8; ++g) acc[g] += (f[u] == g) ? packed : 0u;
-                    }
-                    if (layer == 0) {                   // uniform branch: only the CTAs of layer 0 count families
-                        if (live) famc += 1ull << (8 * f[u]);
                     }
                     if constexpr (kQueued) {
                         const unsigned dm = __ballot_sync(0xffffffffu, defer);
@@ -574,7 +566,7 @@ eval_kernel(EvalParams p) {
                     if (home >= P) home -= P;
                 }
                 since += kQueued ? 2 * U : U;     // a queued token adds to acc when it is drained
-                if (since >= (layer == 0 ? 252 : 3800)) flush_acc();   // 8-bit / 16-bit fields must not overflow
+                if (since >= 120) flush_acc();      // 11-bit fields: 124 tokens x (span <= 15, remote <= 16) fit
             }
             if constexpr (kQueued) {
                 while (qn > 0) drain(min(qn, 32));
@@ -729,9 +721,15 @@ template <int KT>
 int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     const size_t smem = eval_smem_bytes(p.E, p.P, p.r);
     const bool rep = p.replicas != nullptr && p.r > 0;
-    void (*kern)(EvalParams) =
-        p.P <= 32 ? (rep ? eval_kernel<KT, true, unsigned> : eval_kernel<KT, false, unsigned>)
-                  : (rep ? eval_kernel<KT, true, unsigned long long> : eval_kernel<KT, false, unsigned long long>);
+    const bool out = p.cost != nullptr || p.serve != nullptr;
+    void (*kern)(EvalParams);
+    if (p.P <= 32) {
+        kern = rep ? (out ? eval_kernel<KT, true, unsigned, true> : eval_kernel<KT, true, unsigned, false>)
+                   : (out ? eval_kernel<KT, false, unsigned, true> : eval_kernel<KT, false, unsigned, false>);
+    } else {
+        kern = rep ? (out ? eval_kernel<KT, true, unsigned long long, true> : eval_kernel<KT, true, unsigned long long, false>)
+                   : (out ? eval_kernel<KT, false, unsigned long long, true> : eval_kernel<KT, false, unsigned long long, false>);
+    }
     int occ = 0;
     TACG_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kEvalThreads, smem));
     if (occ < 1) occ = 1;
