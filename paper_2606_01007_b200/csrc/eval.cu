@@ -731,6 +731,8 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
                    : (out ? eval_kernel<KT, false, unsigned long long, true> : eval_kernel<KT, false, unsigned long long, false>);
     }
     int occ = 0;
+    // the largest shapes (E = 512, P = 64, r = 8) need a little more than the 48 KB default
+    TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     TACG_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kEvalThreads, smem));
     if (occ < 1) occ = 1;
     const int max_grid = ctx->sm_count * occ;

@@ -336,3 +336,30 @@ def test_eval_validate_placement(tacg, ctx):
                                  torch.from_numpy(rep).cuda(), flags=tacg.TACG_VALIDATE)
     tacg.tacg_eval_placement(ctx, idx.cuda(), fam.cuda(), cfg.E, cfg.F, cfg.P, torch.from_numpy(primary).cuda(),
                              flags=tacg.TACG_VALIDATE)
+
+
+def test_limits_of_the_abi(tacg, ctx):
+    """The largest shapes tacg.h admits (E = 512, P = 64, F = 8, r = 8, k = 16): global-atomic
+    co-activation fallback, 64-bit partition masks, generic-k loaders, > 48 KB of shared memory."""
+    rng = np.random.default_rng(11)
+    E, k, F, P, r, N, L = 512, 16, 8, 64, 8, 3000, 2
+    idx = np.stack([np.stack([rng.permutation(E)[:k] for _ in range(N)]) for _ in range(L)]).astype(np.int16)
+    idx[rng.random(idx.shape) < 0.05] = -1
+    fam = rng.integers(0, F, size=N).astype(np.int8)
+    D, C, ntok = cbind.coact(idx, fam, E, F)
+    out = tacg.tacg_coact_accumulate(ctx, torch.from_numpy(idx).cuda(), torch.from_numpy(fam).cuda(), E, F,
+                                     flags=tacg.TACG_ZERO_FIRST)
+    torch.cuda.synchronize()
+    assert (_u32(out["D"]) == D).all() and (_u32(out["C"]) == C).all() and (_u64(out["ntok"]) == ntok).all()
+    primary = tracegen.random_placement(E, P, 8, L, seed=3)
+    replicas = tracegen.random_replicas(primary, P, r, 40, seed=4)
+    want = cbind.eval_placement(idx, fam, E, F, P, primary, replicas, theta=0.1, rho=0.9, microbatch=500,
+                                token_offset=3, want_cost=True, want_serve=True, load_state=np.zeros((L, P)))
+    st = torch.zeros((L, P), dtype=torch.float64, device="cuda")
+    got = tacg.tacg_eval_placement(ctx, torch.from_numpy(idx).cuda(), torch.from_numpy(fam).cuda(), E, F, P,
+                                   torch.from_numpy(primary).cuda(), torch.from_numpy(replicas).cuda(), theta=0.1,
+                                   rho=0.9, microbatch=500, token_offset=3, load_state=st, want_cost=True,
+                                   want_serve=True)
+    torch.cuda.synchronize()
+    got["load_state"] = st
+    _assert_eval_equal(want, got)
