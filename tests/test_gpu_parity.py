@@ -363,3 +363,32 @@ def test_limits_of_the_abi(tacg, ctx):
     torch.cuda.synchronize()
     got["load_state"] = st
     _assert_eval_equal(want, got)
+
+
+def test_unaligned_indices_take_the_generic_loaders(tacg, ctx):
+    """A trace whose device pointer is not 16-byte aligned (a view one element into a buffer) must give
+    the same results through the 2-byte loaders."""
+    cfg, idx, fam = _trace(2, 5003, 2)
+    flat = torch.empty(idx.numel() + 1, dtype=torch.int16, device="cuda")
+    flat[1:] = idx.reshape(-1).cuda()
+    view = flat[1:].view(idx.shape)
+    assert view.data_ptr() % 16 != 0
+    D, C, ntok = cbind.coact(idx.numpy(), fam.numpy(), cfg.E, cfg.F)
+    out = tacg.tacg_coact_accumulate(ctx, view, fam.cuda(), cfg.E, cfg.F, flags=tacg.TACG_ZERO_FIRST)
+    torch.cuda.synchronize()
+    assert (_u32(out["D"]) == D).all() and (_u32(out["C"]) == C).all() and (_u64(out["ntok"]) == ntok).all()
+    primary = tracegen.random_placement(cfg.E, cfg.P, cfg.capacity, cfg.L, seed=5)
+    replicas = tracegen.random_replicas(primary, cfg.P, 2, 6, seed=6)
+    want = cbind.eval_placement(idx.numpy(), fam.numpy(), cfg.E, cfg.F, cfg.P, primary, replicas, theta=0.15, rho=0.995,
+                                microbatch=1000, want_cost=True, want_serve=True, load_state=np.zeros((cfg.L, cfg.P)))
+    st = torch.zeros((cfg.L, cfg.P), dtype=torch.float64, device="cuda")
+    got = tacg.tacg_eval_placement(ctx, view, fam.cuda(), cfg.E, cfg.F, cfg.P, torch.from_numpy(primary).cuda(),
+                                   torch.from_numpy(replicas).cuda(), theta=0.15, rho=0.995, microbatch=1000,
+                                   load_state=st, want_cost=True, want_serve=True)
+    torch.cuda.synchronize()
+    got["load_state"] = st
+    _assert_eval_equal(want, got)
+    # the tensor path needs aligned rows and says so
+    D0 = torch.zeros_like(out["D"]); C0 = torch.zeros_like(out["C"]); n0 = torch.zeros_like(out["ntok"])
+    assert ctx.tacg_coact_accumulate(view, fam.cuda(), idx.shape[1], cfg.k, cfg.L, cfg.E, cfg.F, D0, C0, n0,
+                                     tacg.TACG_PATH_MMA) == -2
