@@ -5,11 +5,13 @@
 //                          (layer, token-chunk) items and keeps a PRIVATE strict-upper-triangular
 //                          uint32 pair histogram in shared memory (all F families when they fit,
 //                          else one family per CTA with the tokens of that family compacted through
-//                          a per-warp queue).  It is written once per (CTA, layer) to a scratch slot
-//                          with 16-byte stores.
-//   coact_finalize_kernel  one CTA per (layer, family): sums the slots of that layer, mirrors the
-//                          triangle into the symmetric C (zero diagonal untouched), derives D, adds
-//                          ntok.  With TACG_ZERO_FIRST it stores, otherwise it adds to what is there.
+//                          a per-warp queue).  Four bank-spread copies of the bins when they fit; for
+//                          k = 8 a small token-set table short-cuts repeated expert sets.  The
+//                          histogram is written once per (CTA, layer) to a scratch slot.
+//   coact_finalize_kernel  grid (E/8, L*F), one warp per output row: sums the slots of the layer (L2
+//                          resident), mirrors the triangle into the symmetric C, derives D, adds ntok.
+//                          With TACG_ZERO_FIRST it stores (diagonal cleared), otherwise it adds to what
+//                          is there (diagonal untouched).
 //
 // D is not counted with its own atomics.  A token with all k slots valid and distinct puts each of
 // its experts into exactly k-1 pair increments, so D[e] = (sum of the pair bins touching e) / (k-1);
