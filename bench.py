@@ -285,7 +285,6 @@ def main():
     remote = torch.empty((L, F), dtype=torch.int64, device=dev)
     ntok_e = torch.empty((F,), dtype=torch.int64, device=dev)
     fair = torch.empty((L + 1, 3), dtype=torch.float32, device=dev)
-    state = torch.zeros((L, P), dtype=torch.float64, device=dev)
 
     # placement used by the step: local search on the first build trace, GESR table per config
     bi0, bf0, _, _ = sets[0]
@@ -301,9 +300,8 @@ def main():
                   "tacg_coact_accumulate")
         ctx.check(ctx.tacg_affinity_swapgain(D, Cm, ntok, L, E, F, P, cfg.capacity, primary, 0.25, 1.0, 1e-6,
                                              pref, W, aff, gain), "tacg_affinity_swapgain")
-        state.zero_()
         ctx.check(ctx.tacg_eval_placement(ei, ef, cfg.N_eval, k, L, E, F, P, primary, replicas, r, 0.15, 0.995,
-                                          cfg.microbatch, 0, state, load, span, remote, ntok_e, fair, None, None, 0),
+                                          cfg.microbatch, 0, None, load, span, remote, ntok_e, fair, None, None, 0),
                   "tacg_eval_placement")
 
     def barrier():
