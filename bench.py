@@ -232,6 +232,8 @@ def main():
     ap.add_argument("--impl", default="tacg", choices=["tacg", "reference"])
     ap.add_argument("--sets", type=int, default=0, help="distinct trace sets rotated over (0 = enough to exceed L2)")
     ap.add_argument("--path", default="auto", choices=["auto", "hist", "mma"])
+    ap.add_argument("--compare-paths", action="store_true",
+                    help="also time tacg_coact_accumulate alone on both paths (histogram, tcgen05 kind::i8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -357,6 +359,28 @@ def main():
         "other_kernels_avg_ms": {"affinity_swapgain(4 kernels)": af_ms / max(1, af_n), "eval_kernel": ev_ms / max(1, ev_n)},
     }
 
+    # ---- optional: the co-activation call alone on both paths
+    coact_paths = None
+    if args.compare_paths:
+        coact_paths = {}
+        epad = 64 if E <= 64 else (128 if E <= 128 else 256)
+        for name, flag in (("hist", tacg.TACG_PATH_HIST), ("mma", tacg.TACG_PATH_MMA)):
+            def one(i, flag=flag):
+                bi, bf, _, _ = sets[i % n_sets]
+                ctx.check(ctx.tacg_coact_accumulate(bi, bf, cfg.N, k, L, E, F, D, Cm, ntok, tacg.TACG_ZERO_FIRST | flag),
+                          "tacg_coact_accumulate")
+            try:
+                timed(one, max(3, min(args.steps, 20)), 3, profile=True)
+            except Exception as exc:                         # shape not supported by the tensor path
+                coact_paths[name] = {"unsupported": str(exc)}
+                continue
+            ms, n = ctx.profile_read(tacg.TACG_PROF_COACT)
+            avg = ms / max(1, n)
+            coact_paths[name] = {"avg_call_ms": avg, "routed_tokens_per_s": cfg.L * cfg.N / (avg * 1e-3),
+                                 "hbm_frac": abytes / (avg * 1e-3) / 1e9 / peak}
+        coact_paths["useful_over_dense"] = (k * (k - 1) / 2) / float(epad * epad)
+        coact_paths["note"] = "tensor path: Epad^2 MACs per token in kind::i8 against k(k-1)/2 useful increments"
+
     # ---- end to end through host buffers: H2D of both traces, the calls, D2H of the results
     e2e = None
     if not args.no_e2e:
@@ -407,6 +431,8 @@ def main():
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "coact_path": used_path, "local_search_swaps_mean": float(np.mean(swaps)),
         }
+        if coact_paths is not None:
+            line["coact_paths"] = coact_paths
         print(json.dumps(line), flush=True)
     ctx.close()
     if dist is not None:
