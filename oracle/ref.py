@@ -406,3 +406,54 @@ def replica_table(Abar: np.ndarray, aff: np.ndarray, primary: Sequence[int], n_r
         for i, m in enumerate(cands[:r]):
             rep[e, i] = m
     return rep
+
+
+# --------------------------------------------------------------------------
+# O13 -- GESR offline scoring with lambda1, lambda2 != 0.
+# PAPER.md:132-138, Eq. 11: r_e = Cent_e + lambda1 Cons_e - lambda2 Spec_e with
+#   Cent_e = sum_e' Abar[e,e']                                   (pooled coactivation)
+#   Cons_e = average over families of the cosine similarity between the expert's
+#            family-specific coactivation profile A^f[e,:] and the mean profile Abar[e,:]
+#   Spec_e = maximum deviation from that mean profile across families.
+# Readings (Q29-Q31): the cosine of a zero vector with anything is 0; the
+# "deviation" is the Euclidean norm of A^f[e,:] - Abar[e,:]; ties in the top-n_rep
+# selection and among secondaries go to the lower id.  A^f and Abar as in O2/O6
+# (A^f = C^f / max(1, N_f), Abar = mean over families, readings Q2, Q4).
+# --------------------------------------------------------------------------
+def gesr_scores(C: np.ndarray, ntok: np.ndarray, lam1: float, lam2: float) -> Dict[str, np.ndarray]:
+    """C: counts [F,E,E] of one layer; returns cent, cons, spec, score as float64[E]."""
+    F, E, _ = C.shape
+    A = [[[float(C[f][i][j]) / max(1.0, float(ntok[f])) for j in range(E)] for i in range(E)] for f in range(F)]
+    Abar = [[sum(A[f][i][j] for f in range(F)) / F for j in range(E)] for i in range(E)]
+    cent, cons, spec, score = [], [], [], []
+    for e in range(E):
+        mean = Abar[e]
+        nm = math.sqrt(sum(v * v for v in mean))
+        c_e = sum(mean)
+        cos_sum = 0.0
+        dev_max = 0.0
+        for f in range(F):
+            row = A[f][e]
+            nr = math.sqrt(sum(v * v for v in row))
+            dot = sum(row[j] * mean[j] for j in range(E))
+            cos_sum += dot / (nr * nm) if nr > 0.0 and nm > 0.0 else 0.0
+            dev = math.sqrt(sum((row[j] - mean[j]) ** 2 for j in range(E)))
+            dev_max = max(dev_max, dev)
+        cent.append(c_e)
+        cons.append(cos_sum / F)
+        spec.append(dev_max)
+        score.append(c_e + lam1 * (cos_sum / F) - lam2 * dev_max)
+    return {"cent": np.array(cent), "cons": np.array(cons), "spec": np.array(spec), "score": np.array(score)}
+
+
+def gesr_replica_table(score: Sequence[float], aff: np.ndarray, primary: Sequence[int], n_rep: int, r: int) -> np.ndarray:
+    """Eq. 12: the n_rep top-scoring experts keep their primary and receive the r non-primary
+    partitions with the largest affinity aff[e,m]; -1 elsewhere.  Ties -> lower id."""
+    E, P = aff.shape
+    order = sorted(range(E), key=lambda e: (-float(score[e]), e))
+    rep = np.full((E, r), -1, dtype=np.int64)
+    for e in order[:n_rep]:
+        cands = sorted((m for m in range(P) if m != int(primary[e])), key=lambda m: (-float(aff[e, m]), m))
+        for i, m in enumerate(cands[:r]):
+            rep[e, i] = m
+    return rep

@@ -460,3 +460,69 @@ def test_replica_table_and_comm_reduction_plausibility():
         assert primary[e] not in rep[e] and len(set(rep[e])) == 2
         others = [m for m in range(cfg.P) if m != primary[e]]
         assert aff[e, rep[e, 0]] == max(aff[e, m] for m in others)
+
+
+# --------------------------------------------------------------------------- O13 GESR scoring (Eq. 11)
+def test_gesr_scores_handworked_and_special_cases():
+    # hand-worked: E=3, F=2, N_f=1.  Expert 0 co-activates with expert 1 in family 0 and with
+    # expert 2 in family 1: profiles (0,1,0) and (0,0,1), mean (0,.5,.5).
+    C = np.zeros((2, 3, 3), dtype=np.int64)
+    C[0, 0, 1] = C[0, 1, 0] = 1
+    C[1, 0, 2] = C[1, 2, 0] = 1
+    s = ref.gesr_scores(C, np.array([1, 1]), lam1=2.0, lam2=3.0)
+    assert s["cent"][0] == pytest.approx(1.0)                       # .5 + .5
+    assert s["cons"][0] == pytest.approx(0.5 / math.sqrt(0.5))      # both cosines = .5 / (1 * sqrt(.5))
+    assert s["spec"][0] == pytest.approx(math.sqrt(0.5))            # ||(0,.5,-.5)||
+    assert s["score"][0] == pytest.approx(1.0 + 2.0 * math.sqrt(0.5) - 3.0 * math.sqrt(0.5))
+    # expert 1: profiles (1,0,0) and (0,0,0): mean (.5,0,0); cosines 1 and 0 (zero vector, reading Q29)
+    assert s["cent"][1] == pytest.approx(0.5)
+    assert s["cons"][1] == pytest.approx(0.5)
+    assert s["spec"][1] == pytest.approx(0.5)
+    # identical families (C^f proportional to N_f): consistency 1, no specificity, any lambda
+    rng = np.random.default_rng(3)
+    B = rng.integers(1, 9, size=(5, 5)); B = B + B.T; np.fill_diagonal(B, 0)
+    Cs = np.stack([B * 2, B * 6, B * 10])
+    s = ref.gesr_scores(Cs, np.array([2, 6, 10]), lam1=0.7, lam2=0.3)
+    assert np.allclose(s["cons"], 1.0, atol=1e-12) and np.allclose(s["spec"], 0.0, atol=1e-12)
+    assert np.allclose(s["cent"], B.sum(axis=1), atol=1e-12)
+    assert np.allclose(s["score"], s["cent"] + 0.7)
+    # scaling every count by 4 (same N_f): Cent and Spec scale by 4, Cons does not move
+    Cr = rng.integers(0, 7, size=(3, 6, 6)); Cr = Cr + Cr.transpose(0, 2, 1)
+    for f in range(3):
+        np.fill_diagonal(Cr[f], 0)
+    a = ref.gesr_scores(Cr, np.array([5, 7, 9]), 0.0, 0.0)
+    b = ref.gesr_scores(Cr * 4, np.array([5, 7, 9]), 0.0, 0.0)
+    assert np.allclose(b["cent"], 4 * a["cent"]) and np.allclose(b["spec"], 4 * a["spec"])
+    assert np.allclose(b["cons"], a["cons"])
+    # an expert that is never routed: all three terms are 0
+    Cz = Cr.copy(); Cz[:, 2, :] = 0; Cz[:, :, 2] = 0
+    z = ref.gesr_scores(Cz, np.array([5, 7, 9]), 1.0, 1.0)
+    assert z["cent"][2] == 0.0 and z["cons"][2] == 0.0 and z["spec"][2] == 0.0
+    # Cauchy-Schwarz / triangle bounds that any correct implementation satisfies
+    assert (a["cons"] <= 1.0 + 1e-12).all() and (a["cons"] >= 0.0).all() and (a["spec"] >= 0.0).all()
+
+
+def test_gesr_replica_table_reduces_to_centrality_at_lambda_zero():
+    rng = np.random.default_rng(8)
+    E, F, P, cap = 12, 3, 4, 3
+    Cr = rng.integers(0, 9, size=(F, E, E)); Cr = Cr + Cr.transpose(0, 2, 1)
+    for f in range(F):
+        np.fill_diagonal(Cr[f], 0)
+    ntok = np.array([11, 13, 17])
+    Abar = sum(Cr[f] / ntok[f] for f in range(F)) / F
+    primary = np.arange(E) // cap
+    aff = ref.affinity(Abar, primary, P)
+    s = ref.gesr_scores(Cr, ntok, 0.0, 0.0)
+    assert np.allclose(s["score"], Abar.sum(axis=1))
+    got = ref.gesr_replica_table(s["score"], aff, primary, n_rep=4, r=2)
+    assert (got == ref.replica_table(Abar, aff, primary, n_rep=4, r=2)).all()
+    # structure of Eq. 12: exactly n_rep rows filled, never the primary, no duplicate partition
+    filled = [e for e in range(E) if got[e, 0] >= 0]
+    assert len(filled) == 4
+    for e in filled:
+        assert primary[e] not in got[e] and len(set(got[e])) == 2
+    # a large specificity penalty removes the most family-specific expert from the generic set
+    spec_top = int(np.argmax(s["spec"]))
+    pen = ref.gesr_scores(Cr, ntok, 0.0, 1e6)
+    rep_pen = ref.gesr_replica_table(pen["score"], aff, primary, n_rep=4, r=2)
+    assert rep_pen[spec_top, 0] == -1
