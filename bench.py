@@ -292,9 +292,10 @@ def main():
     bi0, bf0, _, _ = sets[0]
     co = tacg.tacg_coact_accumulate(ctx, bi0, bf0, E, F, D=D, Cm=Cm, ntok=ntok, flags=tacg.TACG_ZERO_FIRST | path_flag)
     primary_np, swaps = placement.local_search(ctx, D, Cm, ntok, P, cfg.capacity)
-    replicas_np = placement.replica_table(ctx, D, Cm, ntok, P, cfg.capacity, primary_np, cfg.n_rep, cfg.r) if cfg.r else None
     primary = torch.from_numpy(primary_np).to(dev)
-    replicas = None if replicas_np is None else torch.from_numpy(replicas_np).to(dev)
+    # GESR offline step on the device (Eq. 11 with the canonical lambda1 = lambda2 = 0, Eq. 12)
+    replicas = tacg.gesr_build_replicas(ctx, D, Cm, ntok, P, cfg.capacity, primary, cfg.n_rep, cfg.r)[0] if cfg.r else None
+    replicas_np = None if replicas is None else replicas.cpu().numpy()
     r = cfg.r if replicas is not None else 0
 
     def step(bi, bf, ei, ef):

@@ -146,6 +146,28 @@ int gesr_select(tacg_ctx* ctx,
                 int8_t* serve,          /* dev [L,N,k] out */
                 uint32_t flags);        /* 0 or TACG_VALIDATE */
 
+/* SURVEY.md 8(f) f2 (adjacent to the hot path) -- GESR offline step on the device: the generic-expert
+ * score of Eq. 11 and the replica table of Eq. 12:
+ *   A^f = C^f/max(1,ntok[f]);  Abar = mean_f A^f;  Cent[e] = sum_e' Abar[e,e'];
+ *   Cons[e] = mean_f cos(A^f[e,:], Abar[e,:])  (0 when either vector is zero);
+ *   Spec[e] = max_f ||A^f[e,:] - Abar[e,:]||_2;   score = Cent + lambda1*Cons - lambda2*Spec;
+ *   per layer the n_rep experts of largest score (ties -> lower id) receive the r non-primary
+ *   partitions of largest affinity aff[e,m] (aff as in tacg_affinity_swapgain with the same
+ *   alpha, tau, eps and primary; ties -> lower id); replicas = -1 for every other expert and for
+ *   slots beyond the P-1 other partitions.
+ * fp64 on device; terms (optional) is stored as fp32.  Errors as tacg_affinity_swapgain, plus
+ * TACG_ERR_SHAPE for n_rep < 0, r < 1 or r > 8. */
+int gesr_build_replicas(tacg_ctx* ctx,
+                        const uint32_t* D,     /* dev [L,F,E] */
+                        const uint32_t* C,     /* dev [L,F,E,E] */
+                        const uint64_t* ntok,  /* dev [F] */
+                        int L, int E, int F, int P, int capacity,
+                        const int8_t* primary, /* dev [L,E] */
+                        float alpha, float tau, float eps,
+                        float lambda1, float lambda2, int n_rep, int r,
+                        int8_t* replicas,      /* dev [L,E,r] out */
+                        float* terms);         /* dev [L,E,4] out or NULL: (score, Cent, Cons, Spec) */
+
 /* S8..S12 -- score a placement over a held-out trace (Eq. 13-15,
  * Comm per PAPER.md:363, Jain/MaxVio Eq. 17-18).  Tokens are processed
  * in micro-batches of `microbatch` consecutive tokens; every token of a micro-batch sees

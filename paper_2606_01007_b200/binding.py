@@ -26,7 +26,7 @@ TACG_PROF_COACT, TACG_PROF_AFFINITY, TACG_PROF_EVAL = 0, 1, 2
 EXPORTS = (
     "tacg_create", "tacg_destroy", "tacg_strerror", "tacg_last_detail", "tacg_last_path",
     "tacg_launch_count", "tacg_version", "tacg_profile_enable", "tacg_profile_read", "tacg_coact_accumulate", "tacg_affinity_swapgain",
-    "gesr_select", "tacg_eval_placement",
+    "gesr_select", "tacg_eval_placement", "gesr_build_replicas",
 )
 
 _lib = None
@@ -69,6 +69,8 @@ def lib():
         L.tacg_affinity_swapgain.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, f32, f32, f32,
                                              vp, vp, vp, vp]
         L.gesr_select.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp, vp, i32, vp, f32, i64, vp, u32]
+        L.gesr_build_replicas.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, f32, f32, f32, f32, f32,
+                                          i32, i32, vp, vp]
         L.tacg_eval_placement.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, i32, vp, vp, i32, f32, f64,
                                           i64, i64, vp, vp, vp, vp, vp, vp, vp, vp, u32]
         for name in EXPORTS:
@@ -164,6 +166,14 @@ class Context:
             float(alpha), float(tau), float(eps), _ptr(pref, torch.float32, "pref"),
             _ptr(W, torch.float32, "W"), _ptr(aff, torch.float32, "aff"), _ptr(gain, torch.float32, "gain"))
 
+    def gesr_build_replicas(self, D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps, lambda1, lambda2,
+                            n_rep, r, replicas, terms) -> int:
+        return lib().gesr_build_replicas(
+            self._h, _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"), _ptr(ntok, torch.int64, "ntok"),
+            int(L), int(E), int(F), int(P), int(capacity), _ptr(primary, torch.int8, "primary"),
+            float(alpha), float(tau), float(eps), float(lambda1), float(lambda2), int(n_rep), int(r),
+            _ptr(replicas, torch.int8, "replicas"), _ptr(terms, torch.float32, "terms"))
+
     def gesr_select(self, indices, N, k, L, E, P, primary, replicas, r, load_snapshot, theta,
                     token_offset, serve, flags=0) -> int:
         return lib().gesr_select(
@@ -224,6 +234,18 @@ def tacg_affinity_swapgain(ctx: Context, D, Cm, ntok, P: int, capacity: int, pri
                                          out["pref"], out["W"], out["aff"], out["gain"]),
               "tacg_affinity_swapgain")
     return out
+
+
+def gesr_build_replicas(ctx: Context, D, Cm, ntok, P: int, capacity: int, primary, n_rep: int, r: int,
+                        lambda1: float = 0.0, lambda2: float = 0.0, alpha=0.25, tau=1.0, eps=1e-6):
+    """Eq. 11 scores and the Eq. 12 replica table on the device: returns (replicas int8[L,E,r],
+    terms float32[L,E,4] = (score, Cent, Cons, Spec))."""
+    L, F, E = D.shape
+    replicas = torch.empty((L, E, r), dtype=torch.int8, device=D.device)
+    terms = torch.empty((L, E, 4), dtype=torch.float32, device=D.device)
+    ctx.check(ctx.gesr_build_replicas(D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps, lambda1, lambda2,
+                                      n_rep, r, replicas, terms), "gesr_build_replicas")
+    return replicas, terms
 
 
 def gesr_select(ctx: Context, indices, E: int, P: int, primary, replicas, load_snapshot, theta: float,

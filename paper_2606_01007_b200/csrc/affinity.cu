@@ -23,6 +23,7 @@ struct AffScratch {
     double* amax;                // [L]
     double* pref64;              // [L,E,F]
     double* aff64;               // [L,E,P]
+    double* score64;             // [L,E] GESR score (Eq. 11)
 };
 
 __device__ __forceinline__ double warp_sum(double v) {
@@ -255,17 +256,153 @@ gain_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// GESR offline step: Eq. 11 scores and the Eq. 12 replica table.
+// One warp per (layer, expert): the F family profiles A^f[e,:] and their mean are walked once and
+// every sum is a warp reduction in fp64.  Readings Q29-Q31: cosine with a zero vector
+// is 0, "deviation" is the Euclidean norm, ties go to the lower id.
+__global__ void __launch_bounds__(kRowThreads)
+gesr_score_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, double lam1,
+                  double lam2, AffScratch s, float* __restrict__ terms_out) {
+    const int l = blockIdx.y;
+    const int e = blockIdx.x * kRowsPerCta + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (e >= E) return;
+    double inv[8];
+    for (int f = 0; f < F; ++f) inv[f] = 1.0 / (double)max(1ull, ntok[f]);
+    const unsigned* Cl = C + (size_t)l * F * E * E;
+    double cent = 0.0, nm2 = 0.0, dot[8], n2[8], dev2[8];
+#pragma unroll
+    for (int f = 0; f < 8; ++f) { dot[f] = 0.0; n2[f] = 0.0; dev2[f] = 0.0; }
+    const double invF = 1.0 / (double)F;
+    for (int j = lane; j < E; j += 32) {
+        double a[8], mean = 0.0;
+#pragma unroll
+        for (int f = 0; f < 8; ++f) {
+            a[f] = f < F ? (double)__ldg(&Cl[((size_t)f * E + e) * E + j]) * inv[f] : 0.0;
+            mean += a[f];
+        }
+        mean *= invF;
+        cent += mean;
+        nm2 += mean * mean;
+#pragma unroll
+        for (int f = 0; f < 8; ++f) {
+            if (f < F) {
+                dot[f] += a[f] * mean;
+                n2[f] += a[f] * a[f];
+                const double d = a[f] - mean;
+                dev2[f] += d * d;
+            }
+        }
+    }
+    cent = warp_sum(cent);
+    nm2 = warp_sum(nm2);
+    double cons = 0.0, spec = 0.0;
+#pragma unroll
+    for (int f = 0; f < 8; ++f) {
+        if (f < F) {
+            const double dt = warp_sum(dot[f]), nn = warp_sum(n2[f]), dv = warp_sum(dev2[f]);
+            if (nn > 0.0 && nm2 > 0.0) cons += dt / (sqrt(nn) * sqrt(nm2));
+            spec = fmax(spec, sqrt(dv));
+        }
+    }
+    cons *= invF;
+    if (lane == 0) {
+        const double score = cent + lam1 * cons - lam2 * spec;
+        s.score64[(size_t)l * E + e] = score;
+        if (terms_out) {
+            float* o = terms_out + ((size_t)l * E + e) * 4;
+            o[0] = (float)score; o[1] = (float)cent; o[2] = (float)cons; o[3] = (float)spec;
+        }
+    }
+}
+
+// One CTA per layer: the n_rep experts with the largest score (ties -> lower id), each with the r
+// non-primary partitions of largest affinity (ties -> lower id); -1 everywhere else.
+__global__ void __launch_bounds__(256)
+gesr_pick_kernel(int E, int P, int n_rep, int r, const int8_t* __restrict__ primary, AffScratch s,
+                 signed char* __restrict__ replicas) {
+    __shared__ unsigned char taken[512];
+    __shared__ double wbest[8];
+    __shared__ int wbest_e[8];
+    __shared__ int chosen_s;
+    const int l = blockIdx.x;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    signed char* rep = replicas + (size_t)l * E * r;
+    for (int i = threadIdx.x; i < E * r; i += blockDim.x) rep[i] = -1;
+    for (int e = threadIdx.x; e < E; e += blockDim.x) taken[e] = 0;
+    __syncthreads();
+    const double* sc = s.score64 + (size_t)l * E;
+    const int rounds = min(n_rep, E);
+    for (int it = 0; it < rounds; ++it) {
+        double best = 0.0;
+        int be = -1;
+        for (int e = threadIdx.x; e < E; e += blockDim.x) {
+            if (taken[e]) continue;
+            const double v = sc[e];
+            if (be < 0 || v > best) { best = v; be = e; }            // ascending e: the first maximum is the lowest id
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double ov = __shfl_xor_sync(0xffffffffu, best, o);
+            const int oe = __shfl_xor_sync(0xffffffffu, be, o);
+            if (oe >= 0 && (be < 0 || ov > best || (ov == best && oe < be))) { best = ov; be = oe; }
+        }
+        if (lane == 0) { wbest[warp] = best; wbest_e[warp] = be; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double b = 0.0;
+            int e = -1;
+            for (int w = 0; w < 8; ++w) {
+                const int oe = wbest_e[w];
+                if (oe >= 0 && (e < 0 || wbest[w] > b || (wbest[w] == b && oe < e))) { b = wbest[w]; e = oe; }
+            }
+            chosen_s = e;
+            if (e >= 0) taken[e] = 1;
+        }
+        __syncthreads();
+        const int e = chosen_s;
+        if (e >= 0 && warp == 0) {
+            // secondaries of expert e: r rounds of arg max over the non-primary partitions (warp 0)
+            const int pm = primary[(size_t)l * E + e] & 63;
+            const double* af = s.aff64 + ((size_t)l * E + e) * P;
+            unsigned long long used = 1ull << pm;
+            for (int a = 0; a < r; ++a) {
+                double bv = 0.0;
+                int bm = -1;
+                for (int m = lane; m < P; m += 32) {
+                    if ((used >> m) & 1ull) continue;
+                    const double v = af[m];
+                    if (bm < 0 || v > bv) { bv = v; bm = m; }
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    const double ov = __shfl_xor_sync(0xffffffffu, bv, o);
+                    const int om = __shfl_xor_sync(0xffffffffu, bm, o);
+                    if (om >= 0 && (bm < 0 || ov > bv || (ov == bv && om < bm))) { bv = ov; bm = om; }
+                }
+                if (bm < 0) break;                                   // fewer than r other partitions
+                used |= 1ull << bm;
+                if (lane == 0) rep[(size_t)e * r + a] = (signed char)bm;
+            }
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace
 
 int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L, int E,
                          int F, int P, const int8_t* primary, double alpha, double tau, double eps, float* pref,
-                         float* W, float* aff, float* gain) {
+                         float* W, float* aff, float* gain, const tacg_gesr_build* gesr) {
     size_t off = 0;
     const size_t o_rowsum = off; off += tacg_align_up(sizeof(unsigned long long) * (size_t)L * F * E, 256);
     const size_t o_rowmax = off; off += tacg_align_up(sizeof(double) * (size_t)L * E, 256);
     const size_t o_amax = off;   off += tacg_align_up(sizeof(double) * (size_t)L, 256);
     const size_t o_pref = off;   off += tacg_align_up(sizeof(double) * (size_t)L * E * F, 256);
     const size_t o_aff = off;    off += tacg_align_up(sizeof(double) * (size_t)L * E * P, 256);
+    const size_t o_score = off;  off += tacg_align_up(sizeof(double) * (size_t)L * E, 256);
     char* base = static_cast<char*>(tacg_scratch(ctx, off));
     if (!base) return TACG_ERR_CUDA;
     AffScratch s;
@@ -274,6 +411,7 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     s.amax = reinterpret_cast<double*>(base + o_amax);
     s.pref64 = reinterpret_cast<double*>(base + o_pref);
     s.aff64 = reinterpret_cast<double*>(base + o_aff);
+    s.score64 = reinterpret_cast<double*>(base + o_score);
     const unsigned long long* nt = reinterpret_cast<const unsigned long long*>(ntok);
     const dim3 rows((E + kRowsPerCta - 1) / kRowsPerCta, L);
     tacg_prof_scope prof(ctx, TACG_PROF_AFFINITY);
@@ -283,13 +421,20 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(pref_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
     pref_kernel<<<L, 256, psm, ctx->stream>>>(D, nt, E, F, tau, eps, s, pref);
     TACG_LAUNCH_CHECK(ctx);
-    if (W || aff || gain) {
+    if (W || aff || gain || gesr) {
         const size_t gsm = sizeof(double) * (size_t)kRowsPerCta * E + sizeof(short) * (size_t)E;
         graph_aff_kernel<<<rows, kRowThreads, gsm, ctx->stream>>>(C, nt, E, F, P, primary, alpha, s, W, aff);
         TACG_LAUNCH_CHECK(ctx);
     }
     if (gain) {
         gain_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, P, primary, alpha, s, gain);
+        TACG_LAUNCH_CHECK(ctx);
+    }
+    if (gesr) {
+        gesr_score_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, gesr->lambda1, gesr->lambda2, s, gesr->terms);
+        TACG_LAUNCH_CHECK(ctx);
+        gesr_pick_kernel<<<L, 256, 0, ctx->stream>>>(E, P, gesr->n_rep, gesr->r, primary, s,
+                                                     reinterpret_cast<signed char*>(gesr->replicas));
         TACG_LAUNCH_CHECK(ctx);
     }
     return TACG_OK;

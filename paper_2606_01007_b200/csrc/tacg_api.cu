@@ -202,6 +202,24 @@ int tacg_affinity_swapgain(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, 
                                 (double)eps, pref, W, aff, gain);
 }
 
+int gesr_build_replicas(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L, int E, int F,
+                        int P, int capacity, const int8_t* primary, float alpha, float tau, float eps, float lambda1,
+                        float lambda2, int n_rep, int r, int8_t* replicas, float* terms) {
+    if (!ctx) return TACG_ERR_NULL;
+    if (L < 1 || E < 1 || E > 512 || F < 1 || F > 8) return fail(ctx, TACG_ERR_SHAPE, "gesr_build: L/E/F out of range");
+    if (!D || !C || !ntok || !primary || !replicas) return fail(ctx, TACG_ERR_NULL, "gesr_build: NULL pointer");
+    if (P < 1 || P > 64 || capacity < 1 || (int64_t)E > (int64_t)P * capacity)
+        return fail(ctx, TACG_ERR_SHAPE, "gesr_build: P out of range or E > P*capacity");
+    if (n_rep < 0 || r < 1 || r > 8) return fail(ctx, TACG_ERR_SHAPE, "gesr_build: n_rep < 0 or r outside [1,8]");
+    if (!(tau > 0.0f) || !(eps >= 0.0f)) return fail(ctx, TACG_ERR_SHAPE, "gesr_build: tau must be > 0 and eps >= 0");
+    TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    tacg_gesr_build g;
+    g.lambda1 = (double)lambda1; g.lambda2 = (double)lambda2; g.n_rep = n_rep; g.r = r;
+    g.replicas = replicas; g.terms = terms;
+    return tacg_launch_affinity(ctx, D, C, ntok, L, E, F, P, primary, (double)alpha, (double)tau, (double)eps, nullptr,
+                                nullptr, nullptr, nullptr, &g);
+}
+
 int gesr_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P, const int8_t* primary,
                 const int8_t* replicas, int r, const double* load_snapshot, float theta, int64_t token_offset,
                 int8_t* serve, uint32_t flags) {

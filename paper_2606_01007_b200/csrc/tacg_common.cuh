@@ -79,9 +79,16 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
 bool tacg_coact_mma_supported(int k, int E, int F);
 int tacg_launch_coact_mma(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k,
                           int L, int E, int F, uint32_t* D, uint32_t* C, uint64_t* ntok, bool zero_first);
+// Optional GESR offline step run after the affinity kernels (gesr_build_replicas).
+struct tacg_gesr_build {
+    double lambda1, lambda2;
+    int n_rep, r;
+    int8_t* replicas;   // dev [L,E,r] out
+    float* terms;       // dev [L,E,4] out or NULL: (score, Cent, Cons, Spec)
+};
 int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L,
                          int E, int F, int P, const int8_t* primary, double alpha, double tau, double eps,
-                         float* pref, float* W, float* aff, float* gain);
+                         float* pref, float* W, float* aff, float* gain, const tacg_gesr_build* gesr = nullptr);
 int tacg_launch_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P,
                        const int8_t* primary, const int8_t* replicas, int r, const double* snapshot,
                        float theta, int64_t token_offset, int8_t* serve);
