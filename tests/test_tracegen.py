@@ -48,3 +48,29 @@ def test_random_placement_feasible():
         for e in rows:
             v = [x for x in rep[l, e] if x >= 0]
             assert pr[l, e] not in v and len(set(v)) == len(v)
+
+
+def test_skew_workloads_have_the_stated_shares():
+    names = tracegen.skew_workloads(4)
+    assert len(names) == 13
+    N = 40000
+    for w in names:
+        fam = tracegen.gen_family_workload(N, w, 4, seed=5)
+        assert fam.shape == (N,) and fam.dtype == torch.int8 and fam.min() >= 0 and fam.max() < 4
+        assert torch.equal(fam, tracegen.gen_family_workload(N, w, 4, seed=5))
+        h = np.bincount(fam.numpy(), minlength=4) / N
+        kind, *rest = w.split(":")
+        if kind == "balanced":
+            assert np.allclose(h, 0.25, atol=0.01)
+        elif kind == "single":
+            f, s = int(rest[0]), float(rest[1])
+            assert abs(h[f] - s) < 0.01 and np.allclose(np.delete(h, f), (1 - s) / 3, atol=0.01)
+        elif kind == "phase":
+            span = fam.numpy()[: N // 8]
+            dom = 0 if rest[0] == "up" else 3
+            assert abs((span == dom).mean() - 0.8) < 0.02
+        else:
+            f = int(rest[0])
+            lo = int(0.4 * N)
+            assert (fam.numpy()[lo:lo + int(0.15 * N)] == f).all()
+            assert abs(h[f] - (0.15 + 0.85 * 0.25)) < 0.01

@@ -17,6 +17,8 @@ from .generator import (
     TraceParams,
     make_params,
     gen_family,
+    gen_family_workload,
+    skew_workloads,
     gen_indices,
     gen_trace,
     random_placement,
@@ -26,6 +28,6 @@ from .generator import (
 
 __all__ = [
     "TraceConfig", "CONFIGS", "get_config", "scaled", "TraceParams", "make_params",
-    "gen_family", "gen_indices", "gen_trace", "random_placement",
+    "gen_family", "gen_family_workload", "skew_workloads", "gen_indices", "gen_trace", "random_placement",
     "random_replicas", "checksum64",
 ]

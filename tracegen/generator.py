@@ -115,6 +115,58 @@ def gen_family(N: int, mix, seed: int, device="cpu") -> torch.Tensor:
     return out
 
 
+SKEW_SHARES = (0.6, 0.8)
+BURST_SHARE = 0.15
+BURST_FAMILIES = (2, 3)     # "math", "complex_reasoning" in the paper's family order
+
+
+def skew_workloads(F: int = 4):
+    """Names of the 13 online workloads of the paper's skew sweep: one
+    balanced reference, F families x two single-family shares, two phase-shift streams, two
+    bursty streams.  Only the family-label stream changes between them."""
+    names = ["balanced"]
+    names += [f"single:{f}:{s}" for f in range(F) for s in SKEW_SHARES]
+    names += ["phase:up", "phase:down"]
+    names += [f"burst:{f}" for f in BURST_FAMILIES if f < F]
+    return names
+
+
+def gen_family_workload(N: int, workload: str, F: int, seed: int, device="cpu",
+                        phases: int = 8) -> torch.Tensor:
+    """int8[N] family labels of one skew workload (the paper gives the suite in one sentence,
+    PAPER.md:383; the numbers it leaves open are fixed here and listed in DESIGN.md Q32):
+      balanced       i.i.d. uniform over the F families;
+      single:f:s     i.i.d., family f with share s, the others (1-s)/(F-1) each;
+      phase:up|down  the stream is cut into `phases` equal spans; span j is i.i.d. with family
+                     j mod F (up) or F-1 - j mod F (down) at share 0.8;
+      burst:f        the balanced stream with one contiguous span of 15 % of the tokens, starting
+                     at 40 % of the stream, relabelled f.
+    """
+    kind, *rest = workload.split(":")
+    if kind == "balanced":
+        return gen_family(N, (1.0 / F,) * F, seed, device=device)
+    if kind == "single":
+        f, s = int(rest[0]), float(rest[1])
+        mix = [(1.0 - s) / (F - 1)] * F
+        mix[f] = s
+        return gen_family(N, mix, seed, device=device)
+    if kind == "phase":
+        out = torch.empty(N, dtype=torch.int8, device=device)
+        for j in range(phases):
+            lo, hi = j * N // phases, (j + 1) * N // phases
+            f = j % F if rest[0] == "up" else F - 1 - j % F
+            mix = [0.2 / (F - 1)] * F
+            mix[f] = 0.8
+            out[lo:hi] = gen_family(hi - lo, mix, seed * 31 + j, device=device)
+        return out
+    if kind == "burst":
+        out = gen_family(N, (1.0 / F,) * F, seed, device=device)
+        lo = int(0.4 * N)
+        out[lo:lo + int(BURST_SHARE * N)] = int(rest[0])
+        return out
+    raise ValueError(workload)
+
+
 def gen_indices(cfg: TraceConfig, params: TraceParams, family: torch.Tensor, seed: int,
                 eval_trace: bool = False, device="cpu", chunk: int = 1 << 20,
                 out: Optional[torch.Tensor] = None) -> torch.Tensor:
