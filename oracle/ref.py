@@ -15,7 +15,9 @@ Parity pins (tests/test_oracle_pins.py): hand-worked trace of SURVEY.md 8(c)
 enumeration of Eq. 9, swap-gain identity by recomputing the objective,
 closed-form Comm under uniform routing against the paper's printed Baseline
 Comm, Jain/MaxVio closed forms, special cases alpha=0,
-F=1, identical families, theta=inf, rho in {0,1}.  No function here is
+F=1, identical families, theta=inf, rho in {0,1}; for O14 (spectral-then-repair)
+the spectrum of disjoint cliques and of a path, hand-worked repairs, recovery of
+planted communities and brute force on tiny graphs.  No function here is
 "parity unpinned".
 """
 from __future__ import annotations
@@ -457,3 +459,107 @@ def gesr_replica_table(score: Sequence[float], aff: np.ndarray, primary: Sequenc
         for i, m in enumerate(cands[:r]):
             rep[e, i] = m
     return rep
+
+
+# --------------------------------------------------------------------------
+# O14 -- capacity-feasible expert grouping, spectral-then-repair.
+# PAPER.md:117-124.  Stage 1: "symmetrize A-tilde, scale it to [0,1], add a small diagonal jitter
+# ... form the symmetric normalized Laplacian L_sym = I - D^-1/2 A D^-1/2 with degree matrix D,
+# embed experts via its M smallest eigenvectors, and run k-means with k = M".  Stage 2: every
+# overfull group keeps its top-C_m members by intra-group affinity, the rest enter an overflow
+# pool and are inserted greedily by Eq. 10.
+# Readings (Q33-Q37): scale = divide by the largest entry; jitter 1e-6; the degree
+# includes the jitter; rows of the embedding are not renormalised (the text does not say so);
+# k-means is Lloyd's iteration from a deterministic farthest-point start (first centre = the
+# expert of largest degree, then the expert farthest from the chosen centres), an empty cluster
+# keeps its centre, ties go to the lower id everywhere; C_m = capacity is an upper bound when
+# E < M*capacity; the pool is served group by group, strongest evicted member first.  After the
+# greedy pass every expert sits in a group of size <= C_m (a non-full group always exists while
+# sum C_m >= E), so the donor-receiver loop of PAPER.md:124 has nothing left to move: it is
+# stated here as a check, not as code.
+# --------------------------------------------------------------------------
+def scaled_affinity(W: np.ndarray) -> np.ndarray:
+    """(W + W^T)/2 divided by its largest entry (all zeros stay all zeros).  float64[E,E]."""
+    E = W.shape[0]
+    S = [[(float(W[i][j]) + float(W[j][i])) * 0.5 for j in range(E)] for i in range(E)]
+    top = max(max(row) for row in S)
+    if top > 0.0:
+        S = [[v / top for v in row] for row in S]
+    return np.array(S, dtype=np.float64)
+
+
+def spectral_embedding(W: np.ndarray, M: int, jitter: float = 1e-6):
+    """Returns (X float64[E,M], eigenvalues float64[M]): the eigenvectors of the M smallest
+    eigenvalues of L_sym of the scaled, jittered affinity (columns in increasing eigenvalue
+    order; an eigenvector's sign, and the basis inside a repeated eigenvalue, are not unique)."""
+    S = scaled_affinity(W)
+    E = S.shape[0]
+    A = S + jitter * np.eye(E)
+    deg = A.sum(axis=1)
+    inv = 1.0 / np.sqrt(deg)
+    Lsym = np.eye(E) - inv[:, None] * A * inv[None, :]
+    vals, vecs = np.linalg.eigh(Lsym)            # library step: symmetric eigendecomposition, ascending
+    return vecs[:, :M].copy(), vals[:M].copy()
+
+
+def kmeans_labels(X: np.ndarray, k: int, first: int, iters: int = 100) -> List[int]:
+    """Lloyd's k-means on the rows of X from a farthest-point start whose first centre is row `first`."""
+    E = X.shape[0]
+
+    def d2(a, b):
+        return float(sum((float(a[t]) - float(b[t])) ** 2 for t in range(len(a))))
+
+    centres = [list(map(float, X[first]))]
+    mind = [d2(X[e], centres[0]) for e in range(E)]
+    while len(centres) < k:
+        nxt = max(range(E), key=lambda e: (mind[e], -e))
+        centres.append(list(map(float, X[nxt])))
+        for e in range(E):
+            mind[e] = min(mind[e], d2(X[e], centres[-1]))
+    labels = [-1] * E
+    for _ in range(iters):
+        new = [min(range(k), key=lambda c: (d2(X[e], centres[c]), c)) for e in range(E)]
+        if new == labels:
+            break
+        labels = new
+        for c in range(k):
+            members = [e for e in range(E) if labels[e] == c]
+            if members:
+                centres[c] = [sum(float(X[e][t]) for e in members) / len(members) for t in range(X.shape[1])]
+    return labels
+
+
+def capacity_repair(S: np.ndarray, labels0: Sequence[int], P: int, capacity: int) -> List[int]:
+    """Stage 2 on the scaled affinity S (self-affinity never counted)."""
+    E = S.shape[0]
+    groups = [[e for e in range(E) if int(labels0[e]) == m] for m in range(P)]
+    pool: List[int] = []
+    for m in range(P):
+        if len(groups[m]) > capacity:
+            intra = {e: sum(float(S[e][e2]) for e2 in groups[m] if e2 != e) for e in groups[m]}
+            ranked = sorted(groups[m], key=lambda e: (-intra[e], e))
+            groups[m] = sorted(ranked[:capacity])
+            pool.extend(ranked[capacity:])
+    for e in pool:
+        open_groups = [m for m in range(P) if len(groups[m]) < capacity]
+        inc = {m: sum(float(S[e][e2]) for e2 in groups[m]) for m in open_groups}       # Eq. 10
+        best = max(open_groups, key=lambda m: (inc[m], -m))
+        groups[best] = sorted(groups[best] + [e])
+    assert all(len(g) <= capacity for g in groups)        # nothing left for the donor-receiver loop
+    out = [-1] * E
+    for m in range(P):
+        for e in groups[m]:
+            out[e] = m
+    return out
+
+
+def spectral_place(W: np.ndarray, P: int, capacity: int, jitter: float = 1e-6, iters: int = 100):
+    """Stage 1 + Stage 2 for one layer.  Returns (primary list[E], labels0 list[E], X float64[E,P])."""
+    E = W.shape[0]
+    assert E <= P * capacity
+    X, _ = spectral_embedding(W, P, jitter)
+    S = scaled_affinity(W)
+    deg = [sum(float(S[e][e2]) for e2 in range(E)) + jitter for e in range(E)]
+    first = max(range(E), key=lambda e: (deg[e], -e))
+    labels0 = kmeans_labels(X, P, first, iters)
+    return capacity_repair(S, labels0, P, capacity), labels0, X

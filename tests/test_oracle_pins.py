@@ -526,3 +526,99 @@ def test_gesr_replica_table_reduces_to_centrality_at_lambda_zero():
     pen = ref.gesr_scores(Cr, ntok, 0.0, 1e6)
     rep_pen = ref.gesr_replica_table(pen["score"], aff, primary, n_rep=4, r=2)
     assert rep_pen[spec_top, 0] == -1
+
+
+# ---------------------------------------------------------------------------------------------
+# O14 -- spectral-then-repair grouping
+# ---------------------------------------------------------------------------------------------
+def _sym(E, entries):
+    S = np.zeros((E, E))
+    for (i, j), v in entries.items():
+        S[i, j] = S[j, i] = v
+    return S
+
+
+def test_spectral_embedding_closed_forms():
+    # scale: symmetrise then divide by the largest entry
+    assert (ref.scaled_affinity(np.array([[0.0, 2.0], [4.0, 0.0]])) == np.array([[0.0, 1.0], [1.0, 0.0]])).all()
+    assert (ref.scaled_affinity(np.zeros((3, 3))) == 0).all()
+    # two disjoint cliques K3 + K4, no jitter: L_sym of K_n has eigenvalues 0 and n/(n-1) (n-1 times)
+    W = np.zeros((7, 7))
+    W[:3, :3] = 1.0
+    W[3:, 3:] = 1.0
+    np.fill_diagonal(W, 0.0)
+    X, vals = ref.spectral_embedding(W, 7, jitter=0.0)
+    assert np.allclose(vals, [0, 0, 4 / 3, 4 / 3, 4 / 3, 1.5, 1.5], atol=1e-12)
+    # the null space is spanned by the (degree-weighted) clique indicators: rows equal inside a clique
+    assert np.allclose(X[:3, :2], X[0, :2], atol=1e-10) and np.allclose(X[3:, :2], X[3, :2], atol=1e-10)
+    assert np.linalg.norm(X[0, :2] - X[3, :2]) > 0.1
+    # a path 0-1-2: L_sym eigenvalues 0, 1, 2 (bipartite)
+    _, vals = ref.spectral_embedding(_sym(3, {(0, 1): 1.0, (1, 2): 1.0}), 3, jitter=0.0)
+    assert np.allclose(vals, [0, 1, 2], atol=1e-12)
+
+
+def test_kmeans_separated_points_and_rotation():
+    rng = np.random.default_rng(3)
+    truth = np.array([0, 1, 2] * 5)
+    X = np.stack([truth * 10.0 + 0.1 * rng.standard_normal(15), 0.1 * rng.standard_normal(15)], axis=1)
+    lab = ref.kmeans_labels(X, 3, first=0)
+    assert len(set(lab)) == 3 and all((lab[i] == lab[j]) == (truth[i] == truth[j]) for i in range(15) for j in range(15))
+    assert lab[0] == 0                                       # cluster ids follow the order the centres were chosen
+    th = 0.7
+    Q = np.array([[np.cos(th), -np.sin(th)], [np.sin(th), np.cos(th)]])
+    assert ref.kmeans_labels(X @ Q, 3, first=0) == lab       # distances only: the basis does not matter
+    assert ref.kmeans_labels(-X, 3, first=0) == lab
+    # k = 1 and k = number of points
+    assert ref.kmeans_labels(X, 1, first=4) == [0] * 15
+    assert sorted(ref.kmeans_labels(X[:3], 3, first=1)) == [0, 1, 2]
+
+
+def test_capacity_repair_handworked():
+    # group 0 = {0,1,2,3} over capacity 3: intra sums 1.8, 1.6, 1.7, 0.7 -> expert 3 leaves and can only go to group 1
+    S = _sym(5, {(0, 1): 0.9, (0, 2): 0.8, (0, 3): 0.1, (1, 2): 0.5, (1, 3): 0.2, (2, 3): 0.4, (0, 4): 0.05, (3, 4): 0.6})
+    assert ref.capacity_repair(S, [0, 0, 0, 0, 1], 2, 3) == [0, 0, 0, 1, 1]
+    # capacity 2: intra sums 1.7, 1.5, 1.2, 0.6 -> pool = [2, 3], strongest first.  Expert 2 prefers group 2
+    # (0.7 > 0.1) and fills it; expert 3 would prefer group 2 (0.9) but only group 1 is open.
+    S = _sym(6, {(0, 1): 1.0, (0, 2): 0.5, (0, 3): 0.2, (1, 2): 0.4, (1, 3): 0.1, (2, 3): 0.3,
+                 (2, 4): 0.1, (2, 5): 0.7, (3, 4): 0.2, (3, 5): 0.9})
+    assert ref.capacity_repair(S, [0, 0, 0, 0, 1, 2], 3, 2) == [0, 0, 2, 1, 1, 2]
+    # ties: equal gains -> lower group id; equal intra sums -> lower expert id stays
+    S = _sym(4, {(0, 1): 1.0, (0, 2): 1.0, (1, 2): 1.0})
+    assert ref.capacity_repair(S, [0, 0, 0, 1], 3, 2) == [0, 0, 1, 1]
+    # feasible input is returned unchanged
+    assert ref.capacity_repair(S, [2, 0, 1, 0], 3, 2) == [2, 0, 1, 0]
+
+
+def test_spectral_place_planted_and_close_to_exhaustive():
+    # planted equal-size communities are recovered exactly and are the brute-force optimum of Eq. 9
+    for E, P, cap, seed in ((8, 2, 4, 0), (9, 3, 3, 1), (12, 3, 4, 2)):
+        rng = np.random.default_rng(seed)
+        lab = np.empty(E, dtype=int)
+        lab[rng.permutation(E)] = np.arange(E) // cap
+        W = 0.02 * rng.random((E, E))
+        W = (W + W.T) / 2 + (lab[:, None] == lab[None, :])
+        np.fill_diagonal(W, 0.0)
+        pr, labels0, X = ref.spectral_place(W, P, cap)
+        assert X.shape == (E, P)
+        assert all((pr[i] == pr[j]) == (lab[i] == lab[j]) for i in range(E) for j in range(E))
+        assert pr == labels0                                 # nothing to repair
+        if E <= 9:
+            best, _, _ = ref.brute_force_optimum(W, P, cap)
+            assert abs(ref.objective_half(W, pr) - best) < 1e-12
+    # unstructured graphs: feasible, never above the optimum, and "very close to exhaustive search"
+    ratios = []
+    for seed in range(12):
+        rng = np.random.default_rng(100 + seed)
+        E, P, cap = (8, 2, 4) if seed % 2 else (9, 3, 3)
+        W = rng.random((E, E)) ** 3
+        W = (W + W.T) / 2
+        np.fill_diagonal(W, 0.0)
+        pr, _, _ = ref.spectral_place(W, P, cap)
+        assert np.bincount(pr, minlength=P).max() <= cap and min(pr) >= 0
+        best, _, _ = ref.brute_force_optimum(W, P, cap)
+        ratios.append(ref.objective_half(W, pr) / best)
+    assert max(ratios) <= 1.0 + 1e-12 and min(ratios) > 0.8 and np.mean(ratios) > 0.93
+    # capacity slack (E < P*capacity): capacities are upper bounds
+    W = np.random.default_rng(5).random((10, 10))
+    pr, _, _ = ref.spectral_place(W, 4, 3)
+    assert np.bincount(pr, minlength=4).max() <= 3
