@@ -168,6 +168,31 @@ int gesr_build_replicas(tacg_ctx* ctx,
                         int8_t* replicas,      /* dev [L,E,r] out */
                         float* terms);         /* dev [L,E,4] out or NULL: (score, Cent, Cons, Spec) */
 
+/* SURVEY.md 8(f) f1 (adjacent to the hot path) -- capacity-feasible expert grouping by the
+ * spectral-then-repair procedure of PAPER.md:110-124 (Eq. 9-10), per layer, on the device:
+ *   Stage 1  S = (W + W^T)/2 divided by its largest entry;  A = S + jitter*I;  deg = rowsum A;
+ *            L_sym = I - D^-1/2 A D^-1/2;  X = eigenvectors of its P smallest eigenvalues (rows not
+ *            renormalised);  Lloyd's k-means with k = P on the rows of X from a farthest-point start
+ *            (first centre = expert of largest degree), at most kmeans_iters rounds, an empty cluster
+ *            keeps its centre, ties -> lower id.
+ *   Stage 2  every group over `capacity` keeps its `capacity` members of largest intra-group
+ *            affinity sum_{e' in group, e' != e} S[e,e'] (ties -> lower id); the others, group by
+ *            group, strongest first, go to the non-full group of largest sum_{e' in group} S[e,e']
+ *            (Eq. 10; ties -> lower group).
+ * W must be non-negative.  labels_in (optional) replaces Stage 1: the repair alone, which is then
+ * exact (sums in increasing expert id, fp64).  labels0 (optional) receives the Stage-1 labels and
+ * embed (optional) the embedding; an eigenvector's sign and the basis inside a repeated eigenvalue
+ * are not unique, the labels do not depend on them.  TACG_ERR_SHAPE for E > 512, P > min(64, E),
+ * E > P*capacity, jitter < 0 or kmeans_iters < 1. */
+int tacg_spectral_place(tacg_ctx* ctx,
+                        const float* W,          /* dev [L,E,E] graph of tacg_affinity_swapgain */
+                        int L, int E, int P, int capacity,
+                        double jitter, int kmeans_iters,
+                        const int8_t* labels_in, /* dev [L,E] in [0,P), or NULL */
+                        int8_t* primary,         /* dev [L,E] out */
+                        int8_t* labels0,         /* dev [L,E] out or NULL */
+                        double* embed);          /* dev [L,E,P] out or NULL */
+
 /* S8..S12 -- score a placement over a held-out trace (Eq. 13-15,
  * Comm per PAPER.md:363, Jain/MaxVio Eq. 17-18).  Tokens are processed
  * in micro-batches of `microbatch` consecutive tokens; every token of a micro-batch sees

@@ -26,7 +26,7 @@ TACG_PROF_COACT, TACG_PROF_AFFINITY, TACG_PROF_EVAL = 0, 1, 2
 EXPORTS = (
     "tacg_create", "tacg_destroy", "tacg_strerror", "tacg_last_detail", "tacg_last_path",
     "tacg_launch_count", "tacg_version", "tacg_profile_enable", "tacg_profile_read", "tacg_coact_accumulate", "tacg_affinity_swapgain",
-    "gesr_select", "tacg_eval_placement", "gesr_build_replicas",
+    "gesr_select", "tacg_eval_placement", "gesr_build_replicas", "tacg_spectral_place",
 )
 
 _lib = None
@@ -71,6 +71,7 @@ def lib():
         L.gesr_select.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp, vp, i32, vp, f32, i64, vp, u32]
         L.gesr_build_replicas.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, f32, f32, f32, f32, f32,
                                           i32, i32, vp, vp]
+        L.tacg_spectral_place.argtypes = [vp, vp, i32, i32, i32, i32, f64, i32, vp, vp, vp, vp]
         L.tacg_eval_placement.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, i32, vp, vp, i32, f32, f64,
                                           i64, i64, vp, vp, vp, vp, vp, vp, vp, vp, u32]
         for name in EXPORTS:
@@ -174,6 +175,12 @@ class Context:
             float(alpha), float(tau), float(eps), float(lambda1), float(lambda2), int(n_rep), int(r),
             _ptr(replicas, torch.int8, "replicas"), _ptr(terms, torch.float32, "terms"))
 
+    def tacg_spectral_place(self, W, L, E, P, capacity, jitter, kmeans_iters, labels_in, primary, labels0, embed) -> int:
+        return lib().tacg_spectral_place(
+            self._h, _ptr(W, torch.float32, "W"), int(L), int(E), int(P), int(capacity), float(jitter),
+            int(kmeans_iters), _ptr(labels_in, torch.int8, "labels_in"), _ptr(primary, torch.int8, "primary"),
+            _ptr(labels0, torch.int8, "labels0"), _ptr(embed, torch.float64, "embed"))
+
     def gesr_select(self, indices, N, k, L, E, P, primary, replicas, r, load_snapshot, theta,
                     token_offset, serve, flags=0) -> int:
         return lib().gesr_select(
@@ -246,6 +253,19 @@ def gesr_build_replicas(ctx: Context, D, Cm, ntok, P: int, capacity: int, primar
     ctx.check(ctx.gesr_build_replicas(D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps, lambda1, lambda2,
                                       n_rep, r, replicas, terms), "gesr_build_replicas")
     return replicas, terms
+
+
+def tacg_spectral_place(ctx: Context, W, P: int, capacity: int, jitter: float = 1e-6, kmeans_iters: int = 100,
+                        labels_in=None, want_embed: bool = False):
+    """Spectral-then-repair primary placement of every layer of W float32[L,E,E]:
+    returns dict(primary int8[L,E], labels0 int8[L,E], embed float64[L,E,P] or None)."""
+    L, E, _ = W.shape
+    primary = torch.empty((L, E), dtype=torch.int8, device=W.device)
+    labels0 = torch.empty((L, E), dtype=torch.int8, device=W.device)
+    embed = torch.empty((L, E, P), dtype=torch.float64, device=W.device) if want_embed else None
+    ctx.check(ctx.tacg_spectral_place(W, L, E, P, capacity, jitter, kmeans_iters, labels_in, primary, labels0, embed),
+              "tacg_spectral_place")
+    return dict(primary=primary, labels0=labels0, embed=embed)
 
 
 def gesr_select(ctx: Context, indices, E: int, P: int, primary, replicas, load_snapshot, theta: float,

@@ -220,6 +220,18 @@ int gesr_build_replicas(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, con
                                 nullptr, nullptr, nullptr, &g);
 }
 
+int tacg_spectral_place(tacg_ctx* ctx, const float* W, int L, int E, int P, int capacity, double jitter,
+                        int kmeans_iters, const int8_t* labels_in, int8_t* primary, int8_t* labels0, double* embed) {
+    if (!ctx) return TACG_ERR_NULL;
+    if (L < 1 || E < 1 || E > 512) return fail(ctx, TACG_ERR_SHAPE, "spectral_place: L/E out of range");
+    if (!W || !primary) return fail(ctx, TACG_ERR_NULL, "spectral_place: NULL pointer");
+    if (P < 1 || P > 64 || P > E || capacity < 1 || (int64_t)E > (int64_t)P * capacity)
+        return fail(ctx, TACG_ERR_SHAPE, "spectral_place: P outside [1, min(64,E)] or E > P*capacity");
+    if (!(jitter >= 0.0) || kmeans_iters < 1) return fail(ctx, TACG_ERR_SHAPE, "spectral_place: jitter < 0 or kmeans_iters < 1");
+    TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return tacg_launch_spectral(ctx, W, L, E, P, capacity, jitter, kmeans_iters, labels_in, primary, labels0, embed);
+}
+
 int gesr_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P, const int8_t* primary,
                 const int8_t* replicas, int r, const double* load_snapshot, float theta, int64_t token_offset,
                 int8_t* serve, uint32_t flags) {
