@@ -1,8 +1,9 @@
 """Host-side placement driver (harness) -- consumes the library's outputs.
 
 These are the consumers of the hot path, not part of it: a capacity-preserving best-swap
-local search driven by the GPU swap gains (standing in for the repair loop of
-PAPER.md:119-124; the paper's spectral stage is NEXT f1), and the GESR replica table with
+local search driven by the GPU swap gains (the "only if the move improves" test of
+PAPER.md:124 applied to every pair), the whole offline stage of the method chained on the device
+(`tacg_gesr_placement`: counts -> graph -> spectral-then-repair -> replicas), and the GESR replica table with
 the canonical lambda1 = lambda2 = 0 (centrality only).  All
 E x E arithmetic stays in tacg_affinity_swapgain; the host only takes argmaxes.
 """
@@ -83,3 +84,23 @@ def replica_table(ctx: "_b.Context", D, Cm, ntok, P: int, capacity: int, primary
             for i, m in enumerate(cands[:r]):
                 rep[l, e, i] = m
     return rep
+
+
+def tacg_gesr_placement(ctx: "_b.Context", D, Cm, ntok, P: int, capacity: int, n_rep: int, r: int,
+                        alpha: float = 0.25, tau: float = 1.0, eps: float = 1e-6, lambda1: float = 0.0,
+                        lambda2: float = 0.0, refine: bool = False):
+    """The offline stage of the method, every step on the device: the task-modulated
+    graph W (Eq. 7-8), the spectral-then-repair primary placement (Eq. 9-10), optionally refined by the
+    swap-gain local search, and the GESR replica table (Eq. 11-12).  Returns (primary int8[L,E] tensor,
+    replicas int8[L,E,r] tensor or None)."""
+    W = _b.tacg_affinity_swapgain(ctx, D, Cm, ntok, P, capacity, None, alpha=alpha, tau=tau, eps=eps, want=("W",))["W"]
+    primary = _b.tacg_spectral_place(ctx, W, P, capacity)["primary"]
+    if refine:
+        refined, _ = local_search(ctx, D, Cm, ntok, P, capacity, alpha=alpha, tau=tau, eps=eps,
+                                  primary0=primary.cpu().numpy())
+        primary = torch.from_numpy(refined).to(D.device)
+    replicas = None
+    if r > 0 and n_rep > 0:
+        replicas, _ = _b.gesr_build_replicas(ctx, D, Cm, ntok, P, capacity, primary, n_rep, r, lambda1=lambda1,
+                                             lambda2=lambda2, alpha=alpha, tau=tau, eps=eps)
+    return primary, replicas
