@@ -563,3 +563,46 @@ def spectral_place(W: np.ndarray, P: int, capacity: int, jitter: float = 1e-6, i
     first = max(range(E), key=lambda e: (deg[e], -e))
     labels0 = kmeans_labels(X, P, first, iters)
     return capacity_repair(S, labels0, P, capacity), labels0, X
+
+
+# --------------------------------------------------------------------------
+# O15 -- motivation diagnostics.  PAPER.md:469: "The activation Frobenius
+# distance between two task families is the Frobenius norm ||P_i - P_j||_F of the difference
+# between their expert-activation distributions ... The top-64 pair Jaccard overlap measures the
+# Jaccard similarity between the sets of top-64 most frequently coactivated expert pairs of two
+# task families."
+# Readings (Q38): P_f[l,e] = D[l,f,e] / max(1, N_f), the per-expert activation
+# probability of the same paragraph; the distance is reported per layer (the 2-norm of a row) and
+# over the whole [L,E] matrix (row L of the output); the top pairs are taken per layer among pairs
+# that co-activated at least once, most frequent first, ties -> smaller (i,j); the Jaccard
+# similarity of two empty sets is 0; row L is the mean over layers.
+# --------------------------------------------------------------------------
+def top_pairs(Cf: np.ndarray, topk: int = 64) -> List[Tuple[int, int]]:
+    """The topk unordered pairs (i<j) of one family's count matrix, most frequent first."""
+    E = Cf.shape[0]
+    pairs = [(i, j) for i in range(E) for j in range(i + 1, E) if int(Cf[i][j]) > 0]
+    pairs.sort(key=lambda ij: (-int(Cf[ij[0]][ij[1]]), ij[0], ij[1]))
+    return pairs[:topk]
+
+
+def family_divergence(D: np.ndarray, C: np.ndarray, ntok: np.ndarray, topk: int = 64):
+    """D [L,F,E], C [L,F,E,E], ntok [F] -> (frob float64[L+1,F,F], jaccard float64[L+1,F,F])."""
+    L, F, E = D.shape
+    frob = np.zeros((L + 1, F, F))
+    jac = np.zeros((L + 1, F, F))
+    sq_all = [[0.0] * F for _ in range(F)]
+    for l in range(L):
+        P = [[float(D[l][f][e]) / max(1.0, float(ntok[f])) for e in range(E)] for f in range(F)]
+        sets = [set(top_pairs(C[l][f], topk)) for f in range(F)]
+        for f in range(F):
+            for g in range(F):
+                sq = sum((P[f][e] - P[g][e]) ** 2 for e in range(E))
+                frob[l, f, g] = math.sqrt(sq)
+                sq_all[f][g] += sq
+                union = len(sets[f] | sets[g])
+                jac[l, f, g] = len(sets[f] & sets[g]) / union if union else 0.0
+    for f in range(F):
+        for g in range(F):
+            frob[L, f, g] = math.sqrt(sq_all[f][g])
+            jac[L, f, g] = sum(jac[l, f, g] for l in range(L)) / L
+    return frob, jac

@@ -622,3 +622,60 @@ def test_spectral_place_planted_and_close_to_exhaustive():
     W = np.random.default_rng(5).random((10, 10))
     pr, _, _ = ref.spectral_place(W, 4, 3)
     assert np.bincount(pr, minlength=4).max() <= 3
+
+
+# ---------------------------------------------------------------------------------------------
+# O15 -- motivation diagnostics
+# ---------------------------------------------------------------------------------------------
+def test_family_divergence_handworked_and_library():
+    # hand-worked: E = 4, two families, one layer
+    C = np.zeros((1, 2, 4, 4), dtype=np.int64)
+
+    def put(f, i, j, v):
+        C[0, f, i, j] = C[0, f, j, i] = v
+
+    put(0, 0, 1, 5); put(0, 2, 3, 5); put(0, 0, 2, 1)           # family 0: (0,1)=5 (2,3)=5 (0,2)=1
+    put(1, 0, 1, 2); put(1, 1, 3, 7)                            # family 1: (1,3)=7 (0,1)=2
+    assert ref.top_pairs(C[0, 0], 2) == [(0, 1), (2, 3)]        # equal counts: smaller (i,j) first
+    assert ref.top_pairs(C[0, 0], 64) == [(0, 1), (2, 3), (0, 2)]   # never a pair that did not co-activate
+    assert ref.top_pairs(C[0, 1], 1) == [(1, 3)]
+    D = np.array([[[4, 2, 2, 0], [1, 3, 0, 4]]], dtype=np.int64)
+    ntok = np.array([4, 8], dtype=np.int64)
+    frob, jac = ref.family_divergence(D, C, ntok, topk=2)
+    # P0 = (1, .5, .5, 0), P1 = (.125, .375, 0, .5): squared differences .765625 + .015625 + .25 + .25
+    assert abs(frob[0, 0, 1] - np.sqrt(1.28125)) < 1e-15 and frob[0, 0, 0] == 0 and frob[0, 0, 1] == frob[0, 1, 0]
+    assert (frob[1] == frob[0]).all()                           # one layer: the matrix norm is the row norm
+    # top-2 sets {(0,1),(2,3)} and {(1,3),(0,1)}: 1 common of 3
+    assert abs(jac[0, 0, 1] - 1 / 3) < 1e-15 and jac[0, 0, 0] == 1.0 and jac[0, 1, 1] == 1.0
+    # against library routines on a random case: matrix Frobenius norm, argsort-based top sets
+    rng = np.random.default_rng(11)
+    L, F, E, k = 3, 3, 9, 7
+    D = rng.integers(0, 50, size=(L, F, E))
+    ntok = rng.integers(1, 40, size=F)
+    C = rng.integers(0, 6, size=(L, F, E, E))
+    C = np.triu(C, 1)
+    C = C + C.transpose(0, 1, 3, 2)
+    frob, jac = ref.family_divergence(D, C, ntok, topk=k)
+    Pm = D / ntok[None, :, None]
+    for f in range(F):
+        for g in range(F):
+            assert abs(frob[L, f, g] - np.linalg.norm(Pm[:, f] - Pm[:, g], "fro")) < 1e-12
+            for l in range(L):
+                assert abs(frob[l, f, g] - np.linalg.norm(Pm[l, f] - Pm[l, g])) < 1e-12
+    iu = np.triu_indices(E, 1)
+    for l in range(L):
+        sets = []
+        for f in range(F):
+            v = C[l, f][iu]
+            order = np.argsort(-v, kind="stable")               # stable: row-major (i,j) order among equals
+            sets.append({(int(iu[0][t]), int(iu[1][t])) for t in order[:k] if v[t] > 0})
+        for f in range(F):
+            for g in range(F):
+                u = len(sets[f] | sets[g])
+                assert abs(jac[l, f, g] - (len(sets[f] & sets[g]) / u if u else 0.0)) < 1e-15
+    assert np.allclose(jac[L], jac[:L].mean(axis=0))
+    # identical families: distance 0, overlap 1; a family with no tokens: empty set, overlap 0 with everything
+    D2 = np.stack([D[:, 0], D[:, 0], np.zeros_like(D[:, 0])], axis=1)
+    C2 = np.stack([C[:, 0], C[:, 0], np.zeros_like(C[:, 0])], axis=1)
+    frob, jac = ref.family_divergence(D2, C2, np.array([5, 5, 0]), topk=k)
+    assert (frob[:, 0, 1] == 0).all() and (jac[:, 0, 1] == 1).all() and (jac[:, 2, :] == 0).all()
