@@ -193,6 +193,23 @@ int tacg_spectral_place(tacg_ctx* ctx,
                         int8_t* labels0,         /* dev [L,E] out or NULL */
                         double* embed);          /* dev [L,E,P] out or NULL */
 
+/* SURVEY.md 8(f) f3 (adjacent to the hot path) -- the motivation diagnostics of PAPER.md:469 from
+ * the counts of tacg_coact_accumulate:
+ *   P_f[l,e] = D[l,f,e]/max(1,ntok[f]);   frob[l,f,g] = ||P_f[l,:] - P_g[l,:]||_2 for l < L and
+ *   frob[L,f,g] = ||P_f - P_g||_F over the whole [L,E] matrix;
+ *   T_f[l] = the topk unordered pairs {i<j} of largest C[l,f,i,j] among pairs with a positive count
+ *   (ties -> smaller (i,j));   jaccard[l,f,g] = |T_f ^ T_g| / |T_f u T_g| (0 when both are empty),
+ *   jaccard[L,f,g] = mean over layers.
+ * The sets are exact (integer select); the two outputs are fp64 on the device, stored as fp32.
+ * TACG_ERR_SHAPE for E > 512, F > 8 or topk outside [1,256]. */
+int tacg_family_divergence(tacg_ctx* ctx,
+                           const uint32_t* D,    /* dev [L,F,E] */
+                           const uint32_t* C,    /* dev [L,F,E,E] */
+                           const uint64_t* ntok, /* dev [F] */
+                           int L, int E, int F, int topk,
+                           float* frob,          /* dev [L+1,F,F] out */
+                           float* jaccard);      /* dev [L+1,F,F] out */
+
 /* S8..S12 -- score a placement over a held-out trace (Eq. 13-15,
  * Comm per PAPER.md:363, Jain/MaxVio Eq. 17-18).  Tokens are processed
  * in micro-batches of `microbatch` consecutive tokens; every token of a micro-batch sees

@@ -8,7 +8,7 @@ ABI can be inspected), but creating a Context without an sm_100 device raises.
 from .binding import (  # noqa: F401
     Context, TacgError, lib, lib_path, version,
     tacg_coact_accumulate, tacg_affinity_swapgain, gesr_select, tacg_eval_placement, gesr_build_replicas,
-    tacg_spectral_place,
+    tacg_spectral_place, tacg_family_divergence,
     TACG_ZERO_FIRST, TACG_VALIDATE, TACG_PATH_AUTO, TACG_PATH_HIST, TACG_PATH_MMA,
     TACG_PROF_COACT, TACG_PROF_AFFINITY, TACG_PROF_EVAL, EXPORTS,
 )

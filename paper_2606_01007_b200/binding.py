@@ -26,7 +26,7 @@ TACG_PROF_COACT, TACG_PROF_AFFINITY, TACG_PROF_EVAL = 0, 1, 2
 EXPORTS = (
     "tacg_create", "tacg_destroy", "tacg_strerror", "tacg_last_detail", "tacg_last_path",
     "tacg_launch_count", "tacg_version", "tacg_profile_enable", "tacg_profile_read", "tacg_coact_accumulate", "tacg_affinity_swapgain",
-    "gesr_select", "tacg_eval_placement", "gesr_build_replicas", "tacg_spectral_place",
+    "gesr_select", "tacg_eval_placement", "gesr_build_replicas", "tacg_spectral_place", "tacg_family_divergence",
 )
 
 _lib = None
@@ -71,6 +71,7 @@ def lib():
         L.gesr_select.argtypes = [vp, vp, i64, i32, i32, i32, i32, vp, vp, i32, vp, f32, i64, vp, u32]
         L.gesr_build_replicas.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, f32, f32, f32, f32, f32,
                                           i32, i32, vp, vp]
+        L.tacg_family_divergence.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, vp, vp]
         L.tacg_spectral_place.argtypes = [vp, vp, i32, i32, i32, i32, f64, i32, vp, vp, vp, vp]
         L.tacg_eval_placement.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, i32, vp, vp, i32, f32, f64,
                                           i64, i64, vp, vp, vp, vp, vp, vp, vp, vp, u32]
@@ -175,6 +176,11 @@ class Context:
             float(alpha), float(tau), float(eps), float(lambda1), float(lambda2), int(n_rep), int(r),
             _ptr(replicas, torch.int8, "replicas"), _ptr(terms, torch.float32, "terms"))
 
+    def tacg_family_divergence(self, D, Cm, ntok, L, E, F, topk, frob, jaccard) -> int:
+        return lib().tacg_family_divergence(
+            self._h, _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"), _ptr(ntok, torch.int64, "ntok"),
+            int(L), int(E), int(F), int(topk), _ptr(frob, torch.float32, "frob"), _ptr(jaccard, torch.float32, "jaccard"))
+
     def tacg_spectral_place(self, W, L, E, P, capacity, jitter, kmeans_iters, labels_in, primary, labels0, embed) -> int:
         return lib().tacg_spectral_place(
             self._h, _ptr(W, torch.float32, "W"), int(L), int(E), int(P), int(capacity), float(jitter),
@@ -253,6 +259,16 @@ def gesr_build_replicas(ctx: Context, D, Cm, ntok, P: int, capacity: int, primar
     ctx.check(ctx.gesr_build_replicas(D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps, lambda1, lambda2,
                                       n_rep, r, replicas, terms), "gesr_build_replicas")
     return replicas, terms
+
+
+def tacg_family_divergence(ctx: Context, D, Cm, ntok, topk: int = 64):
+    """Activation Frobenius distance and top-k pair Jaccard overlap between task families:
+    returns (frob float32[L+1,F,F], jaccard float32[L+1,F,F]); row L = whole model."""
+    L, F, E = D.shape
+    frob = torch.empty((L + 1, F, F), dtype=torch.float32, device=D.device)
+    jac = torch.empty((L + 1, F, F), dtype=torch.float32, device=D.device)
+    ctx.check(ctx.tacg_family_divergence(D, Cm, ntok, L, E, F, topk, frob, jac), "tacg_family_divergence")
+    return frob, jac
 
 
 def tacg_spectral_place(ctx: Context, W, P: int, capacity: int, jitter: float = 1e-6, kmeans_iters: int = 100,

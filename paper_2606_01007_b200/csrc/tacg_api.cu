@@ -232,6 +232,16 @@ int tacg_spectral_place(tacg_ctx* ctx, const float* W, int L, int E, int P, int 
     return tacg_launch_spectral(ctx, W, L, E, P, capacity, jitter, kmeans_iters, labels_in, primary, labels0, embed);
 }
 
+int tacg_family_divergence(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L, int E,
+                           int F, int topk, float* frob, float* jaccard) {
+    if (!ctx) return TACG_ERR_NULL;
+    if (L < 1 || E < 1 || E > 512 || F < 1 || F > 8 || topk < 1 || topk > 256)
+        return fail(ctx, TACG_ERR_SHAPE, "family_divergence: L/E/F/topk out of range");
+    if (!D || !C || !ntok || !frob || !jaccard) return fail(ctx, TACG_ERR_NULL, "family_divergence: NULL pointer");
+    TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    return tacg_launch_divergence(ctx, D, C, ntok, L, E, F, topk, frob, jaccard);
+}
+
 int gesr_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P, const int8_t* primary,
                 const int8_t* replicas, int r, const double* load_snapshot, float theta, int64_t token_offset,
                 int8_t* serve, uint32_t flags) {

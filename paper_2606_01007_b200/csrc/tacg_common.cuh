@@ -92,6 +92,9 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
 // Spectral-then-repair primary placement (tacg_spectral_place).
 int tacg_launch_spectral(tacg_ctx* ctx, const float* W, int L, int E, int P, int capacity, double jitter, int iters,
                          const int8_t* labels_in, int8_t* primary, int8_t* labels0, double* embed);
+// Family-divergence diagnostics (tacg_family_divergence).
+int tacg_launch_divergence(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, const uint64_t* ntok, int L, int E,
+                           int F, int topk, float* frob, float* jaccard);
 int tacg_launch_select(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P,
                        const int8_t* primary, const int8_t* replicas, int r, const double* snapshot,
                        float theta, int64_t token_offset, int8_t* serve);
