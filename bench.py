@@ -357,7 +357,7 @@ def main():
         "traffic": ncu_traffic(args.config, used_path), "kernel": f"coact_{used_path}_kernel", "peak_source": peak_src,
         "algorithmic_bytes_per_launch": abytes, "avg_launch_ms": co_avg_ms, "launches_timed": co_n,
         "coact_routed_tokens_per_s": cfg.L * cfg.N / (co_avg_ms * 1e-3) if co_avg_ms > 0 else 0.0,
-        "other_kernels_avg_ms": {"affinity_swapgain(4 kernels)": af_ms / max(1, af_n), "eval_kernel": ev_ms / max(1, ev_n)},
+        "other_kernels_avg_ms": {"affinity_fused_kernel": af_ms / max(1, af_n), "eval_kernel": ev_ms / max(1, ev_n)},
     }
 
     # ---- optional: the co-activation call alone on both paths

@@ -10,10 +10,15 @@
 // The E x E work is HBM/L2 streaming of C (4*F*E*E bytes per layer); the contraction
 // pref.pref^T has inner dimension F <= 8 and W.M is a segmented row sum over a one-hot
 // membership matrix, so neither is tensor-core work.
+#include <cooperative_groups.h>
+
 #include "tacg_common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
+constexpr int kCluster = 8;        // CTAs per layer (one thread-block cluster)
 constexpr int kRowsPerCta = 8;     // one warp per matrix row
 constexpr int kRowThreads = kRowsPerCta * 32;
 
@@ -55,28 +60,6 @@ __device__ __forceinline__ double w_entry(double abar, double iamax, const doubl
     return (1.0 - alpha) * ah + alpha * (at * ah);
 }
 
-__global__ void __launch_bounds__(kRowThreads)
-rowstats_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, AffScratch s) {
-    const int l = blockIdx.y;
-    const int i = blockIdx.x * kRowsPerCta + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (i >= E) return;
-    double nf[8];
-    for (int f = 0; f < F; ++f) nf[f] = 1.0 / ((double)F * (double)max(1ull, ntok[f]));
-    const unsigned* Cl = C + (size_t)l * F * E * E;
-    double rmax = 0.0;
-    for (int j = lane; j < E; j += 32) rmax = fmax(rmax, abar_entry(Cl, nf, F, E, i, j));
-    rmax = warp_max(rmax);
-    for (int f = 0; f < F; ++f) {
-        unsigned long long acc = 0;
-        for (int j = lane; j < E; j += 32) acc += __ldg(&Cl[((size_t)f * E + i) * E + j]);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-        if (lane == 0) s.rowsum[((size_t)l * F + f) * E + i] = acc;
-    }
-    if (lane == 0) s.rowmax[(size_t)l * E + i] = rmax;
-}
-
 // relative advantage of family f at one expert: x^f - mean of the other families (Eq. 2-3, Q5)
 __device__ __forceinline__ double rel_adv(const double* x, int E, int F, int f, int e) {
     double other = 0.0;
@@ -88,36 +71,110 @@ __device__ __forceinline__ double rel_adv(const double* x, int E, int F, int f, 
     return x[f * E + e] - other;
 }
 
-// One CTA per layer.  Dynamic smem: u[F][E], c[F][E], sc[F][E], dv[F][E] doubles.
-__global__ void __launch_bounds__(256)
-pref_kernel(const unsigned* __restrict__ D, const unsigned long long* __restrict__ ntok, int E, int F, double tau,
-            double eps, AffScratch s, float* __restrict__ pref_out) {
-    extern __shared__ double psm[];
-    __shared__ double red[64];
-    double* u = psm;
-    double* c = psm + (size_t)F * E;
-    double* sc = psm + (size_t)2 * F * E;
-    double* dv = psm + (size_t)3 * F * E;
-    const int l = blockIdx.x;
-    const unsigned* Dl = D + (size_t)l * F * E;
-    // Warp f owns family f (F <= 8 = warps of the CTA): every sum over experts is a warp reduction,
-    // so the only CTA-wide barriers are the two below.
-    const int f = threadIdx.x >> 5, lane = threadIdx.x & 31;
+// Region A of the fused kernel's shared memory holds first the four F x E work arrays of the preference
+// step, later kRowsPerCta W rows and the partition order (E shorts): the larger of the two, in doubles.
+__host__ __device__ __forceinline__ size_t region_a_doubles(int E, int F) {
+    const size_t pref = (size_t)4 * F * E, graph = (size_t)kRowsPerCta * E + (size_t)(E + 3) / 4;
+    return pref > graph ? pref : graph;
+}
+
+struct AffArgs {
+    const unsigned* C;                 // [L,F,E,E]
+    const unsigned* D;                 // [L,F,E]
+    const unsigned long long* ntok;    // [F]
+    int E, F, P;
+    const int8_t* primary;             // [L,E] or NULL
+    double alpha, tau, eps;
+    AffScratch s;
+    float* pref_out;                   // any of the four may be NULL
+    float* W_out;
+    float* aff_out;
+    float* gain_out;
+    int need_graph;                    // W, aff or gain wanted (or the GESR step follows)
+};
+
+// One thread-block cluster of kCluster CTAs per layer walks S3..S7 in one launch.  Row blocks of
+// kRowsPerCta rows (one warp per row) are dealt round-robin to the CTAs of the cluster; the two points
+// where a row needs every other row's result (the z-scores of Eq. 4 need all row sums, the gains need all
+// affinities) are cluster barriers instead of kernel boundaries.  The preference table is small (E x F),
+// so every CTA computes its own copy into shared memory rather than exchanging it.
+// Dynamic smem: region A = 4*F*E doubles (u, c, sc, dv of the preference step; afterwards the W rows of
+// this CTA's row block and the partition order), region B = E*F doubles (the preference table).
+__global__ void __cluster_dims__(kCluster, 1, 1) __launch_bounds__(kRowThreads)
+affinity_fused_kernel(AffArgs a) {
+    extern __shared__ double fsm[];
+    __shared__ double red[kRowsPerCta];
+    __shared__ double amax_s;
+    __shared__ int start[65];
+    cg::cluster_group cluster = cg::this_cluster();
+    const int E = a.E, F = a.F, P = a.P;
+    const int l = blockIdx.x / kCluster, rank = blockIdx.x % kCluster;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const AffScratch s = a.s;
+    const unsigned* Cl = a.C + (size_t)l * F * E * E;
+    const int nblocks = (E + kRowsPerCta - 1) / kRowsPerCta;
+    double nf[8];
+    for (int f = 0; f < F; ++f) nf[f] = 1.0 / ((double)F * (double)max(1ull, a.ntok[f]));
+
+    // ---- row sums of C^f and the row maxima of Abar, for this CTA's rows ----
+    for (int b = rank; b < nblocks; b += kCluster) {
+        const int i = b * kRowsPerCta + warp;
+        if (i >= E) continue;
+        // one pass over the F rows: integer row sums and the row maximum of Abar together
+        double rmax = 0.0;
+        unsigned long long acc[8];
+#pragma unroll
+        for (int f = 0; f < 8; ++f) acc[f] = 0ull;
+        for (int j = lane; j < E; j += 32) {
+            double ab = 0.0;
+#pragma unroll
+            for (int f = 0; f < 8; ++f) {
+                if (f < F) {
+                    const unsigned v = __ldg(&Cl[((size_t)f * E + i) * E + j]);
+                    acc[f] += v;
+                    ab += (double)v * nf[f];
+                }
+            }
+            rmax = fmax(rmax, ab);
+        }
+        rmax = warp_max(rmax);
+#pragma unroll
+        for (int f = 0; f < 8; ++f) {
+            if (f < F) {
+                unsigned long long t = acc[f];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+                if (lane == 0) s.rowsum[((size_t)l * F + f) * E + i] = t;
+            }
+        }
+        if (lane == 0) s.rowmax[(size_t)l * E + i] = rmax;
+    }
+    cluster.sync();        // release/acquire at cluster scope: the scratch rows written above are visible to the cluster
+
+    // ---- preferences of the whole layer (every CTA its own copy) ----
+    double* u = fsm;
+    double* c = fsm + (size_t)F * E;
+    double* sc = fsm + (size_t)2 * F * E;
+    double* dv = fsm + (size_t)3 * F * E;
+    double* ptab = fsm + region_a_doubles(E, F);    // [E][F]
+    const unsigned* Dl = a.D + (size_t)l * F * E;
+    // Warp f owns family f (F <= 8 = warps of the CTA): every sum over experts is a warp reduction.
     // O2: u = D / sum D (Q1), c = rowsum(C)/N_f (Eq. 2 right; counts >= 0 so |.| is the identity, Q3)
-    if (f < F) {
+    if (warp < F) {
+        const int f = warp;
         double part = 0.0;
         for (int e = lane; e < E; e += 32) part += (double)Dl[f * E + e];          // exact: integers < 2^53
         const double tot = fmax(1.0, warp_sum(part));
-        const double nf = (double)max(1ull, ntok[f]);
+        const double nfam = (double)max(1ull, a.ntok[f]);
         for (int e = lane; e < E; e += 32) {
             u[f * E + e] = (double)Dl[f * E + e] / tot;
-            c[f * E + e] = (double)s.rowsum[((size_t)l * F + f) * E + e] / nf;
+            c[f * E + e] = (double)s.rowsum[((size_t)l * F + f) * E + e] / nfam;
         }
     }
     __syncthreads();
     // O3, O4: relative advantage (Eq. 2-3) and z-score over experts (Eq. 4), summed into s (Eq. 5).
-    // The relative advantages of a pass are computed once into dv (owned by warp f) and reused.
-    if (f < F) {
+    if (warp < F) {
+        const int f = warp;
         for (int e = lane; e < E; e += 32) sc[f * E + e] = 0.0;
         for (int pass = 0; pass < 2; ++pass) {
             const double* x = pass == 0 ? u : c;
@@ -134,53 +191,45 @@ pref_kernel(const unsigned* __restrict__ D, const unsigned long long* __restrict
                 vpart += d * d;
             }
             const double sigma = sqrt(warp_sum(vpart) / (double)E);
-            for (int e = lane; e < E; e += 32) sc[f * E + e] += (dv[f * E + e] - mu) / (sigma + eps);
+            for (int e = lane; e < E; e += 32) sc[f * E + e] += (dv[f * E + e] - mu) / (sigma + a.eps);
         }
     }
     __syncthreads();
     // O5: temperature softmax over families (Eq. 6), max subtracted
-    for (int e = threadIdx.x; e < E; e += blockDim.x) {
+    for (int e = threadIdx.x; e < E; e += kRowThreads) {
         double m = -INFINITY;
-        for (int f = 0; f < F; ++f) m = fmax(m, sc[f * E + e] / tau);
+        for (int f = 0; f < F; ++f) m = fmax(m, sc[f * E + e] / a.tau);
         double ex[8];
         double tot = 0.0;
         for (int f = 0; f < F; ++f) {
-            ex[f] = exp(sc[f * E + e] / tau - m);
+            ex[f] = exp(sc[f * E + e] / a.tau - m);
             tot += ex[f];
         }
         for (int f = 0; f < F; ++f) {
             const double p = ex[f] / tot;
-            s.pref64[((size_t)l * E + e) * F + f] = p;
-            if (pref_out) pref_out[((size_t)l * E + e) * F + f] = (float)p;
+            ptab[(size_t)e * F + f] = p;
+            if (a.pref_out && rank == 0) a.pref_out[((size_t)l * E + e) * F + f] = (float)p;
         }
     }
     // max Abar over the layer (Q8)
     double mx = 0.0;
-    for (int e = threadIdx.x; e < E; e += blockDim.x) mx = fmax(mx, s.rowmax[(size_t)l * E + e]);
+    for (int e = threadIdx.x; e < E; e += kRowThreads) mx = fmax(mx, s.rowmax[(size_t)l * E + e]);
     mx = warp_max(mx);
-    __syncthreads();
-    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+    if (lane == 0) red[warp] = mx;
     __syncthreads();
     if (threadIdx.x == 0) {
         double t = 0.0;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t = fmax(t, red[w]);
-        s.amax[l] = t;
+        for (int w = 0; w < kRowsPerCta; ++w) t = fmax(t, red[w]);
+        amax_s = t;
     }
-}
+    __syncthreads();
+    if (!a.need_graph) return;                       // uniform over the cluster
 
-// Dynamic smem: wrow[kRowsPerCta][E] doubles, then order[E] int16 (experts sorted by partition),
-// start[65] int.
-__global__ void __launch_bounds__(kRowThreads)
-graph_aff_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, int P,
-                 const int8_t* __restrict__ primary, double alpha, AffScratch s, float* __restrict__ W_out,
-                 float* __restrict__ aff_out) {
-    extern __shared__ double gsm[];
-    double* wrow = gsm;
-    short* order = reinterpret_cast<short*>(gsm + (size_t)kRowsPerCta * E);
-    __shared__ int start[65];
-    const int l = blockIdx.y;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int8_t* pr = primary ? primary + (size_t)l * E : nullptr;
+    // ---- W rows (Eq. 8) and their per-partition sums (Eq. 10), for this CTA's rows ----
+    const double iamax = amax_s > 0.0 ? 1.0 / amax_s : 0.0;
+    double* wrow = fsm;                                                   // region A is free again
+    short* order = reinterpret_cast<short*>(fsm + (size_t)kRowsPerCta * E);
+    const int8_t* pr = a.primary ? a.primary + (size_t)l * E : nullptr;
     if (pr) {
         // counting sort of the experts by partition, ascending expert id inside a partition
         if (threadIdx.x < P) {
@@ -201,61 +250,49 @@ graph_aff_kernel(const unsigned* __restrict__ C, const unsigned long long* __res
         }
         __syncthreads();
     }
-    const int i = blockIdx.x * kRowsPerCta + warp;
-    if (i >= E) return;
-    double nf[8], pi[8];
-    for (int f = 0; f < F; ++f) {
-        nf[f] = 1.0 / ((double)F * (double)max(1ull, ntok[f]));
-        pi[f] = s.pref64[((size_t)l * E + i) * F + f];
-    }
-    const unsigned* Cl = C + (size_t)l * F * E * E;
-    const double amax = s.amax[l] > 0.0 ? 1.0 / s.amax[l] : 0.0;
     double* wr = wrow + (size_t)warp * E;
-    for (int j = lane; j < E; j += 32) {
-        const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), amax, pi, s.pref64 + ((size_t)l * E + j) * F, F, alpha);
-        wr[j] = w;
-        if (W_out) W_out[((size_t)l * E + i) * E + j] = (float)w;
-    }
-    __syncwarp();
-    if (pr) {
-        // aff[i,m] = sum over the members of partition m, in ascending expert id (Eq. 10 inner sum)
-        for (int m = lane; m < P; m += 32) {
-            double acc = 0.0;
-            for (int q = start[m]; q < start[m + 1]; ++q) acc += wr[order[q]];
-            s.aff64[((size_t)l * E + i) * P + m] = acc;
-            if (aff_out) aff_out[((size_t)l * E + i) * P + m] = (float)acc;
+    for (int b = rank; b < nblocks; b += kCluster) {
+        const int i = b * kRowsPerCta + warp;
+        if (i >= E) continue;
+        const double* pi = ptab + (size_t)i * F;
+        for (int j = lane; j < E; j += 32) {
+            const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), iamax, pi, ptab + (size_t)j * F, F, a.alpha);
+            wr[j] = w;
+            if (a.W_out) a.W_out[((size_t)l * E + i) * E + j] = (float)w;
         }
+        __syncwarp();
+        if (pr) {
+            // aff[i,m] = sum over the members of partition m, in ascending expert id (Eq. 10 inner sum)
+            for (int m = lane; m < P; m += 32) {
+                double acc = 0.0;
+                for (int q = start[m]; q < start[m + 1]; ++q) acc += wr[order[q]];
+                s.aff64[((size_t)l * E + i) * P + m] = acc;
+                if (a.aff_out) a.aff_out[((size_t)l * E + i) * P + m] = (float)acc;
+            }
+        }
+        __syncwarp();
     }
-}
+    if (!a.gain_out) return;                         // uniform over the cluster
+    cluster.sync();        // release/acquire at cluster scope: the scratch rows written above are visible to the cluster
 
-__global__ void __launch_bounds__(kRowThreads)
-gain_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, int P,
-            const int8_t* __restrict__ primary, double alpha, AffScratch s, float* __restrict__ gain_out) {
-    const int l = blockIdx.y;
-    const int i = blockIdx.x * kRowsPerCta + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (i >= E) return;
-    const int8_t* pr = primary + (size_t)l * E;
-    double nf[8], pi[8];
-    for (int f = 0; f < F; ++f) {
-        nf[f] = 1.0 / ((double)F * (double)max(1ull, ntok[f]));
-        pi[f] = s.pref64[((size_t)l * E + i) * F + f];
-    }
-    const unsigned* Cl = C + (size_t)l * F * E * E;
-    const double amax = s.amax[l] > 0.0 ? 1.0 / s.amax[l] : 0.0;
+    // ---- all-pairs swap gains from the affinities of both endpoints and W (recomputed in fp64) ----
     const double* affl = s.aff64 + (size_t)l * E * P;
-    const int a = pr[i] & 63;
-    for (int j = lane; j < E; j += 32) {
-        const int b = pr[j] & 63;
-        double g = 0.0;
-        if (a != b) {
-            const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), amax, pi, s.pref64 + ((size_t)l * E + j) * F, F, alpha);
-            g = affl[(size_t)i * P + b] + affl[(size_t)j * P + a] - affl[(size_t)i * P + a] - affl[(size_t)j * P + b] - 2.0 * w;
+    for (int b = rank; b < nblocks; b += kCluster) {
+        const int i = b * kRowsPerCta + warp;
+        if (i >= E) continue;
+        const double* pi = ptab + (size_t)i * F;
+        const int pa = pr[i] & 63;
+        for (int j = lane; j < E; j += 32) {
+            const int pb = pr[j] & 63;
+            double g = 0.0;
+            if (pa != pb) {
+                const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), iamax, pi, ptab + (size_t)j * F, F, a.alpha);
+                g = affl[(size_t)i * P + pb] + affl[(size_t)j * P + pa] - affl[(size_t)i * P + pa] - affl[(size_t)j * P + pb] - 2.0 * w;
+            }
+            a.gain_out[((size_t)l * E + i) * E + j] = (float)g;
         }
-        gain_out[((size_t)l * E + i) * E + j] = (float)g;
     }
 }
-
 
 // ---------------------------------------------------------------------------------------------
 // GESR offline step: Eq. 11 scores and the Eq. 12 replica table.
@@ -415,21 +452,15 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     const unsigned long long* nt = reinterpret_cast<const unsigned long long*>(ntok);
     const dim3 rows((E + kRowsPerCta - 1) / kRowsPerCta, L);
     tacg_prof_scope prof(ctx, TACG_PROF_AFFINITY);
-    rowstats_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, s);
+    AffArgs a;
+    a.C = C; a.D = D; a.ntok = nt; a.E = E; a.F = F; a.P = P; a.primary = primary;
+    a.alpha = alpha; a.tau = tau; a.eps = eps; a.s = s;
+    a.pref_out = pref; a.W_out = W; a.aff_out = aff; a.gain_out = gain;
+    a.need_graph = (W || aff || gain || gesr) ? 1 : 0;
+    const size_t smem = sizeof(double) * (region_a_doubles(E, F) + (size_t)E * F);
+    TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(affinity_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    affinity_fused_kernel<<<L * kCluster, kRowThreads, smem, ctx->stream>>>(a);
     TACG_LAUNCH_CHECK(ctx);
-    const size_t psm = sizeof(double) * (size_t)4 * F * E;
-    TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(pref_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)psm));
-    pref_kernel<<<L, 256, psm, ctx->stream>>>(D, nt, E, F, tau, eps, s, pref);
-    TACG_LAUNCH_CHECK(ctx);
-    if (W || aff || gain || gesr) {
-        const size_t gsm = sizeof(double) * (size_t)kRowsPerCta * E + sizeof(short) * (size_t)E;
-        graph_aff_kernel<<<rows, kRowThreads, gsm, ctx->stream>>>(C, nt, E, F, P, primary, alpha, s, W, aff);
-        TACG_LAUNCH_CHECK(ctx);
-    }
-    if (gain) {
-        gain_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, P, primary, alpha, s, gain);
-        TACG_LAUNCH_CHECK(ctx);
-    }
     if (gesr) {
         gesr_score_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, gesr->lambda1, gesr->lambda2, s, gesr->terms);
         TACG_LAUNCH_CHECK(ctx);
