@@ -100,6 +100,8 @@ struct AffArgs {
 // so every CTA computes its own copy into shared memory rather than exchanging it.
 // Dynamic smem: region A = 4*F*E doubles (u, c, sc, dv of the preference step; afterwards the W rows of
 // this CTA's row block and the partition order), region B = E*F doubles (the preference table).
+// FT = the family count at compile time (4 and 8: the paper's F = 4 and the ABI maximum), 0 = runtime.
+template <int FT>
 __global__ void __cluster_dims__(kCluster, 1, 1) __launch_bounds__(kRowThreads)
 affinity_fused_kernel(AffArgs a) {
     extern __shared__ double fsm[];
@@ -107,7 +109,7 @@ affinity_fused_kernel(AffArgs a) {
     __shared__ double amax_s;
     __shared__ int start[65];
     cg::cluster_group cluster = cg::this_cluster();
-    const int E = a.E, F = a.F, P = a.P;
+    const int E = a.E, F = FT ? FT : a.F, P = a.P;
     const int l = blockIdx.x / kCluster, rank = blockIdx.x % kCluster;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const AffScratch s = a.s;
@@ -458,9 +460,14 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     a.pref_out = pref; a.W_out = W; a.aff_out = aff; a.gain_out = gain;
     a.need_graph = (W || aff || gain || gesr) ? 1 : 0;
     const size_t smem = sizeof(double) * (region_a_doubles(E, F) + (size_t)E * F);
-    TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(affinity_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    affinity_fused_kernel<<<L * kCluster, kRowThreads, smem, ctx->stream>>>(a);
-    TACG_LAUNCH_CHECK(ctx);
+    auto launch = [&](auto kernel) -> int {
+        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        kernel<<<L * kCluster, kRowThreads, smem, ctx->stream>>>(a);
+        TACG_LAUNCH_CHECK(ctx);
+        return TACG_OK;
+    };
+    const int rc = F == 4 ? launch(affinity_fused_kernel<4>) : F == 8 ? launch(affinity_fused_kernel<8>) : launch(affinity_fused_kernel<0>);
+    if (rc != TACG_OK) return rc;
     if (gesr) {
         gesr_score_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, gesr->lambda1, gesr->lambda2, s, gesr->terms);
         TACG_LAUNCH_CHECK(ctx);
