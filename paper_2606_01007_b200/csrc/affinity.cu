@@ -104,6 +104,7 @@ struct AffArgs {
 template <int FT>
 __global__ void __cluster_dims__(kCluster, 1, 1) __launch_bounds__(kRowThreads)
 affinity_fused_kernel(AffArgs a) {
+    tacg_pdl_prologue();
     extern __shared__ double fsm[];
     __shared__ double red[kRowsPerCta];
     __shared__ double amax_s;
@@ -462,7 +463,7 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     const size_t smem = sizeof(double) * (region_a_doubles(E, F) + (size_t)E * F);
     auto launch = [&](auto kernel) -> int {
         TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        kernel<<<L * kCluster, kRowThreads, smem, ctx->stream>>>(a);
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(kernel, dim3(L * kCluster), dim3(kRowThreads), smem, ctx->stream, a));
         TACG_LAUNCH_CHECK(ctx);
         return TACG_OK;
     };

@@ -188,6 +188,7 @@ __device__ __forceinline__ void count_token(const int16_t* __restrict__ row, int
 // CP (non-filter mode only): bank-spread copies of the pair bins, one per quarter warp.
 template <int KT, bool FILTER, int CP>
 __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParams p) {
+    tacg_pdl_prologue();
     extern __shared__ __align__(16) unsigned hsm[];
     const int tid = threadIdx.x;
     const int g = FILTER ? blockIdx.x / p.nfg : blockIdx.x;
@@ -363,6 +364,7 @@ template <bool ZERO>
 __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p, unsigned* __restrict__ D,
                                                             unsigned* __restrict__ C,
                                                             unsigned long long* __restrict__ ntok) {
+    tacg_pdl_prologue();
     const int lf = blockIdx.y;
     const int l = lf / p.F, f = lf % p.F;
     const int E = p.E, tri = p.tri;
@@ -453,7 +455,7 @@ template <int KT, bool FILTER, int CP>
 int launch_hist(tacg_ctx* ctx, const HistParams& p, size_t smem, int grid) {
     auto kern = coact_hist_kernel<KT, FILTER, CP>;
     TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<grid, kThreads, smem, ctx->stream>>>(p);
+    TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kThreads), smem, ctx->stream, p));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
@@ -535,8 +537,8 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     if (rc != TACG_OK) return rc;
     unsigned long long* nt = reinterpret_cast<unsigned long long*>(ntok);
     const dim3 fgrid((E + 7) / 8, L * F);
-    if (zero_first) coact_finalize_kernel<true><<<fgrid, 256, 0, ctx->stream>>>(p, D, C, nt);
-    else coact_finalize_kernel<false><<<fgrid, 256, 0, ctx->stream>>>(p, D, C, nt);
+    if (zero_first) TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_finalize_kernel<true>, fgrid, dim3(256), 0, ctx->stream, p, D, C, nt));
+    else TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_finalize_kernel<false>, fgrid, dim3(256), 0, ctx->stream, p, D, C, nt));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }

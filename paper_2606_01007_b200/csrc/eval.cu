@@ -291,6 +291,7 @@ __device__ __forceinline__ void load_row_raw(const int16_t* __restrict__ row, un
 template <int KT, bool REP, typename M, bool OUT>
 __global__ void __launch_bounds__(kEvalThreads, 2)
 eval_kernel(EvalParams p) {
+    tacg_pdl_prologue();
     extern __shared__ __align__(16) unsigned char esm[];
     constexpr int KM = KT > 0 ? KT : 16;
     constexpr int U = KT > 0 ? kEvalBatch : 1;
@@ -622,6 +623,7 @@ eval_kernel(EvalParams p) {
 // statistics are then computed by one thread from the P sums in the fixed order m = 0..P-1.
 __global__ void __launch_bounds__(1024) fairness_kernel(const unsigned long long* __restrict__ load, int L, int P,
                                                        float* __restrict__ out) {
+    tacg_pdl_prologue();
     __shared__ unsigned long long part[16][64];
     __shared__ double x[64];
     const int row = blockIdx.x;
@@ -703,6 +705,7 @@ select_kernel(const int16_t* __restrict__ indices, long long N, int k, int E, in
 __global__ void eval_zero_kernel(unsigned long long* a, size_t na, unsigned long long* b, size_t nb,
                                  unsigned long long* c, size_t nc, unsigned long long* d, size_t nd,
                                  unsigned long long* s, size_t ns) {
+    tacg_pdl_prologue();
     const size_t stride = (size_t)gridDim.x * blockDim.x;
     const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     for (size_t i = i0; i < na; i += stride) a[i] = 0ull;
@@ -760,9 +763,9 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     {
         const size_t ns = p.cpl > 1 ? off / sizeof(unsigned long long) : 0;
         const int zgrid = (int)max((size_t)1, min((size_t)ctx->sm_count, (ns + 1023) / 1024));
-        eval_zero_kernel<<<zgrid, 1024, 0, ctx->stream>>>(p.comm_span, (size_t)p.L * p.F, p.comm_remote, (size_t)p.L * p.F,
-                                                          p.load, (size_t)p.L * p.P, p.ntok, (size_t)p.F,
-                                                          reinterpret_cast<unsigned long long*>(base), ns);
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(eval_zero_kernel, dim3(zgrid), dim3(1024), 0, ctx->stream, p.comm_span,
+                                           (size_t)p.L * p.F, p.comm_remote, (size_t)p.L * p.F, p.load, (size_t)p.L * p.P,
+                                           p.ntok, (size_t)p.F, reinterpret_cast<unsigned long long*>(base), ns));
         TACG_LAUNCH_CHECK(ctx);
     }
     tacg_prof_scope prof(ctx, TACG_PROF_EVAL);
@@ -772,7 +775,7 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
                                                        ctx->stream));
         ctx->launches += 1;
     } else {
-        kern<<<grid, kEvalThreads, smem, ctx->stream>>>(p);
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kEvalThreads), smem, ctx->stream, p));
         TACG_LAUNCH_CHECK(ctx);
     }
     return TACG_OK;
@@ -845,7 +848,8 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         }
         if (rc != TACG_OK) return rc;
     }
-    fairness_kernel<<<L + 1, 1024, 0, ctx->stream>>>(reinterpret_cast<const unsigned long long*>(load), L, P, fairness);
+    TACG_CUDA_TRY(ctx, tacg_launch_pdl(fairness_kernel, dim3(L + 1), dim3(1024), 0, ctx->stream,
+                                       reinterpret_cast<const unsigned long long*>(load), L, P, fairness));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }

@@ -106,6 +106,32 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
 
 // ---- device helpers ----
 #ifdef __CUDACC__
+// Programmatic dependent launch: the kernels of one step are launched with
+// tacg_launch_pdl and begin with tacg_pdl_prologue().  The prologue lets the NEXT kernel of the stream start
+// being scheduled (its CTAs become resident as resources free up) and then blocks until the PREVIOUS kernel
+// has completed and its memory is visible, so everything after the prologue is ordered exactly as with plain
+// stream serialisation; what is saved is the drain-and-dispatch gap between small dependent kernels.
+__device__ __forceinline__ void tacg_pdl_prologue() {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t tacg_launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                                   Args... args) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
 // Static work split of the co-activation kernels: T items (layer-major) over `groups` CTA groups;
 // group g owns items [g*T/groups, (g+1)*T/groups) and writes one scratch slot per layer it visits.
 __host__ __device__ __forceinline__ long long group_lo(long long g, long long T, int groups) {
