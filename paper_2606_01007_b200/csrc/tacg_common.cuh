@@ -106,13 +106,13 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
 
 // ---- device helpers ----
 #ifdef __CUDACC__
-// Programmatic dependent launch: the kernels of one step are launched with
-// tacg_launch_pdl and begin with tacg_pdl_prologue().  The prologue lets the NEXT kernel of the stream start
-// being scheduled (its CTAs become resident as resources free up) and then blocks until the PREVIOUS kernel
-// has completed and its memory is visible, so everything after the prologue is ordered exactly as with plain
-// stream serialisation; what is saved is the drain-and-dispatch gap between small dependent kernels.
+// Programmatic dependent launch: the kernels of one step are launched with tacg_launch_pdl and begin with
+// tacg_pdl_prologue(), which blocks until the PREVIOUS kernel of the stream has completed and its memory is
+// visible.  Everything after the prologue is ordered exactly as with plain stream serialisation; what is saved
+// is the drain-and-dispatch gap between small dependent kernels (the dependent grid is set up while its
+// predecessor finishes).  No kernel triggers its dependents early: measured, an early trigger packs the next
+// kernel's CTAs onto the first SMs that free up and costs more than it saves.
 __device__ __forceinline__ void tacg_pdl_prologue() {
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     asm volatile("griddepcontrol.wait;" ::: "memory");
 }
 
