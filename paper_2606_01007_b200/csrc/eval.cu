@@ -303,6 +303,10 @@ eval_kernel(EvalParams p) {
     // deferred-token queue of each warp (replicated slots are resolved 32 tokens at a time)
     constexpr bool kQueued = REP && KT > 0 && sizeof(M) == 4;
     unsigned* wqueue = reinterpret_cast<unsigned*>(esm + off) + (threadIdx.x >> 5) * (kDeferCap * kDeferWords);
+    if (kQueued) off += sizeof(unsigned) * (size_t)(kEvalThreads / 32) * kDeferCap * kDeferWords;
+    // per-family packed accumulators, one word per (warp, family, lane): a token is one shared atomic on its own
+    // thread's word instead of a compare-select-add per family
+    unsigned* acc = reinterpret_cast<unsigned*>(esm + off) + (threadIdx.x >> 5) * (8 * 32) + (threadIdx.x & 31);
     __shared__ double Ls[64];              // EMA state of this layer
     __shared__ unsigned long long ltot[64];  // cumulative integer load of this layer
     __shared__ unsigned long long feas_s;
@@ -329,25 +333,25 @@ eval_kernel(EvalParams p) {
         if (tid < 8) fam_s[tid] = 0u;
         __syncthreads();
         // per family, over this thread's tokens: span (bits 0-10) | remote (11-21) | token count (22-31)
-        unsigned acc[8];
 #pragma unroll
-        for (int g = 0; g < 8; ++g) acc[g] = 0u;
+        for (int g = 0; g < 8; ++g) acc[g * 32] = 0u;
         int since = 0;                      // tokens added to acc since the last flush (uniform per warp)
         auto flush_acc = [&]() {
 #pragma unroll
             for (int g = 0; g < 8; ++g) {
                 if (g < F) {
-                    const unsigned s = __reduce_add_sync(0xffffffffu, acc[g] & 0x7ffu);
-                    const unsigned q = __reduce_add_sync(0xffffffffu, (acc[g] >> 11) & 0x7ffu);
+                    const unsigned av = acc[g * 32];
+                    const unsigned s = __reduce_add_sync(0xffffffffu, av & 0x7ffu);
+                    const unsigned q = __reduce_add_sync(0xffffffffu, (av >> 11) & 0x7ffu);
                     if (lane == 0) {
                         if (s) atomicAdd(&comm_s[g], (unsigned long long)s);
                         if (q) atomicAdd(&comm_s[8 + g], (unsigned long long)q);
                     }
                     if (layer == 0) {               // tokens per family, counted once (family is shared by all layers)
-                        const unsigned c = __reduce_add_sync(0xffffffffu, acc[g] >> 22);
+                        const unsigned c = __reduce_add_sync(0xffffffffu, av >> 22);
                         if (lane == 0 && c) atomicAdd(&fam_s[g], c);
                     }
-                    acc[g] = 0u;
+                    acc[g * 32] = 0u;
                 }
             }
             since = 0;
@@ -420,12 +424,7 @@ eval_kernel(EvalParams p) {
                     R = serve_pending_packed<KM, M>(e, pend, hm, R, T, svp);
                 }
                 const unsigned packed = finish_packed(svp, R, hm, (int)q[5]);
-#pragma unroll
-                for (int g = 0; g < 4; ++g) acc[g] += (fq == g) ? packed : 0u;
-                if (F > 4) {
-#pragma unroll
-                    for (int g = 4; g < 8; ++g) acc[g] += (fq == g) ? packed : 0u;
-                }
+                atomicAdd(&acc[fq * 32], packed);         // queued tokens are live: fq < F
             }
             qn -= nact;
             __syncwarp();
@@ -451,6 +450,7 @@ eval_kernel(EvalParams p) {
             const int n = t1 > t0 ? (int)(t1 - t0) : 0;            // tokens of the slice (per <= 2^31 checked on the host)
             slice0 = t0;
             int home = (int)((p.token_offset + t0 + tid) % P);
+            M notHome = ~((M)1 << home);            // constant over the slice when P divides the CTA width (stepP == 0)
             const int8_t* fam0 = p.family + t0;
             const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
             for (int ob = tid; ob < n + tid; ob += kEvalThreads * U) {      // uniform trip count across the CTA
@@ -526,7 +526,6 @@ eval_kernel(EvalParams p) {
                                 for (int j = 0; j < KM; ++j)
                                     if (j < k && sv[j] >= 0) atomicAdd(cnt_lane + sv[j] * 32, 1u);
                             }
-                            const M notHome = ~((M)1 << home);
                             int nR, rem;
                             if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
                             else { nR = __popc(R); rem = __popc(R & notHome); }
@@ -544,13 +543,8 @@ eval_kernel(EvalParams p) {
                         if (OUT && serve_l)
                             for (int j = 0; j < k; ++j) serve_l[((size_t)t0 + o) * k + j] = -1;
                     }
-                    // packed is 0 unless f[u] is a family < F, so no bound check on g is needed
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) acc[g] += (f[u] == g) ? packed : 0u;
-                    if (F > 4) {
-#pragma unroll
-                        for (int g = 4; g < 8; ++g) acc[g] += (f[u] == g) ? packed : 0u;
-                    }
+                    // packed is 0 unless f[u] is a family < F
+                    if (packed) atomicAdd(&acc[f[u] * 32], packed);
                     if constexpr (kQueued) {
                         const unsigned dm = __ballot_sync(0xffffffffu, defer);
                         if (defer) {
@@ -563,8 +557,11 @@ eval_kernel(EvalParams p) {
                         qn += __popc(dm);
                         if (qn >= 32) drain(32);
                     }
-                    home += stepP;
-                    if (home >= P) home -= P;
+                    if (stepP) {
+                        home += stepP;
+                        if (home >= P) home -= P;
+                        notHome = ~((M)1 << home);
+                    }
                 }
                 since += kQueued ? 2 * U : U;     // a queued token adds to acc when it is drained
                 if (since >= 120) flush_acc();      // 11-bit fields: 124 tokens x (span <= 15, remote <= 16) fit
@@ -717,7 +714,8 @@ __global__ void eval_zero_kernel(unsigned long long* a, size_t na, unsigned long
 
 size_t eval_smem_bytes(int E, int P, int r) {
     return tables_bytes(E, r) + 64 * sizeof(unsigned long long) + sizeof(unsigned) * (size_t)P * 32 +
-           (r > 0 ? sizeof(unsigned) * (size_t)(kEvalThreads / 32) * kDeferCap * kDeferWords : 0);
+           (r > 0 ? sizeof(unsigned) * (size_t)(kEvalThreads / 32) * kDeferCap * kDeferWords : 0) +
+           sizeof(unsigned) * (size_t)(kEvalThreads / 32) * 8 * 32;
 }
 
 template <int KT>
