@@ -87,3 +87,68 @@ def test_random_shapes(tacg, ctx, seed):
         sv = tacg.gesr_select(ctx, di, E, P, torch.from_numpy(primary).cuda(), torch.from_numpy(replicas).cuda(),
                               torch.from_numpy(snap).cuda(), theta, token_offset=2)
         assert (sv.cpu().numpy() == cbind.gesr_select(idx, E, P, primary, replicas, snap, theta, 2)).all()
+
+
+@pytest.mark.parametrize("seed", list(range(16)))
+def test_random_shapes_offline_stage(tacg, ctx, seed):
+    """The E x E kernels on awkward shapes: the cluster-fused affinity kernel (every family count 1..8, E not a
+    multiple of the 8-row blocks or of the cluster's 64 rows, more layers than clusters fit), the GESR offline step,
+    the capacity repair and the divergence diagnostics, against the oracle."""
+    from oracle import ref
+    rng = np.random.default_rng(5000 + seed)
+    k = int(rng.choice([2, 4, 6, 8, 3]))
+    E = int(rng.integers(max(k, 3), 200))
+    F = int(rng.integers(1, 9))
+    L = int(rng.choice([1, 2, 3, 21]))
+    N = int(rng.choice([300, 2000, 6000]))
+    P = int(rng.integers(2, min(E, 64) + 1))
+    cap = -(-E // P) + int(rng.integers(0, 3))
+    idx = np.empty((L, N, k), dtype=np.int16)
+    hot = rng.dirichlet(np.full(E, 0.3), size=(L, F))                # family-dependent popularity, so sigma > 0
+    fam = rng.integers(0, F, size=N).astype(np.int8)
+    for l in range(L):
+        keys = rng.random((N, E)) ** (1.0 / np.maximum(hot[l][fam], 1e-9))
+        idx[l] = np.argsort(-keys, axis=1)[:, :k]
+    D, C, ntok = cbind.coact(idx, fam, E, F)
+    primary = tracegen.random_placement(E, P, cap, L, seed=seed)
+    alpha, tau = float(rng.choice([0.0, 0.25, 0.6])), float(rng.choice([0.5, 1.0, 2.0]))
+    want = cbind.affinity_swapgain(D, C, ntok, P, primary, alpha=float(np.float32(alpha)), tau=float(np.float32(tau)),
+                                   eps=float(np.float32(1e-6)))
+    dD = torch.from_numpy(D.view(np.int32)).cuda()
+    dC = torch.from_numpy(C.view(np.int32)).cuda()
+    dn = torch.from_numpy(ntok.view(np.int64)).cuda()
+    dp = torch.from_numpy(primary).cuda()
+    got = tacg.tacg_affinity_swapgain(ctx, dD, dC, dn, P, cap, dp, alpha=alpha, tau=tau, eps=1e-6)
+    torch.cuda.synchronize()
+    for key in ("pref", "W", "aff"):
+        g = got[key].cpu().numpy().astype(np.float64)
+        assert (np.abs(g - want[key]) <= 1e-5 * np.maximum(np.abs(want[key]), 1e-6)).all(), key
+    G = got["gain"].cpu().numpy().astype(np.float64)
+    for l in range(L):
+        pr = primary[l].astype(np.int64)
+        aff, W = want["aff"][l], want["W"][l]
+        ia, ib = aff[np.arange(E), pr], aff[:, pr]
+        mag = np.abs(ib) + np.abs(ib.T) + np.abs(ia)[:, None] + np.abs(ia)[None, :] + 2 * np.abs(W)
+        assert (np.abs(G[l] - want["gain"][l]) <= 1e-5 * np.maximum(mag, 1e-6)).all(), ("gain", l)
+    # W alone (no placement): the kernel leaves before the affinity phases
+    only_w = tacg.tacg_affinity_swapgain(ctx, dD, dC, dn, P, cap, None, alpha=alpha, tau=tau, eps=1e-6, want=("W",))["W"]
+    assert torch.equal(only_w, got["W"])
+    # GESR offline terms
+    _, terms = tacg.gesr_build_replicas(ctx, dD, dC, dn, P, cap, dp, max(1, E // 8), min(2, P - 1), lambda1=0.5,
+                                        lambda2=0.25, alpha=alpha, tau=tau)
+    sc = ref.gesr_scores(C[0].astype(np.int64), ntok, 0.5, 0.25)
+    t0 = terms[0].cpu().numpy().astype(np.float64)
+    for col, key in enumerate(("score", "cent", "cons", "spec")):
+        assert np.allclose(t0[:, col], sc[key], rtol=1e-5, atol=1e-9), key
+    # capacity repair from skewed labels: exact
+    Wh = np.ascontiguousarray(want["W"], dtype=np.float32)
+    labels = np.minimum(rng.geometric(0.4, size=(L, E)) - 1, P - 1).astype(np.int8)
+    rep = tacg.tacg_spectral_place(ctx, torch.from_numpy(Wh).cuda(), P, cap, labels_in=torch.from_numpy(labels).cuda())
+    for l in range(min(L, 3)):
+        assert rep["primary"][l].cpu().numpy().tolist() == ref.capacity_repair(ref.scaled_affinity(Wh[l]), labels[l], P, cap)
+    # divergence diagnostics on the first layers
+    Ls = min(L, 2)
+    fr, jc = tacg.tacg_family_divergence(ctx, dD[:Ls].contiguous(), dC[:Ls].contiguous(), dn, topk=64)
+    wf, wj = ref.family_divergence(D[:Ls].astype(np.int64), C[:Ls].astype(np.int64), ntok.astype(np.int64), topk=64)
+    assert (jc[:-1].cpu().numpy() == wj[:-1].astype(np.float32)).all()
+    assert np.allclose(fr.cpu().numpy().astype(np.float64), wf, rtol=1e-6, atol=1e-12)
