@@ -109,6 +109,8 @@ affinity_fused_kernel(AffArgs a) {
     __shared__ double red[kRowsPerCta];
     __shared__ double amax_s;
     __shared__ int start[65];
+    __shared__ double nf_s[8];
+    __shared__ short order[512];          // experts sorted by partition (E <= 512)
     cg::cluster_group cluster = cg::this_cluster();
     const int E = a.E, F = FT ? FT : a.F, P = a.P;
     const int l = blockIdx.x / kCluster, rank = blockIdx.x % kCluster;
@@ -116,8 +118,40 @@ affinity_fused_kernel(AffArgs a) {
     const AffScratch s = a.s;
     const unsigned* Cl = a.C + (size_t)l * F * E * E;
     const int nblocks = (E + kRowsPerCta - 1) / kRowsPerCta;
+    const int8_t* pr = a.primary ? a.primary + (size_t)l * E : nullptr;
+    // Up front, off the critical path: the per-family reciprocals (one division each for the CTA, not per
+    // thread) and the experts sorted by partition (ascending id inside a partition), one warp per partition:
+    // ballots over 32 experts at a time.
+    if (threadIdx.x < F) nf_s[threadIdx.x] = 1.0 / ((double)F * (double)max(1ull, a.ntok[threadIdx.x]));
+    if (pr && a.need_graph) {
+        for (int m = warp; m < P; m += kRowsPerCta) {
+            int n = 0;
+            for (int e0 = 0; e0 < E; e0 += 32) {
+                const int e = e0 + lane;
+                n += __popc(__ballot_sync(0xffffffffu, e < E && pr[e] == m));
+            }
+            if (lane == 0) start[m + 1] = n;
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            start[0] = 0;
+            for (int m = 0; m < P; ++m) start[m + 1] += start[m];
+        }
+        __syncthreads();
+        for (int m = warp; m < P; m += kRowsPerCta) {
+            int pos = start[m];
+            for (int e0 = 0; e0 < E; e0 += 32) {
+                const int e = e0 + lane;
+                const bool mine = e < E && pr[e] == m;
+                const unsigned bal = __ballot_sync(0xffffffffu, mine);
+                if (mine) order[pos + __popc(bal & ((1u << lane) - 1u))] = (short)e;
+                pos += __popc(bal);
+            }
+        }
+    }
+    __syncthreads();
     double nf[8];
-    for (int f = 0; f < F; ++f) nf[f] = 1.0 / ((double)F * (double)max(1ull, a.ntok[f]));
+    for (int f = 0; f < F; ++f) nf[f] = nf_s[f];
 
     // ---- row sums of C^f and the row maxima of Abar, for this CTA's rows ----
     for (int b = rank; b < nblocks; b += kCluster) {
@@ -175,37 +209,41 @@ affinity_fused_kernel(AffArgs a) {
         }
     }
     __syncthreads();
-    // O3, O4: relative advantage (Eq. 2-3) and z-score over experts (Eq. 4), summed into s (Eq. 5).
-    if (warp < F) {
-        const int f = warp;
-        for (int e = lane; e < E; e += 32) sc[f * E + e] = 0.0;
-        for (int pass = 0; pass < 2; ++pass) {
-            const double* x = pass == 0 ? u : c;
-            double part = 0.0;
-            for (int e = lane; e < E; e += 32) {
-                const double d = rel_adv(x, E, F, f, e);
-                dv[f * E + e] = d;
-                part += d;
-            }
-            const double mu = warp_sum(part) / (double)E;
-            double vpart = 0.0;
-            for (int e = lane; e < E; e += 32) {
-                const double d = dv[f * E + e] - mu;
-                vpart += d * d;
-            }
-            const double sigma = sqrt(warp_sum(vpart) / (double)E);
-            for (int e = lane; e < E; e += 32) sc[f * E + e] += (dv[f * E + e] - mu) / (sigma + a.eps);
+    // O3, O4: relative advantage (Eq. 2-3) and z-score over experts (Eq. 4).  One warp per (family, quantity):
+    // the usage and the co-activation z-scores are independent, so 2F warps work at once; each leaves its
+    // z-scores in place of its relative advantages and Eq. 5 adds the two in the softmax below.
+    for (int task = warp; task < 2 * F; task += kRowsPerCta) {
+        const int f = task % F, pass = task / F;
+        const double* x = pass == 0 ? u : c;
+        double* dvp = pass == 0 ? sc : dv;
+        double part = 0.0;
+        for (int e = lane; e < E; e += 32) {
+            const double d = rel_adv(x, E, F, f, e);
+            dvp[f * E + e] = d;
+            part += d;
         }
+        const double mu = warp_sum(part) / (double)E;
+        double vpart = 0.0;
+        for (int e = lane; e < E; e += 32) {
+            const double d = dvp[f * E + e] - mu;
+            vpart += d * d;
+        }
+        const double sigma = sqrt(warp_sum(vpart) / (double)E);
+        for (int e = lane; e < E; e += 32) dvp[f * E + e] = (dvp[f * E + e] - mu) / (sigma + a.eps);
     }
     __syncthreads();
     // O5: temperature softmax over families (Eq. 6), max subtracted
     for (int e = threadIdx.x; e < E; e += kRowThreads) {
         double m = -INFINITY;
-        for (int f = 0; f < F; ++f) m = fmax(m, sc[f * E + e] / a.tau);
+        double sv[8];
+        for (int f = 0; f < F; ++f) {
+            sv[f] = (sc[f * E + e] + dv[f * E + e]) / a.tau;       // s = z(du) + z(dc), Eq. 5
+            m = fmax(m, sv[f]);
+        }
         double ex[8];
         double tot = 0.0;
         for (int f = 0; f < F; ++f) {
-            ex[f] = exp(sc[f * E + e] / a.tau - m);
+            ex[f] = exp(sv[f] - m);
             tot += ex[f];
         }
         for (int f = 0; f < F; ++f) {
@@ -231,28 +269,6 @@ affinity_fused_kernel(AffArgs a) {
     // ---- W rows (Eq. 8) and their per-partition sums (Eq. 10), for this CTA's rows ----
     const double iamax = amax_s > 0.0 ? 1.0 / amax_s : 0.0;
     double* wrow = fsm;                                                   // region A is free again
-    short* order = reinterpret_cast<short*>(fsm + (size_t)kRowsPerCta * E);
-    const int8_t* pr = a.primary ? a.primary + (size_t)l * E : nullptr;
-    if (pr) {
-        // counting sort of the experts by partition, ascending expert id inside a partition
-        if (threadIdx.x < P) {
-            int n = 0;
-            for (int e = 0; e < E; ++e) n += (pr[e] == (int)threadIdx.x);
-            start[threadIdx.x + 1] = n;
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            start[0] = 0;
-            for (int m = 0; m < P; ++m) start[m + 1] += start[m];
-        }
-        __syncthreads();
-        if (threadIdx.x < P) {
-            int pos = start[threadIdx.x];
-            for (int e = 0; e < E; ++e)
-                if (pr[e] == (int)threadIdx.x) order[pos++] = (short)e;
-        }
-        __syncthreads();
-    }
     double* wr = wrow + (size_t)warp * E;
     for (int b = rank; b < nblocks; b += kCluster) {
         const int i = b * kRowsPerCta + warp;
