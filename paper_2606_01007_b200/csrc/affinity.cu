@@ -61,14 +61,12 @@ __device__ __forceinline__ double w_entry(double abar, double iamax, const doubl
 }
 
 // relative advantage of family f at one expert: x^f - mean of the other families (Eq. 2-3, Q5)
-__device__ __forceinline__ double rel_adv(const double* x, int E, int F, int f, int e) {
+// inv_others = 1/(F-1) (0 when F = 1): one reciprocal per warp instead of a division per expert
+__device__ __forceinline__ double rel_adv(const double* x, int E, int F, int f, int e, double inv_others) {
     double other = 0.0;
-    if (F > 1) {
-        for (int g = 0; g < F; ++g)
-            if (g != f) other += x[g * E + e];
-        other /= (double)(F - 1);
-    }
-    return x[f * E + e] - other;
+    for (int g = 0; g < F; ++g)
+        if (g != f) other += x[g * E + e];
+    return x[f * E + e] - other * inv_others;
 }
 
 // Region A of the fused kernel's shared memory holds first the four F x E work arrays of the preference
@@ -201,11 +199,11 @@ affinity_fused_kernel(AffArgs a) {
         const int f = warp;
         double part = 0.0;
         for (int e = lane; e < E; e += 32) part += (double)Dl[f * E + e];          // exact: integers < 2^53
-        const double tot = fmax(1.0, warp_sum(part));
-        const double nfam = (double)max(1ull, a.ntok[f]);
+        const double itot = 1.0 / fmax(1.0, warp_sum(part));
+        const double infam = 1.0 / (double)max(1ull, a.ntok[f]);
         for (int e = lane; e < E; e += 32) {
-            u[f * E + e] = (double)Dl[f * E + e] / tot;
-            c[f * E + e] = (double)s.rowsum[((size_t)l * F + f) * E + e] / nfam;
+            u[f * E + e] = (double)Dl[f * E + e] * itot;
+            c[f * E + e] = (double)s.rowsum[((size_t)l * F + f) * E + e] * infam;
         }
     }
     __syncthreads();
@@ -216,9 +214,10 @@ affinity_fused_kernel(AffArgs a) {
         const int f = task % F, pass = task / F;
         const double* x = pass == 0 ? u : c;
         double* dvp = pass == 0 ? sc : dv;
+        const double inv_others = F > 1 ? 1.0 / (double)(F - 1) : 0.0;
         double part = 0.0;
         for (int e = lane; e < E; e += 32) {
-            const double d = rel_adv(x, E, F, f, e);
+            const double d = rel_adv(x, E, F, f, e, inv_others);
             dvp[f * E + e] = d;
             part += d;
         }
@@ -228,16 +227,17 @@ affinity_fused_kernel(AffArgs a) {
             const double d = dvp[f * E + e] - mu;
             vpart += d * d;
         }
-        const double sigma = sqrt(warp_sum(vpart) / (double)E);
-        for (int e = lane; e < E; e += 32) dvp[f * E + e] = (dvp[f * E + e] - mu) / (sigma + a.eps);
+        const double isig = 1.0 / (sqrt(warp_sum(vpart) / (double)E) + a.eps);
+        for (int e = lane; e < E; e += 32) dvp[f * E + e] = (dvp[f * E + e] - mu) * isig;
     }
     __syncthreads();
     // O5: temperature softmax over families (Eq. 6), max subtracted
+    const double itau = 1.0 / a.tau;
     for (int e = threadIdx.x; e < E; e += kRowThreads) {
         double m = -INFINITY;
         double sv[8];
         for (int f = 0; f < F; ++f) {
-            sv[f] = (sc[f * E + e] + dv[f * E + e]) / a.tau;       // s = z(du) + z(dc), Eq. 5
+            sv[f] = (sc[f * E + e] + dv[f * E + e]) * itau;        // s = z(du) + z(dc), Eq. 5
             m = fmax(m, sv[f]);
         }
         double ex[8];
@@ -246,8 +246,9 @@ affinity_fused_kernel(AffArgs a) {
             ex[f] = exp(sv[f] - m);
             tot += ex[f];
         }
+        const double itot = 1.0 / tot;
         for (int f = 0; f < F; ++f) {
-            const double p = ex[f] / tot;
+            const double p = ex[f] * itot;
             ptab[(size_t)e * F + f] = p;
             if (a.pref_out && rank == 0) a.pref_out[((size_t)l * E + e) * F + f] = (float)p;
         }
