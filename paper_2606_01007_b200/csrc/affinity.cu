@@ -2,11 +2,11 @@
 // PAPER.md:97-108), expert->partition affinity (Eq. 10 inner sum) and all-pairs
 // swap gains (north_star).  All arithmetic is fp64 on device (DESIGN.md
 // "Precision": the z-score divides rounding noise by eps when sigma ~ 0, Q6), results are
-// rounded once to fp32 on store.  Four small kernels, each a grid over (row block, layer):
-//   rowstats : per (l,f,i) integer row sums of C and the row maximum of Abar
-//   pref     : per layer, u/c/du/dc/z/s/softmax and max Abar
-//   graph_aff: W rows and their per-partition segmented sums (aff)
-//   gain     : all-pairs swap gains from aff (fp64 scratch) and W (recomputed in fp64)
+// rounded once to fp32 on store.  One launch, a thread-block cluster per layer, four phases:
+//   row statistics : per (l,f,i) integer row sums of C and the row maximum of Abar      -> cluster barrier
+//   preferences    : per layer, u/c/du/dc/z/s/softmax and max Abar (every CTA its own copy)
+//   graph, affinity: W rows and their per-partition segmented sums (aff)                 -> cluster barrier
+//   gains          : all-pairs swap gains from aff (fp64 scratch) and W (recomputed in fp64)
 // The E x E work is HBM/L2 streaming of C (4*F*E*E bytes per layer); the contraction
 // pref.pref^T has inner dimension F <= 8 and W.M is a segmented row sum over a one-hot
 // membership matrix, so neither is tensor-core work.
