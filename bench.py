@@ -359,6 +359,18 @@ def main():
         "coact_routed_tokens_per_s": cfg.L * cfg.N / (co_avg_ms * 1e-3) if co_avg_ms > 0 else 0.0,
         "other_kernels_avg_ms": {"affinity_fused_kernel": af_ms / max(1, af_n), "eval_kernel": ev_ms / max(1, ev_n)},
     }
+    if used_path == "hist" and co_avg_ms > 0:
+        # What actually bounds the histogram kernel: k(k-1)/2 shared-memory atomic increments per
+        # token.  Peak from unit counts and the sampled clock: an ATOMS instruction whose 32 lanes hit 32 different
+        # banks takes 2 LSU wavefronts, one wavefront per clock and SM -> 16 increments per clock and SM.
+        sm_count = torch.cuda.get_device_properties(0).multi_processor_count
+        incs = cfg.L * cfg.N * (k * (k - 1) // 2)
+        apeak = 16.0 * sm_count * (clocks.get("sm_mhz") or 0) * 1e6
+        roofline["atomic_pipe"] = {
+            "achieved": incs / (co_avg_ms * 1e-3), "peak": apeak, "unit": "shared-memory increments/s",
+            "frac": (incs / (co_avg_ms * 1e-3)) / apeak if apeak else None,
+            "peak_source": "16 conflict-free lane increments / clk / SM x SMs x sampled SM clock (DESIGN.md 5.1)",
+        }
 
     # ---- optional: the co-activation call alone on both paths
     coact_paths = None
