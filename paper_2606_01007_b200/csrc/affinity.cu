@@ -322,6 +322,7 @@ affinity_fused_kernel(AffArgs a) {
 __global__ void __launch_bounds__(kRowThreads)
 gesr_score_kernel(const unsigned* __restrict__ C, const unsigned long long* __restrict__ ntok, int E, int F, double lam1,
                   double lam2, AffScratch s, float* __restrict__ terms_out) {
+    tacg_pdl_prologue();
     const int l = blockIdx.y;
     const int e = blockIdx.x * kRowsPerCta + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
@@ -380,6 +381,7 @@ gesr_score_kernel(const unsigned* __restrict__ C, const unsigned long long* __re
 __global__ void __launch_bounds__(256)
 gesr_pick_kernel(int E, int P, int n_rep, int r, const int8_t* __restrict__ primary, AffScratch s,
                  signed char* __restrict__ replicas) {
+    tacg_pdl_prologue();
     __shared__ unsigned char taken[512];
     __shared__ double wbest[8];
     __shared__ int wbest_e[8];
@@ -487,10 +489,11 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
     const int rc = F == 4 ? launch(affinity_fused_kernel<4>) : F == 8 ? launch(affinity_fused_kernel<8>) : launch(affinity_fused_kernel<0>);
     if (rc != TACG_OK) return rc;
     if (gesr) {
-        gesr_score_kernel<<<rows, kRowThreads, 0, ctx->stream>>>(C, nt, E, F, gesr->lambda1, gesr->lambda2, s, gesr->terms);
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(gesr_score_kernel, rows, dim3(kRowThreads), 0, ctx->stream, C, nt, E, F, gesr->lambda1,
+                                           gesr->lambda2, s, gesr->terms));
         TACG_LAUNCH_CHECK(ctx);
-        gesr_pick_kernel<<<L, 256, 0, ctx->stream>>>(E, P, gesr->n_rep, gesr->r, primary, s,
-                                                     reinterpret_cast<signed char*>(gesr->replicas));
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(gesr_pick_kernel, dim3(L), dim3(256), 0, ctx->stream, E, P, gesr->n_rep, gesr->r, primary, s,
+                                           reinterpret_cast<signed char*>(gesr->replicas)));
         TACG_LAUNCH_CHECK(ctx);
     }
     return TACG_OK;

@@ -109,6 +109,7 @@ __device__ __forceinline__ void ids_to_mask(const unsigned (&w)[KT / 2], int E, 
 
 template <int EP, int KT>
 __global__ void __launch_bounds__(kMmaThreads, 1) coact_mma_kernel(const MmaParams p) {
+    tacg_pdl_prologue();
     using G = MmaGeom<EP>;
     extern __shared__ __align__(128) unsigned char opbuf[];      // [2][kChunks + 1][kChunkBytes]
     __shared__ uint64_t full_bar[2], empty_bar[2], tmem_free_bar;
@@ -342,6 +343,7 @@ template <bool ZERO>
 __global__ void __launch_bounds__(512) coact_mma_finalize_kernel(const MmaParams p, unsigned* __restrict__ D,
                                                                 unsigned* __restrict__ C,
                                                                 unsigned long long* __restrict__ ntok) {
+    tacg_pdl_prologue();
     const int l = blockIdx.x / p.F, f = blockIdx.x % p.F;
     const int E = p.E;
     const int g0 = group_of_item((long long)l * p.cps, p.T, p.groups);
@@ -387,7 +389,7 @@ int launch_mma(tacg_ctx* ctx, const MmaParams& p) {
     const size_t smem = 2 * (size_t)G::kBufBytes;
     auto kern = coact_mma_kernel<EP, KT>;
     TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    kern<<<p.groups * p.nfg, kMmaThreads, smem, ctx->stream>>>(p);
+    TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(p.groups * p.nfg), dim3(kMmaThreads), smem, ctx->stream, p));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
@@ -438,8 +440,8 @@ int tacg_launch_coact_mma(tacg_ctx* ctx, const int16_t* indices, const int8_t* f
     int rc = EP == 64 ? launch_mma_k<64>(ctx, p) : (EP == 128 ? launch_mma_k<128>(ctx, p) : launch_mma_k<256>(ctx, p));
     if (rc != TACG_OK) return rc;
     unsigned long long* nt = reinterpret_cast<unsigned long long*>(ntok);
-    if (zero_first) coact_mma_finalize_kernel<true><<<L * F, 512, 0, ctx->stream>>>(p, D, C, nt);
-    else coact_mma_finalize_kernel<false><<<L * F, 512, 0, ctx->stream>>>(p, D, C, nt);
+    if (zero_first) TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_mma_finalize_kernel<true>, dim3(L * F), dim3(512), 0, ctx->stream, p, D, C, nt));
+    else TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_mma_finalize_kernel<false>, dim3(L * F), dim3(512), 0, ctx->stream, p, D, C, nt));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
