@@ -578,23 +578,29 @@ eval_kernel(EvalParams p) {
                 if (lane == 0) dsum[m] = (unsigned long long)s;
             }
             __syncthreads();
+            // Without replicas nothing in the micro-batch depends on the snapshot, so the CTAs of a layer only
+            // add their counts to the delta table and never wait for one another: eval_ema_kernel applies
+            // Eq. 15 to the table afterwards, in micro-batch order (the same fp64 operations, bit for bit).
+            const bool ema_here = REP || p.cpl == 1;
             if (p.cpl > 1) {
                 unsigned long long* dl = p.delta + ((size_t)layer * p.nmb + mb) * P;
                 if (tid < P && dsum[tid]) atomicAdd(&dl[tid], dsum[tid]);
-                __threadfence();
-                __syncthreads();
-                if (tid == 0) {
-                    atomicAdd(&p.barrier[layer], 1u);
-                    const unsigned target = (unsigned)((mb + 1) * p.cpl);
-                    volatile unsigned* bar = p.barrier + layer;
-                    while (*bar < target) __nanosleep(20);
+                if constexpr (REP) {
                     __threadfence();
+                    __syncthreads();
+                    if (tid == 0) {
+                        atomicAdd(&p.barrier[layer], 1u);
+                        const unsigned target = (unsigned)((mb + 1) * p.cpl);
+                        volatile unsigned* bar = p.barrier + layer;
+                        while (*bar < target) __nanosleep(20);
+                        __threadfence();
+                    }
+                    __syncthreads();
+                    if (tid < P) dsum[tid] = __ldcg(&dl[tid]);
+                    __syncthreads();
                 }
-                __syncthreads();
-                if (tid < P) dsum[tid] = __ldcg(&dl[tid]);
-                __syncthreads();
             }
-            if (tid < P) {
+            if (ema_here && tid < P) {
                 const unsigned long long d = dsum[tid];
                 Ls[tid] = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
                 ltot[tid] += d;
@@ -607,11 +613,31 @@ eval_kernel(EvalParams p) {
             if (comm_s[tid]) atomicAdd(&p.comm_span[(size_t)layer * F + tid], comm_s[tid]);
             if (comm_s[8 + tid]) atomicAdd(&p.comm_remote[(size_t)layer * F + tid], comm_s[8 + tid]);
         }
-        if (part == 0 && tid < P) {
+        if (part == 0 && tid < P && (REP || p.cpl == 1)) {
             p.load[(size_t)layer * P + tid] = ltot[tid];
             if (p.load_state) p.load_state[(size_t)layer * P + tid] = Ls[tid];
         }
     }
+}
+
+// Eq. 15 over the delta table of a layer (the no-replica path with several CTAs per layer): one CTA per layer,
+// thread m walks the micro-batches of partition m in order.  load = the integer total, load_state = the EMA.
+__global__ void __launch_bounds__(64) eval_ema_kernel(const unsigned long long* __restrict__ delta, int nmb, int P,
+                                                      double rho, unsigned long long* __restrict__ load,
+                                                      double* __restrict__ load_state) {
+    tacg_pdl_prologue();
+    const int layer = blockIdx.x, m = threadIdx.x;
+    if (m >= P) return;
+    double Ls = load_state ? load_state[(size_t)layer * P + m] : 0.0;
+    unsigned long long tot = 0ull;
+    const unsigned long long* dl = delta + (size_t)layer * nmb * P + m;
+    for (int mb = 0; mb < nmb; ++mb) {
+        const unsigned long long d = dl[(size_t)mb * P];
+        Ls = __dadd_rn(__dmul_rn(rho, Ls), (double)d);   // no FMA (Q19)
+        tot += d;
+    }
+    load[(size_t)layer * P + m] = tot;
+    if (load_state) load_state[(size_t)layer * P + m] = Ls;
 }
 
 // O11: (jain, maxvio, cv) per layer and for the loads summed over layers, fp64 -> fp32.
@@ -750,7 +776,7 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     }
     p.groups = (int)min((long long)p.L, (long long)max_grid / cpl);
     const int grid = p.groups * p.cpl;
-    const bool waits = p.cpl > 1 && p.nmb > 1;     // CTAs of a group meet at a barrier per micro-batch
+    const bool waits = rep && p.cpl > 1 && p.nmb > 1;     // CTAs of a group meet at a barrier per micro-batch
     size_t off = 0;
     const size_t o_delta = off; off += tacg_align_up(sizeof(unsigned long long) * (size_t)p.L * (size_t)p.nmb * p.P, 256);
     const size_t o_bar = off;   off += tacg_align_up(sizeof(unsigned) * (size_t)p.L, 256);
@@ -774,6 +800,11 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
         ctx->launches += 1;
     } else {
         TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kEvalThreads), smem, ctx->stream, p));
+        TACG_LAUNCH_CHECK(ctx);
+    }
+    if (!rep && p.cpl > 1) {
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(eval_ema_kernel, dim3(p.L), dim3(64), 0, ctx->stream,
+                                           (const unsigned long long*)p.delta, (int)p.nmb, p.P, p.rho, p.load, p.load_state));
         TACG_LAUNCH_CHECK(ctx);
     }
     return TACG_OK;
