@@ -620,39 +620,40 @@ eval_kernel(EvalParams p) {
     }
 }
 
-// Eq. 15 over the delta table of a layer (the no-replica path with several CTAs per layer): one CTA per layer,
-// thread m walks the micro-batches of partition m in order.  load = the integer total, load_state = the EMA.
-__global__ void __launch_bounds__(64) eval_ema_kernel(const unsigned long long* __restrict__ delta, int nmb, int P,
-                                                      double rho, unsigned long long* __restrict__ load,
-                                                      double* __restrict__ load_state) {
-    tacg_pdl_prologue();
-    const int layer = blockIdx.x, m = threadIdx.x;
-    if (m >= P) return;
-    double Ls = load_state ? load_state[(size_t)layer * P + m] : 0.0;
-    unsigned long long tot = 0ull;
-    const unsigned long long* dl = delta + (size_t)layer * nmb * P + m;
-    for (int mb = 0; mb < nmb; ++mb) {
-        const unsigned long long d = dl[(size_t)mb * P];
-        Ls = __dadd_rn(__dmul_rn(rho, Ls), (double)d);   // no FMA (Q19)
-        tot += d;
-    }
-    load[(size_t)layer * P + m] = tot;
-    if (load_state) load_state[(size_t)layer * P + m] = Ls;
-}
-
 // O11: (jain, maxvio, cv) per layer and for the loads summed over layers, fp64 -> fp32.
 // One CTA per output row (row L = loads summed over layers), 64 x 16 threads: thread (m, q) adds the
 // layers q, q+16, ... of partition m, so no thread walks more than L/16 dependent loads; the
 // statistics are then computed by one thread from the P sums in the fixed order m = 0..P-1.
-__global__ void __launch_bounds__(1024) fairness_kernel(const unsigned long long* __restrict__ load, int L, int P,
-                                                       float* __restrict__ out) {
+// delta != nullptr (the no-replica path with several CTAs per layer): the loads are not in `load` yet but in the
+// per-micro-batch count table; row l < L first applies Eq. 15 to its layer in micro-batch order (the same fp64
+// operations the evaluation kernel applies when it owns a layer alone) and writes load and load_state, row L sums
+// the table itself.
+__global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __restrict__ load, int L, int P,
+                                                       float* __restrict__ out, const unsigned long long* __restrict__ delta,
+                                                       int nmb, double rho, double* __restrict__ load_state) {
     tacg_pdl_prologue();
     __shared__ unsigned long long part[16][64];
     __shared__ double x[64];
     const int row = blockIdx.x;
     const int m = threadIdx.x & 63, q = threadIdx.x >> 6;
     unsigned long long v = 0;
-    if (m < P) {
+    if (m < P && delta) {
+        if (row < L) {
+            if (q == 0) {
+                double Ls = load_state ? load_state[(size_t)row * P + m] : 0.0;
+                const unsigned long long* dl = delta + (size_t)row * nmb * P + m;
+                for (int mb = 0; mb < nmb; ++mb) {
+                    const unsigned long long d = dl[(size_t)mb * P];
+                    Ls = __dadd_rn(__dmul_rn(rho, Ls), (double)d);   // no FMA (Q19)
+                    v += d;
+                }
+                load[(size_t)row * P + m] = v;
+                if (load_state) load_state[(size_t)row * P + m] = Ls;
+            }
+        } else {
+            for (long long i = q; i < (long long)L * nmb; i += 16) v += delta[(size_t)i * P + m];
+        }
+    } else if (m < P) {
         if (row < L) { if (q == 0) v = load[(size_t)row * P + m]; }
         else for (int l = q; l < L; l += 16) v += load[(size_t)l * P + m];
     }
@@ -802,11 +803,7 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
         TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kEvalThreads), smem, ctx->stream, p));
         TACG_LAUNCH_CHECK(ctx);
     }
-    if (!rep && p.cpl > 1) {
-        TACG_CUDA_TRY(ctx, tacg_launch_pdl(eval_ema_kernel, dim3(p.L), dim3(64), 0, ctx->stream,
-                                           (const unsigned long long*)p.delta, (int)p.nmb, p.P, p.rho, p.load, p.load_state));
-        TACG_LAUNCH_CHECK(ctx);
-    }
+    if (rep || p.cpl == 1) p.delta = nullptr;      // tells the caller that load and load_state are already final
     return TACG_OK;
 }
 
@@ -851,6 +848,8 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(load, 0, sizeof(uint64_t) * (size_t)L * P, ctx->stream));
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
     }
+    const unsigned long long* fin_delta = nullptr;   // set when the fairness kernel still has Eq. 15 to apply
+    int fin_nmb = 0;
     if (N > 0) {
         EvalParams p;
         p.indices = indices; p.family = family; p.N = N; p.k = k; p.L = L; p.E = E; p.F = F; p.P = P; p.r = r;
@@ -876,9 +875,12 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
             default: rc = launch_eval_t<0>(ctx, p); break;
         }
         if (rc != TACG_OK) return rc;
+        fin_delta = p.delta;
+        fin_nmb = (int)p.nmb;
     }
     TACG_CUDA_TRY(ctx, tacg_launch_pdl(fairness_kernel, dim3(L + 1), dim3(1024), 0, ctx->stream,
-                                       reinterpret_cast<const unsigned long long*>(load), L, P, fairness));
+                                       reinterpret_cast<unsigned long long*>(load), L, P, fairness,
+                                       (const unsigned long long*)fin_delta, fin_nmb, rho, load_state));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
