@@ -241,6 +241,7 @@ struct EvalParams {
     signed char* serve;     // [L,N,k] or null
     unsigned long long* delta;   // scratch [L,nmb,P], zeroed before launch (only used when cpl > 1)
     unsigned* barrier;           // scratch [L], zeroed before launch
+    unsigned long long* partial; // scratch [L,cpl,P+3F] (no-replica path): per-CTA loads | span | remote | tokens per family
     int cpl;                // CTAs per layer
     int groups;             // number of concurrent layer groups = gridDim.x / cpl
 };
@@ -578,14 +579,14 @@ eval_kernel(EvalParams p) {
                 if (lane == 0) dsum[m] = (unsigned long long)s;
             }
             __syncthreads();
-            // Without replicas nothing in the micro-batch depends on the snapshot, so the CTAs of a layer only
-            // add their counts to the delta table and never wait for one another: eval_ema_kernel applies
-            // Eq. 15 to the table afterwards, in micro-batch order (the same fp64 operations, bit for bit).
-            const bool ema_here = REP || p.cpl == 1;
-            if (p.cpl > 1) {
-                unsigned long long* dl = p.delta + ((size_t)layer * p.nmb + mb) * P;
-                if (tid < P && dsum[tid]) atomicAdd(&dl[tid], dsum[tid]);
-                if constexpr (REP) {
+            // Without replicas nothing depends on the snapshot (and the whole trace is one micro-batch): a CTA only
+            // writes its own row of partial sums, never waits and never touches an accumulated output;
+            // fairness_kernel adds the rows of a layer and applies Eq. 15.
+            const bool ema_here = REP;
+            if constexpr (REP) {
+                if (p.cpl > 1) {
+                    unsigned long long* dl = p.delta + ((size_t)layer * p.nmb + mb) * P;
+                    if (tid < P && dsum[tid]) atomicAdd(&dl[tid], dsum[tid]);
                     __threadfence();
                     __syncthreads();
                     if (tid == 0) {
@@ -599,6 +600,8 @@ eval_kernel(EvalParams p) {
                     if (tid < P) dsum[tid] = __ldcg(&dl[tid]);
                     __syncthreads();
                 }
+            } else {
+                if (tid < P) ltot[tid] += dsum[tid];
             }
             if (ema_here && tid < P) {
                 const unsigned long long d = dsum[tid];
@@ -608,14 +611,24 @@ eval_kernel(EvalParams p) {
             __syncthreads();
         }
         // layer epilogue: communication sums and, from part 0, loads and the final state
-        if (layer == 0 && tid < F && fam_s[tid]) atomicAdd(&p.ntok[tid], (unsigned long long)fam_s[tid]);
-        if (tid < F) {
-            if (comm_s[tid]) atomicAdd(&p.comm_span[(size_t)layer * F + tid], comm_s[tid]);
-            if (comm_s[8 + tid]) atomicAdd(&p.comm_remote[(size_t)layer * F + tid], comm_s[8 + tid]);
-        }
-        if (part == 0 && tid < P && (REP || p.cpl == 1)) {
-            p.load[(size_t)layer * P + tid] = ltot[tid];
-            if (p.load_state) p.load_state[(size_t)layer * P + tid] = Ls[tid];
+        if constexpr (REP) {
+            if (layer == 0 && tid < F && fam_s[tid]) atomicAdd(&p.ntok[tid], (unsigned long long)fam_s[tid]);
+            if (tid < F) {
+                if (comm_s[tid]) atomicAdd(&p.comm_span[(size_t)layer * F + tid], comm_s[tid]);
+                if (comm_s[8 + tid]) atomicAdd(&p.comm_remote[(size_t)layer * F + tid], comm_s[8 + tid]);
+            }
+            if (part == 0 && tid < P) {
+                p.load[(size_t)layer * P + tid] = ltot[tid];
+                if (p.load_state) p.load_state[(size_t)layer * P + tid] = Ls[tid];
+            }
+        } else {
+            unsigned long long* row = p.partial + ((size_t)layer * p.cpl + part) * (size_t)(P + 3 * F);
+            if (tid < P) row[tid] = ltot[tid];
+            if (tid < F) {
+                row[P + tid] = comm_s[tid];
+                row[P + F + tid] = comm_s[8 + tid];
+                row[P + 2 * F + tid] = layer == 0 ? (unsigned long long)fam_s[tid] : 0ull;
+            }
         }
     }
 }
@@ -624,34 +637,42 @@ eval_kernel(EvalParams p) {
 // One CTA per output row (row L = loads summed over layers), 64 x 16 threads: thread (m, q) adds the
 // layers q, q+16, ... of partition m, so no thread walks more than L/16 dependent loads; the
 // statistics are then computed by one thread from the P sums in the fixed order m = 0..P-1.
-// delta != nullptr (the no-replica path with several CTAs per layer): the loads are not in `load` yet but in the
-// per-micro-batch count table; row l < L first applies Eq. 15 to its layer in micro-batch order (the same fp64
-// operations the evaluation kernel applies when it owns a layer alone) and writes load and load_state, row L sums
-// the table itself.
+// partial != nullptr (the no-replica path): the CTAs of the evaluation kernel left one row of partial sums each
+// (loads | span | remote | tokens per family); row l < L adds the rows of its layer, applies Eq. 15 (one
+// micro-batch: the same two fp64 operations the evaluation kernel applies) and writes load, load_state, comm_span,
+// comm_remote and, from layer 0, ntok; row L sums the loads of all layers.
 __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __restrict__ load, int L, int P,
-                                                       float* __restrict__ out, const unsigned long long* __restrict__ delta,
-                                                       int nmb, double rho, double* __restrict__ load_state) {
+                                                       float* __restrict__ out, const unsigned long long* __restrict__ partial,
+                                                       int cpl, int F, double rho, double* __restrict__ load_state,
+                                                       unsigned long long* __restrict__ comm_span,
+                                                       unsigned long long* __restrict__ comm_remote,
+                                                       unsigned long long* __restrict__ ntok) {
     tacg_pdl_prologue();
     __shared__ unsigned long long part[16][64];
     __shared__ double x[64];
     const int row = blockIdx.x;
     const int m = threadIdx.x & 63, q = threadIdx.x >> 6;
     unsigned long long v = 0;
-    if (m < P && delta) {
+    if (partial) {
+        const size_t W = (size_t)(P + 3 * F);
         if (row < L) {
-            if (q == 0) {
-                double Ls = load_state ? load_state[(size_t)row * P + m] : 0.0;
-                const unsigned long long* dl = delta + (size_t)row * nmb * P + m;
-                for (int mb = 0; mb < nmb; ++mb) {
-                    const unsigned long long d = dl[(size_t)mb * P];
-                    Ls = __dadd_rn(__dmul_rn(rho, Ls), (double)d);   // no FMA (Q19)
-                    v += d;
-                }
+            const unsigned long long* rows = partial + (size_t)row * cpl * W;
+            if (q == 0 && m < P) {
+                for (int c = 0; c < cpl; ++c) v += rows[(size_t)c * W + m];
                 load[(size_t)row * P + m] = v;
-                if (load_state) load_state[(size_t)row * P + m] = Ls;
+                if (load_state) {
+                    const double Ls = load_state[(size_t)row * P + m];
+                    load_state[(size_t)row * P + m] = __dadd_rn(__dmul_rn(rho, Ls), (double)v);   // no FMA (Q19)
+                }
+            } else if (q >= 1 && q <= 3 && m < F && (q < 3 || row == 0)) {
+                unsigned long long t = 0;
+                for (int c = 0; c < cpl; ++c) t += rows[(size_t)c * W + P + (size_t)(q - 1) * F + m];
+                if (q == 1) comm_span[(size_t)row * F + m] = t;
+                else if (q == 2) comm_remote[(size_t)row * F + m] = t;
+                else ntok[m] = t;
             }
-        } else {
-            for (long long i = q; i < (long long)L * nmb; i += 16) v += delta[(size_t)i * P + m];
+        } else if (m < P) {
+            for (long long i = q; i < (long long)L * cpl; i += 16) v += partial[(size_t)i * W + m];
         }
     } else if (m < P) {
         if (row < L) { if (q == 0) v = load[(size_t)row * P + m]; }
@@ -779,19 +800,27 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
     const int grid = p.groups * p.cpl;
     const bool waits = rep && p.cpl > 1 && p.nmb > 1;     // CTAs of a group meet at a barrier per micro-batch
     size_t off = 0;
-    const size_t o_delta = off; off += tacg_align_up(sizeof(unsigned long long) * (size_t)p.L * (size_t)p.nmb * p.P, 256);
-    const size_t o_bar = off;   off += tacg_align_up(sizeof(unsigned) * (size_t)p.L, 256);
-    char* base = static_cast<char*>(tacg_scratch(ctx, off));
-    if (!base) return TACG_ERR_CUDA;
-    p.delta = reinterpret_cast<unsigned long long*>(base + o_delta);
-    p.barrier = reinterpret_cast<unsigned*>(base + o_bar);
-    {
+    if (rep) {
+        const size_t o_delta = off; off += tacg_align_up(sizeof(unsigned long long) * (size_t)p.L * (size_t)p.nmb * p.P, 256);
+        const size_t o_bar = off;   off += tacg_align_up(sizeof(unsigned) * (size_t)p.L, 256);
+        char* base = static_cast<char*>(tacg_scratch(ctx, off));
+        if (!base) return TACG_ERR_CUDA;
+        p.delta = reinterpret_cast<unsigned long long*>(base + o_delta);
+        p.barrier = reinterpret_cast<unsigned*>(base + o_bar);
+        p.partial = nullptr;
         const size_t ns = p.cpl > 1 ? off / sizeof(unsigned long long) : 0;
         const int zgrid = (int)max((size_t)1, min((size_t)ctx->sm_count, (ns + 1023) / 1024));
         TACG_CUDA_TRY(ctx, tacg_launch_pdl(eval_zero_kernel, dim3(zgrid), dim3(1024), 0, ctx->stream, p.comm_span,
                                            (size_t)p.L * p.F, p.comm_remote, (size_t)p.L * p.F, p.load, (size_t)p.L * p.P,
                                            p.ntok, (size_t)p.F, reinterpret_cast<unsigned long long*>(base), ns));
         TACG_LAUNCH_CHECK(ctx);
+    } else {
+        // every (layer, part) row is written by exactly one CTA, so nothing needs clearing
+        off = sizeof(unsigned long long) * (size_t)p.L * (size_t)p.cpl * (size_t)(p.P + 3 * p.F);
+        char* base = static_cast<char*>(tacg_scratch(ctx, off));
+        if (!base) return TACG_ERR_CUDA;
+        p.partial = reinterpret_cast<unsigned long long*>(base);
+        p.delta = nullptr; p.barrier = nullptr;
     }
     tacg_prof_scope prof(ctx, TACG_PROF_EVAL);
     if (waits) {
@@ -803,7 +832,6 @@ int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
         TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kEvalThreads), smem, ctx->stream, p));
         TACG_LAUNCH_CHECK(ctx);
     }
-    if (rep || p.cpl == 1) p.delta = nullptr;      // tells the caller that load and load_state are already final
     return TACG_OK;
 }
 
@@ -848,8 +876,8 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(load, 0, sizeof(uint64_t) * (size_t)L * P, ctx->stream));
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
     }
-    const unsigned long long* fin_delta = nullptr;   // set when the fairness kernel still has Eq. 15 to apply
-    int fin_nmb = 0;
+    const unsigned long long* fin_partial = nullptr;   // set when the fairness kernel still has the CTA rows to add
+    int fin_cpl = 0;
     if (N > 0) {
         EvalParams p;
         p.indices = indices; p.family = family; p.N = N; p.k = k; p.L = L; p.E = E; p.F = F; p.P = P; p.r = r;
@@ -865,7 +893,7 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         p.ntok = reinterpret_cast<unsigned long long*>(ntok);
         p.cost = cost_per_token;
         p.serve = reinterpret_cast<signed char*>(serve);
-        p.delta = nullptr; p.barrier = nullptr; p.cpl = 1; p.groups = 1;
+        p.delta = nullptr; p.barrier = nullptr; p.partial = nullptr; p.cpl = 1; p.groups = 1;
         int rc;
         switch (tacg_pick_kt(k, indices)) {
             case 2: rc = launch_eval_t<2>(ctx, p); break;
@@ -875,12 +903,14 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
             default: rc = launch_eval_t<0>(ctx, p); break;
         }
         if (rc != TACG_OK) return rc;
-        fin_delta = p.delta;
-        fin_nmb = (int)p.nmb;
+        fin_partial = p.partial;
+        fin_cpl = p.cpl;
     }
     TACG_CUDA_TRY(ctx, tacg_launch_pdl(fairness_kernel, dim3(L + 1), dim3(1024), 0, ctx->stream,
-                                       reinterpret_cast<unsigned long long*>(load), L, P, fairness,
-                                       (const unsigned long long*)fin_delta, fin_nmb, rho, load_state));
+                                       reinterpret_cast<unsigned long long*>(load), L, P, fairness, fin_partial, fin_cpl, F,
+                                       rho, load_state, reinterpret_cast<unsigned long long*>(comm_span),
+                                       reinterpret_cast<unsigned long long*>(comm_remote),
+                                       reinterpret_cast<unsigned long long*>(ntok)));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
