@@ -649,31 +649,24 @@ __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __re
                                                        unsigned long long* __restrict__ ntok) {
     tacg_pdl_prologue();
     __shared__ unsigned long long part[16][64];
+    __shared__ unsigned long long cpart[16][24];      // span | remote | tokens per family, F <= 8 each
     __shared__ double x[64];
     const int row = blockIdx.x;
     const int m = threadIdx.x & 63, q = threadIdx.x >> 6;
-    unsigned long long v = 0;
+    unsigned long long v = 0, csum = 0;
     if (partial) {
+        // thread (m, q) adds the CTA rows q, q+16, ...: no thread walks more than cpl/16 dependent loads
         const size_t W = (size_t)(P + 3 * F);
         if (row < L) {
             const unsigned long long* rows = partial + (size_t)row * cpl * W;
-            if (q == 0 && m < P) {
-                for (int c = 0; c < cpl; ++c) v += rows[(size_t)c * W + m];
-                load[(size_t)row * P + m] = v;
-                if (load_state) {
-                    const double Ls = load_state[(size_t)row * P + m];
-                    load_state[(size_t)row * P + m] = __dadd_rn(__dmul_rn(rho, Ls), (double)v);   // no FMA (Q19)
-                }
-            } else if (q >= 1 && q <= 3 && m < F && (q < 3 || row == 0)) {
-                unsigned long long t = 0;
-                for (int c = 0; c < cpl; ++c) t += rows[(size_t)c * W + P + (size_t)(q - 1) * F + m];
-                if (q == 1) comm_span[(size_t)row * F + m] = t;
-                else if (q == 2) comm_remote[(size_t)row * F + m] = t;
-                else ntok[m] = t;
+            for (int c = q; c < cpl; c += 16) {
+                if (m < P) v += rows[(size_t)c * W + m];
+                if (m < 3 * F) csum += rows[(size_t)c * W + P + m];
             }
         } else if (m < P) {
             for (long long i = q; i < (long long)L * cpl; i += 16) v += partial[(size_t)i * W + m];
         }
+        if (m < 24) cpart[q][m] = csum;
     } else if (m < P) {
         if (row < L) { if (q == 0) v = load[(size_t)row * P + m]; }
         else for (int l = q; l < L; l += 16) v += load[(size_t)l * P + m];
@@ -685,6 +678,21 @@ __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __re
 #pragma unroll
         for (int z = 0; z < 16; ++z) t += part[z][m];
         x[m] = (double)t;
+        if (partial && row < L && m < P) {
+            load[(size_t)row * P + m] = t;
+            if (load_state) {
+                const double Ls = load_state[(size_t)row * P + m];
+                load_state[(size_t)row * P + m] = __dadd_rn(__dmul_rn(rho, Ls), (double)t);   // no FMA (Q19)
+            }
+        }
+    } else if (q == 1 && partial && row < L && m < 3 * F) {
+        unsigned long long t = 0;
+#pragma unroll
+        for (int z = 0; z < 16; ++z) t += cpart[z][m];
+        const int which = m / F, f = m - which * F;
+        if (which == 0) comm_span[(size_t)row * F + f] = t;
+        else if (which == 1) comm_remote[(size_t)row * F + f] = t;
+        else if (row == 0) ntok[f] = t;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
