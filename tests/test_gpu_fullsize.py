@@ -1,11 +1,13 @@
-"""Parity at BASELINE.json's full per-layer sizes, in the launch configuration bench.py times
-(same flags, same micro-batch, traces generated on the device exactly as bench.py does).
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (same flags, same
+micro-batch, same L and N -- the library's grid split depends on both -- and traces generated on the
+device exactly as bench.py does).
 
-The C oracle finishes these in seconds, so every output is compared element by element:
-config 2 whole; configs 3 and 4 at the full token count per layer on a subset of layers (layers are
-independent problems, Q22, and the library's grid split changes with L, so two values of
-L are used for config 3); config 5 whole.  Invariants that hold at any size (north_star) are
-checked on the GPU result itself.
+The C oracle finishes every configuration in seconds to a minute, so every output is compared element by
+element on the WHOLE configuration ("Parity on configs 3-4 compares the full D, C, load,
+comm and serve outputs"): configs 2, 3, 4 and 5 at their full L and N on the path TACG_PATH_AUTO takes and
+in the evaluator with the GESR table, B = 65 536 and a load state.  Smaller L (layers are independent
+problems, Q22) is used only for the extra variants: the forced tensor path and the per-token
+outputs.  Invariants that hold at any size (north_star) are checked on the GPU result itself.
 """
 import numpy as np
 import pytest
@@ -57,8 +59,8 @@ def _check_invariants(cfg, N, D, C, ntok):
     assert (C.sum(axis=(2, 3), dtype=np.uint64) == (k * (k - 1) * ntok)[None, :]).all()
 
 
-@pytest.mark.parametrize("cfg_id,L,path", [(2, 26, "auto"), (3, 5, "auto"), (3, 2, "auto"), (4, 2, "auto"), (5, 1, "auto"),
-                                           (2, 26, "mma"), (3, 3, "mma"), (4, 2, "mma"), (5, 1, "mma")])
+@pytest.mark.parametrize("cfg_id,L,path", [(2, 26, "auto"), (3, 48, "auto"), (3, 2, "auto"), (4, 58, "auto"), (4, 2, "auto"),
+                                           (5, 1, "auto"), (2, 26, "mma"), (3, 3, "mma"), (4, 2, "mma"), (5, 1, "mma")])
 def test_coact_full_size(tacg, ctx, cfg_id, L, path):
     cfg, idx, fam = _device_trace(cfg_id, L, eval_trace=False)
     flag = tacg.TACG_PATH_MMA if path == "mma" else tacg.TACG_PATH_AUTO
@@ -72,24 +74,27 @@ def test_coact_full_size(tacg, ctx, cfg_id, L, path):
     assert (C == wC).all()
 
 
-@pytest.mark.parametrize("cfg_id,L", [(2, 26), (3, 4), (4, 2), (5, 1)])
-def test_eval_full_size(tacg, ctx, cfg_id, L):
+# want_cost = False is the launch bench.py times (no per-token output: another kernel instantiation)
+@pytest.mark.parametrize("cfg_id,L,want_cost", [(2, 26, True), (2, 26, False), (3, 48, False), (3, 4, True), (4, 58, False),
+                                                (4, 58, True), (4, 2, True), (5, 1, True), (5, 1, False)])
+def test_eval_full_size(tacg, ctx, cfg_id, L, want_cost):
     cfg, idx, fam = _device_trace(cfg_id, L, eval_trace=True)
     primary = tracegen.random_placement(cfg.E, cfg.P, cfg.capacity, cfg.L, seed=cfg.seed)
     replicas = tracegen.random_replicas(primary, cfg.P, cfg.r, cfg.n_rep, seed=cfg.seed + 1) if cfg.r else None
     st = torch.zeros((cfg.L, cfg.P), dtype=torch.float64, device="cuda")
     got = tacg.tacg_eval_placement(ctx, idx, fam, cfg.E, cfg.F, cfg.P, torch.from_numpy(primary).cuda(),
                                    None if replicas is None else torch.from_numpy(replicas).cuda(), theta=0.15,
-                                   rho=0.995, microbatch=cfg.microbatch, load_state=st, want_cost=True)
+                                   rho=0.995, microbatch=cfg.microbatch, load_state=st, want_cost=want_cost)
     torch.cuda.synchronize()
     want = cbind.eval_placement(idx.cpu().numpy(), fam.cpu().numpy(), cfg.E, cfg.F, cfg.P, primary, replicas,
                                 theta=0.15, rho=0.995, microbatch=cfg.microbatch,
-                                load_state=np.zeros((cfg.L, cfg.P)), want_cost=True)
+                                load_state=np.zeros((cfg.L, cfg.P)), want_cost=want_cost)
     assert (_u64(got["load"]) == want["load"]).all()
     assert (_u64(got["comm_span"]) == want["comm_span"]).all()
     assert (_u64(got["comm_remote"]) == want["comm_remote"]).all()
     assert (_u64(got["ntok"]) == want["ntok"]).all()
-    assert (got["cost"].cpu().numpy() == want["cost"]).all()
+    if want_cost:
+        assert (got["cost"].cpu().numpy() == want["cost"]).all()
     assert (st.cpu().numpy().view(np.uint64) == want["load_state"].view(np.uint64)).all()
     assert np.allclose(got["fairness"].cpu().numpy().astype(np.float64), want["fairness"], rtol=1e-5, atol=1e-7)
     # any size: every dispatch is served by exactly one partition; Jain in [1/P, 1]
