@@ -3,50 +3,112 @@
 // (Eq. 15, once per micro-batch per north_star / Q19) and fairness
 // (Eq. 17-18).
 //
-// eval_kernel is persistent: the grid is split into groups of `cpl` CTAs, one group per
-// layer (layers are independent problems, Q22).  Inside a layer the micro-batches are a
-// serial chain: every CTA of the group adds its integer dispatch counts of micro-batch b to
-// delta[l][b][:] in global memory, the group meets at a counter barrier, and each CTA then
-// applies Eq. 15 redundantly from the same integers (same fp64 operations => the same bits),
-// so no CTA ever reads another CTA's floating-point state.  The kernel is launched
-// cooperatively whenever CTAs wait on one another.
+// The evaluation is split where the data dependence is:
+//
+//   eval_scan_kernel   everything that does NOT depend on the load snapshot, at streaming speed and
+//                      without any wait: persistent CTAs walk items = (layer, micro-batch, slice of
+//                      <= 8192 tokens); per token the primary map is looked up in a 16-bit table, the
+//                      slots of experts without replicas are counted (lane-private shared-memory
+//                      counters, no branch) and, when the token has no replicated slot, its communication
+//                      cost is final.  A token WITH replicated slots leaves one 12-byte record (accessed
+//                      set so far | the rank of the replicated expert in each slot | home, family,
+//                      offset).  Every item writes one row of partial sums
+//                      (loads | span | remote | tokens per family | records).
+//   eval_chain_kernel  the serial part (replicas only): one thread-block cluster per layer walks the
+//                      micro-batches in order: snapshot -> guard -> sorted candidate tables of the
+//                      replicated experts -> the records of the micro-batch (each pending slot takes the
+//                      first local candidate of its table, else the first) -> integer dispatch counts,
+//                      exchanged over distributed shared memory with one cluster barrier per
+//                      micro-batch -> Eq. 15 applied redundantly by every CTA from the same integers
+//                      (same fp64 operations, same bits; no floating-point value crosses a CTA).
+//   fairness_kernel    S12; without replicas it first adds the rows of a layer (nothing depends on
+//                      the snapshot then, the whole trace is one micro-batch).
+//
+// No CTA ever spins on another launch-mate: the only waits are cluster barriers, and a cluster is
+// co-scheduled by the hardware.
 //
 // The pick rule of Q17 orders candidates by (not local, snapshot load, candidate slot).  Only the
 // first key depends on the token, so once per micro-batch each replicated expert's feasible
 // candidates are sorted by (snapshot load, slot) into a small table; a token then takes the first
 // entry that is local to it (in its accessed set R or its home), else the first entry.  That is
 // the same argmin, with all fp64 comparisons hoisted out of the token loop.
+//
+// Shapes outside the record format (k not in {2,4,6,8} or an unaligned trace, more than 15 replicated
+// experts in a layer) mark their items "overflow": the chain kernel then serves those tokens itself,
+// straight from the trace.
 #include <cooperative_groups.h>
+
+#include <algorithm>
 
 #include "tacg_common.cuh"
 
+namespace cg = cooperative_groups;
+
 namespace {
 
-constexpr int kEvalThreads = 512;
+constexpr int kEvalThreads = 512;    // eval_scan_kernel, select_kernel
 constexpr int kEvalBatch = 4;        // tokens per thread with their loads in flight together
+constexpr int kSlice = 8192;         // most tokens of a scan item (13-bit offsets in the records, 16 per thread)
+constexpr int kChainThreads = 1024;
 constexpr int kCandStride = 12;      // bytes per expert in the candidate table: [0] = count, [1..9] = partitions
 constexpr unsigned kRepFlag = 0x80u; // ptab bit: the expert has at least one replica
-constexpr int kDeferCap = 64;        // deferred tokens per warp (at most 31 left over + 32 pushed)
-constexpr int kDeferWords = 7;       // ids (<= 4 words), home | family << 8, token offset, pad; odd stride
+constexpr unsigned kBadFlag = 0x40u; // ptab bit: not an expert (empty slot, id outside [0,E))
+constexpr int kPtab = 516;           // ids are clamped to 512; entry 512 is "not an expert"
+constexpr int kSink = 64;            // counter row of the slots the scan kernel does not count
+constexpr int kMaxRank = 15;         // replicated experts per layer the 4-bit rank fields can name
+constexpr unsigned kT16Bad = 0x8000u;
+constexpr unsigned kOverflow = 0xffffffffu;   // record count of an item the chain kernel serves from the trace
 
 struct LayerTables {
-    unsigned char* ptab;   // [E] primary partition | kRepFlag
+    unsigned char* ptab;   // [kPtab] primary partition | kRepFlag, or kBadFlag
     unsigned char* cand;   // [E][kCandStride] sorted feasible candidates of replicated experts
     signed char* rep;      // [E*r] replica partitions as given, -1 = none
     double* S;             // [64] load snapshot
 };
 
-__device__ __forceinline__ void load_tables(int E, int r, const int8_t* __restrict__ pr,
-                                            const int8_t* __restrict__ rp, const LayerTables& T) {
-    for (int e = threadIdx.x; e < E; e += blockDim.x) {
-        unsigned n = 0;
-        for (int a = 0; a < r; ++a) {
-            const signed char c = rp[(size_t)e * r + a];
-            T.rep[e * r + a] = c;
-            n += (c >= 0) ? 1u : 0u;
+__device__ __forceinline__ void load_ptab(int E, int r, const int8_t* __restrict__ pr, const int8_t* __restrict__ rp,
+                                          unsigned char* ptab, signed char* rep) {
+    for (int e = threadIdx.x; e < kPtab; e += blockDim.x) {
+        unsigned v = kBadFlag;
+        if (e < E) {
+            unsigned n = 0;
+            for (int a = 0; a < r; ++a) {
+                const signed char c = rp[(size_t)e * r + a];
+                if (rep) rep[e * r + a] = c;
+                n += (c >= 0) ? 1u : 0u;
+            }
+            v = ((unsigned)pr[e] & 63u) | (n ? kRepFlag : 0u);
         }
-        T.ptab[e] = (unsigned char)(((unsigned)pr[e] & 63u) | (n ? kRepFlag : 0u));
+        ptab[e] = (unsigned char)v;
     }
+}
+
+// Ranks of the replicated experts of a layer: 1, 2, ... in increasing expert id (0 = not replicated).
+// Needs ptab complete (a barrier before); `wsum` is scratch for blockDim/32 words; ends with a barrier.
+// Returns the number of replicated experts.  rank8[e] is clipped to 255; replist[rank-1] = e (optional).
+__device__ __forceinline__ int build_ranks(int E, const unsigned char* ptab, unsigned char* rank8,
+                                           unsigned short* replist, unsigned* wsum) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nw = blockDim.x >> 5;
+    int base = 0;
+    for (int e0 = 0; e0 < E; e0 += blockDim.x) {
+        const int e = e0 + tid;
+        const bool isrep = e < E && (ptab[e] & kRepFlag);
+        const unsigned b = __ballot_sync(0xffffffffu, isrep);
+        if (lane == 0) wsum[warp] = __popc(b);
+        __syncthreads();
+        int before = base;
+        for (int q = 0; q < warp; ++q) before += (int)wsum[q];
+        int total = 0;
+        for (int q = 0; q < nw; ++q) total += (int)wsum[q];
+        if (e < E) {
+            const int rk = isrep ? before + __popc(b & ((1u << lane) - 1u)) + 1 : 0;
+            rank8[e] = (unsigned char)min(rk, 255);
+            if (isrep && replist) replist[rk - 1] = (unsigned short)e;
+        }
+        base += total;
+        __syncthreads();
+    }
+    return base;
 }
 
 // feas from a snapshot: mean summed left to right in double (Q19), theta widened from float.
@@ -61,136 +123,71 @@ __device__ __forceinline__ unsigned long long load_guard(const double* S, int P,
     return fm;
 }
 
-// Candidate table of one snapshot: for every replicated expert the candidates (primary, then
+// Candidate table entry of one replicated expert for one snapshot: the candidates (primary, then
 // replicas in slot order), restricted to the feasible ones unless none is (fallback,
 // PAPER.md:155), stably sorted by snapshot load (strict <, so ties keep slot order).
+// out: [0] = count, [1..count] = partitions, entries up to [3] repeat [1] (pick_first3 reads three).
+__device__ __forceinline__ void build_candidate(int e, int r, const LayerTables& T, unsigned long long feas,
+                                                unsigned char* out) {
+    const unsigned in = T.ptab[e];
+    int c[9];
+    int n = 0;
+    c[n++] = (int)(in & 63u);
+    for (int a = 0; a < r; ++a) {
+        const int v = T.rep[e * r + a];
+        if (v >= 0) c[n++] = v & 63;
+    }
+    unsigned long long cmask = 0ull;
+    for (int i = 0; i < n; ++i) cmask |= 1ull << c[i];
+    const bool anyfeas = (cmask & feas) != 0ull;
+    int m = 0;
+    for (int i = 0; i < n; ++i) {
+        if (anyfeas && !((feas >> c[i]) & 1ull)) continue;
+        // insertion: after every entry whose load is <= this one's
+        const double s = T.S[c[i]];
+        int pos = m;
+        while (pos > 0 && s < T.S[out[pos]]) { out[pos + 1] = out[pos]; --pos; }
+        out[pos + 1] = (unsigned char)c[i];
+        ++m;
+    }
+    out[0] = (unsigned char)m;
+    for (int i = m + 1; i <= 3; ++i) out[i] = out[1];
+}
+
 __device__ __forceinline__ void build_candidates(int E, int r, const LayerTables& T, unsigned long long feas) {
-    for (int e = threadIdx.x; e < E; e += blockDim.x) {
-        const unsigned in = T.ptab[e];
-        if (!(in & kRepFlag)) continue;
-        int c[9];
-        int n = 0;
-        c[n++] = (int)(in & 63u);
-        for (int a = 0; a < r; ++a) {
-            const int v = T.rep[e * r + a];
-            if (v >= 0) c[n++] = v & 63;
-        }
-        unsigned long long cmask = 0ull;
-        for (int i = 0; i < n; ++i) cmask |= 1ull << c[i];
-        const bool anyfeas = (cmask & feas) != 0ull;
-        int m = 0;
-        unsigned char* out = T.cand + e * kCandStride;
-        for (int i = 0; i < n; ++i) {
-            if (anyfeas && !((feas >> c[i]) & 1ull)) continue;
-            // insertion: after every entry whose load is <= this one's
-            const double s = T.S[c[i]];
-            int pos = m;
-            while (pos > 0 && s < T.S[out[pos]]) { out[pos + 1] = out[pos]; --pos; }
-            out[pos + 1] = (unsigned char)c[i];
-            ++m;
-        }
-        out[0] = (unsigned char)m;
-    }
+    for (int e = threadIdx.x; e < E; e += blockDim.x)
+        if (T.ptab[e] & kRepFlag) build_candidate(e, r, T, feas, T.cand + e * kCandStride);
 }
 
-// Pass 2 of the selection: replicated experts (bits of `pending`) in slot order; each takes the first
-// local candidate of its sorted table, else the first, and joins R.
-template <int KM, typename M>
-__device__ __forceinline__ M serve_pending(const int (&e)[KM], unsigned pending, int home, M R, const LayerTables& T,
-                                           int (&sv)[KM]) {
-    const M hb = (M)1 << home;
-    if constexpr (KM <= 8) {
-        // Each lane walks its own set bits (lowest first = slot order), so a warp runs for the
-        // largest number of replicated slots any of its tokens has, not for all KM slots.
-        unsigned long long picks = 0ull;
-        unsigned todo = pending;
-        while (todo) {
-            const int j = __ffs(todo) - 1;
-            todo &= todo - 1u;
-            int ex = e[0];
-#pragma unroll
-            for (int q = 1; q < KM; ++q) ex = (j == q) ? e[q] : ex;
-            const unsigned char* c = T.cand + ex * kCandStride;
-            const int n = c[0];
-            int pick = c[1];
-            const M loc = R | hb;
-            for (int i = 1; i <= n; ++i) {
-                const int v = c[i];
-                if ((loc >> v) & (M)1) { pick = v; break; }
-            }
-            picks |= (unsigned long long)pick << (8 * j);
-            R |= (M)1 << pick;
-        }
-#pragma unroll
-        for (int j = 0; j < KM; ++j)
-            if ((pending >> j) & 1u) sv[j] = (int)((picks >> (8 * j)) & 0xffull);
-    } else {
-#pragma unroll
-        for (int j = 0; j < KM; ++j) {
-            if (!((pending >> j) & 1u)) continue;
-            const unsigned char* c = T.cand + e[j] * kCandStride;
-            const int n = c[0];
-            int pick = c[1];
-            const M loc = R | hb;
-            for (int i = 1; i <= n; ++i) {
-                const int v = c[i];
-                if ((loc >> v) & (M)1) { pick = v; break; }
-            }
-            sv[j] = pick;
-            R |= (M)1 << pick;
-        }
+// One pending (replicated) slot: the first candidate of the expert's sorted table that is local to the
+// token (in R or its home), else the first.
+template <typename M>
+__device__ __forceinline__ int pick_candidate(const unsigned char* __restrict__ c, M loc) {
+    const int n = c[0];
+    int pick = c[1];
+    for (int i = 1; i <= n; ++i) {
+        const int v = c[i];
+        if ((loc >> v) & (M)1) { pick = v; break; }
     }
-    return R;
+    return pick;
 }
 
-// Pass 2 on packed serve bytes (KM <= 8): svp byte j = serving partition of slot j.
-template <int KM, typename M>
-__device__ __forceinline__ M serve_pending_packed(const int (&e)[KM], unsigned pending, int home, M R,
-                                                  const LayerTables& T, unsigned long long& svp) {
-    const M hb = (M)1 << home;
-    unsigned todo = pending;
-    while (todo) {
-        const int j = __ffs(todo) - 1;
-        todo &= todo - 1u;
-        int ex = e[0];
-#pragma unroll
-        for (int q = 1; q < KM; ++q) ex = (j == q) ? e[q] : ex;
-        const unsigned char* c = T.cand + ex * kCandStride;
-        const int n = c[0];
-        int pick = c[1];
-        const M loc = R | hb;
-        for (int i = 1; i <= n; ++i) {
+// The same pick on the table's first word (count | c1 | c2 | c3, entries beyond the count repeat c1): no loop
+// unless more than three candidates are listed and none of the first three is local.
+template <typename M>
+__device__ __forceinline__ int pick_first3(const unsigned char* __restrict__ c, M loc) {
+    const unsigned w0 = *reinterpret_cast<const unsigned*>(c);
+    const unsigned c1 = (w0 >> 8) & 0xffu, c2 = (w0 >> 16) & 0xffu, c3 = w0 >> 24;
+    const bool l1 = (loc >> c1) & (M)1, l2 = (loc >> c2) & (M)1, l3 = (loc >> c3) & (M)1;
+    int pick = l1 ? (int)c1 : (l2 ? (int)c2 : (l3 ? (int)c3 : (int)c1));
+    if (!(l1 | l2 | l3) && (w0 & 0xffu) > 3u) {
+        const int n = (int)(w0 & 0xffu);
+        for (int i = 4; i <= n; ++i) {
             const int v = c[i];
             if ((loc >> v) & (M)1) { pick = v; break; }
         }
-        svp = (svp & ~(0xffull << (8 * j))) | ((unsigned long long)pick << (8 * j));
-        R |= (M)1 << pick;
     }
-    return R;
-}
-
-// All KM slots hold valid ids: pass 1 without branches.
-template <int KM, bool REP, typename M>
-__device__ __forceinline__ M serve_fast(const int (&e)[KM], int home, const LayerTables& T, int (&sv)[KM]) {
-    M R = 0;
-    unsigned pending = 0u;
-#pragma unroll
-    for (int j = 0; j < KM; ++j) {
-        const unsigned in = T.ptab[e[j]];
-        if constexpr (REP) {
-            const unsigned isrep = in >> 7;
-            sv[j] = (int)(in & 63u);
-            R |= (M)(isrep ^ 1u) << (in & 63u);
-            pending |= isrep << j;
-        } else {
-            sv[j] = (int)in;
-            R |= (M)1 << in;
-        }
-    }
-    if constexpr (REP) {
-        if (pending) R = serve_pending<KM, M>(e, pending, home, R, T, sv);
-    }
-    return R;
+    return pick;
 }
 
 // Step 4 of O10 for one token: serve[j] per slot (-1 = empty), returns the accessed set R.
@@ -213,423 +210,661 @@ __device__ __forceinline__ M serve_token(const int (&e)[KM], int k, int E, int h
             }
         }
     }
-    // pass 2: replicated experts in slot order; first local candidate of the sorted table, else the first
-    if (pending) {
-        R = serve_pending<KM, M>(e, pending, home, R, T, sv);
+    // pass 2: replicated experts in slot order
+    const M hb = (M)1 << home;
+#pragma unroll
+    for (int j = 0; j < KM; ++j) {
+        if (!((pending >> j) & 1u)) continue;
+        const int pick = pick_candidate<M>(T.cand + e[j] * kCandStride, R | hb);
+        sv[j] = pick;
+        R |= (M)1 << pick;
     }
     return R;
 }
 
-struct EvalParams {
-    const int16_t* indices;
-    const int8_t* family;
-    long long N;
+// ---- geometry shared by the scan and the chain kernels
+struct EvalGeom {
+    long long N, B, nmb, token_offset;
+    long long ipl;      // items per layer = nmb * spm
+    int spm;            // slices per micro-batch
+    int slice;          // tokens per slice: a multiple of 512, <= kSlice
+    int W;              // 32-bit words per row: P loads | F span | F remote | F tokens per family | records with one
+                        // pending slot | records with several
     int k, L, E, F, P, r;
-    const int8_t* primary;
-    const int8_t* replicas;
-    float theta;
-    double rho;
-    long long B;            // micro-batch size (tokens)
-    long long nmb;          // number of micro-batches
-    long long token_offset;
-    double* load_state;     // [L,P] in/out or null
-    unsigned long long* load;          // [L,P] out
-    unsigned long long* comm_span;     // [L,F] out (zeroed before launch, reduced atomically)
-    unsigned long long* comm_remote;   // [L,F]
-    unsigned long long* ntok;          // [F] out (zeroed before launch; counted by the CTAs of layer 0)
-    unsigned char* cost;    // [L,N] or null
-    signed char* serve;     // [L,N,k] or null
-    unsigned long long* delta;   // scratch [L,nmb,P], zeroed before launch (only used when cpl > 1)
-    unsigned* barrier;           // scratch [L], zeroed before launch
-    unsigned long long* partial; // scratch [L,cpl,P+3F] (no-replica path): per-CTA loads | span | remote | tokens per family
-    int cpl;                // CTAs per layer
-    int groups;             // number of concurrent layer groups = gridDim.x / cpl
 };
 
-__host__ __device__ inline size_t eval_align16(size_t x) { return (x + 15) & ~(size_t)15; }
-
-// carves the per-layer tables out of dynamic shared memory; returns the bytes used
-__device__ __forceinline__ size_t carve_tables(unsigned char* base, int E, int r, LayerTables& T) {
-    size_t off = 0;
-    T.S = reinterpret_cast<double*>(base + off);            off += 64 * sizeof(double);
-    T.ptab = base + off;                                    off += eval_align16((size_t)E);
-    T.cand = base + off;                                    off += eval_align16((size_t)E * kCandStride);
-    T.rep = reinterpret_cast<signed char*>(base + off);     off += eval_align16((size_t)E * (r > 0 ? r : 1));
-    return off;
+__device__ __forceinline__ void item_tokens(const EvalGeom& g, long long mb, int s, long long& t0, long long& t1) {
+    t0 = mb * g.B + (long long)s * g.slice;
+    const long long e = min(g.N, (mb + 1) * g.B);
+    t1 = min(e, t0 + g.slice);
+    if (t1 < t0) t1 = t0;
 }
 
-size_t tables_bytes(int E, int r) {
-    return 64 * sizeof(double) + eval_align16((size_t)E) + eval_align16((size_t)E * kCandStride) +
-           eval_align16((size_t)E * (r > 0 ? r : 1));
+// Records of the deferred tokens of an item, three parallel arrays of g.slice entries per item (tokens with
+// one pending slot from entry 0 upwards, tokens with several from the last entry downwards):
+//   set   M          accessed set after pass 1 (partitions of the slots without replicas)
+//   rank  unsigned   4 bits per slot: rank of the replicated expert in that slot, 0 = not pending
+//   meta  unsigned   offset in the item (13) | family (3) | home (6)
+struct RecArrays {
+    void* set;
+    unsigned* rank;
+    unsigned* meta;
+};
+
+// 1 << s with PTX semantics: a shift count >= the register width gives 0 (the sink row 64 is no partition)
+template <typename M> __device__ __forceinline__ M bit_or_zero(unsigned s);
+template <> __device__ __forceinline__ unsigned bit_or_zero<unsigned>(unsigned s) {
+    unsigned r;
+    asm("shl.b32 %0, 1, %1;" : "=r"(r) : "r"(s));
+    return r;
+}
+template <> __device__ __forceinline__ unsigned long long bit_or_zero<unsigned long long>(unsigned s) {
+    unsigned long long r;
+    asm("shl.b64 %0, 1, %1;" : "=l"(r) : "r"(s));
+    return r;
 }
 
-template <int KT>
-__device__ __forceinline__ void unpack_ids(const unsigned (&w)[KT / 2], int (&e)[KT]) {
-#pragma unroll
-    for (int i = 0; i < KT / 2; ++i) {
-        e[2 * i] = (int)(short)(w[i] & 0xffffu);
-        e[2 * i + 1] = (int)w[i] >> 16;
-    }
+// shared-memory accesses by 32-bit shared-space address (no generic-address arithmetic in the token loop)
+__device__ __forceinline__ unsigned saddr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sred_inc(unsigned a) { asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(a) : "memory"); }
+__device__ __forceinline__ void sred_add(unsigned a, unsigned v) {
+    asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned slds_u32(unsigned a) {
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ unsigned slds_u16(unsigned a) {
+    unsigned short v;
+    asm("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
+    return (unsigned)v;
 }
 
-template <int KT>
-__device__ __forceinline__ void load_row_raw(const int16_t* __restrict__ row, unsigned (&w)[KT / 2]) {
-    if constexpr (KT == 8) {
-        const uint4 v = __ldg(reinterpret_cast<const uint4*>(row));
-        w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
-    } else if constexpr (KT == 4) {
-        const uint2 v = __ldg(reinterpret_cast<const uint2*>(row));
-        w[0] = v.x; w[1] = v.y;
-    } else {
-#pragma unroll
-        for (int i = 0; i < KT / 2; ++i) w[i] = __ldg(reinterpret_cast<const unsigned*>(row) + i);
-    }
-}
+struct ScanParams {
+    EvalGeom g;
+    const int16_t* indices;
+    const int8_t* family;
+    const int8_t* primary;
+    const int8_t* replicas;   // null: no replicas
+    unsigned* rows;           // [L*ipl][W]
+    RecArrays rec;            // [L*ipl][slice] each (replicas only)
+    unsigned char* cost;      // [L,N] or null
+    signed char* serve;       // [L,N,k] or null
+};
+
+template <typename M> __device__ __forceinline__ int popc_m(M x);
+template <> __device__ __forceinline__ int popc_m<unsigned>(unsigned x) { return __popc(x); }
+template <> __device__ __forceinline__ int popc_m<unsigned long long>(unsigned long long x) { return __popcll(x); }
 
 // KT: compile-time k (0 = generic), REP: a replica table is present, M: partition-set mask type
-// (unsigned for P <= 32, else unsigned long long).
-// OUT: per-token outputs (cost_per_token / serve) were requested.
+// (unsigned for P <= 32, else unsigned long long), OUT: per-token outputs were requested.
 template <int KT, bool REP, typename M, bool OUT>
-__global__ void __launch_bounds__(kEvalThreads, 2)
-eval_kernel(EvalParams p) {
+__global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanParams p) {
     tacg_pdl_prologue();
-    extern __shared__ __align__(16) unsigned char esm[];
     constexpr int KM = KT > 0 ? KT : 16;
+    constexpr int NW = KT > 0 ? KT / 2 : 1;
     constexpr int U = KT > 0 ? kEvalBatch : 1;
-    LayerTables T;
-    size_t off = carve_tables(esm, p.E, p.r, T);
-    unsigned long long* dsum = reinterpret_cast<unsigned long long*>(esm + off);   off += 64 * sizeof(unsigned long long);
-    unsigned* cnt = reinterpret_cast<unsigned*>(esm + off);                        // [P][32], lane-private columns
-    off += sizeof(unsigned) * (size_t)p.P * 32;
-    // deferred-token queue of each warp (replicated slots are resolved 32 tokens at a time)
-    constexpr bool kQueued = REP && KT > 0 && sizeof(M) == 4;
-    unsigned* wqueue = reinterpret_cast<unsigned*>(esm + off) + (threadIdx.x >> 5) * (kDeferCap * kDeferWords);
-    if (kQueued) off += sizeof(unsigned) * (size_t)(kEvalThreads / 32) * kDeferCap * kDeferWords;
-    // per-family packed accumulators, one word per (warp, family, lane): a token is one shared atomic on its own
-    // thread's word instead of a compare-select-add per family
-    unsigned* acc = reinterpret_cast<unsigned*>(esm + off) + (threadIdx.x >> 5) * (8 * 32) + (threadIdx.x & 31);
-    __shared__ double Ls[64];              // EMA state of this layer
-    __shared__ unsigned long long ltot[64];  // cumulative integer load of this layer
-    __shared__ unsigned long long feas_s;
-    __shared__ unsigned long long comm_s[16];
-    __shared__ unsigned fam_s[8];          // tokens per family seen by this CTA (layer 0 only)
+    constexpr bool RECS = REP && KT > 0;      // the record format covers compile-time k only
+    extern __shared__ __align__(16) unsigned char esm[];
+    unsigned* cnt = reinterpret_cast<unsigned*>(esm);                      // [65][32]: lane-private columns, row 64 = sink
+    unsigned* accb = cnt + (kSink + 1) * 32;                               // [warps][8][32] per-thread family words
+    __shared__ unsigned char ptab[kPtab];
+    __shared__ unsigned char rank8[kPtab];
+    __shared__ unsigned short tab16[kPtab];   // row (7) | rank << 8 | kT16Bad
+    __shared__ unsigned comm_s[16];           // span[8] | remote[8] of this item
+    __shared__ unsigned fam_s[8];
+    __shared__ unsigned wsum[kEvalThreads / 32 + 1];
+    __shared__ unsigned nrec_s;
 
-    const int group = blockIdx.x / p.cpl;
-    const int part = blockIdx.x % p.cpl;
-    if (group >= p.groups) return;
+    const EvalGeom& g = p.g;
     const int tid = threadIdx.x, lane = tid & 31;
-    const int P = p.P, k = KT > 0 ? KT : p.k, E = p.E, F = p.F, r = REP ? p.r : 0;
+    const int P = g.P, k = KT > 0 ? KT : g.k, E = g.E, F = g.F;
+    const long long T = (long long)g.L * g.ipl;
+    const long long lo = (long long)blockIdx.x * T / gridDim.x, hi = (long long)(blockIdx.x + 1) * T / gridDim.x;
+    const unsigned cl = saddr(cnt + lane);                                  // this lane's counter column
+    unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;                    // this thread's family words
+    const unsigned al = saddr(acc);
+    const unsigned tb = saddr(tab16);
     const int stepP = kEvalThreads % P;
-    unsigned* cnt_lane = cnt + lane;
 
-    for (int layer = group; layer < p.L; layer += p.groups) {
+    for (int i = tid; i < (kSink + 1) * 32; i += kEvalThreads) cnt[i] = 0u;
+#pragma unroll
+    for (int f = 0; f < 8; ++f) acc[f * 32] = 0u;
+    int cur_layer = -1;
+    bool layer_ovf = REP && !RECS;           // this layer's items are left to the chain kernel
+    // (layer, micro-batch, slice) of the first item by division, of the following ones by counting
+    int layer = (int)(lo / g.ipl);
+    long long mb = (lo - (long long)layer * g.ipl) / g.spm;
+    int sl = (int)(lo - (long long)layer * g.ipl - mb * g.spm);
+    int hm0 = (int)((g.token_offset + mb * g.B + (long long)sl * g.slice) % P);   // home of the item's first token
+    const int hstep = g.slice % P;
+    for (long long item = lo; item < hi; ++item) {
+        __syncthreads();                    // the previous item's row is written
+        if (layer != cur_layer) {
+            load_ptab(E, REP ? g.r : 0, p.primary + (size_t)layer * E,
+                      REP ? p.replicas + (size_t)layer * E * g.r : nullptr, ptab, nullptr);
+            __syncthreads();
+            int nrep = 0;
+            if constexpr (REP) nrep = build_ranks(E, ptab, rank8, nullptr, wsum);
+            layer_ovf = REP && (!RECS || nrep > kMaxRank);
+            for (int e = tid; e < kPtab; e += kEvalThreads) {
+                const unsigned v = ptab[e];
+                unsigned t16;
+                if (v & kBadFlag) t16 = kSink | kT16Bad;
+                else if (v & kRepFlag) t16 = kSink | ((REP ? (unsigned)rank8[e] & 15u : 0u) << 8);
+                else t16 = v & 63u;
+                tab16[e] = (unsigned short)t16;
+            }
+            cur_layer = layer;
+        }
+        if (tid < 16) comm_s[tid] = 0u;
+        if (tid < 8) fam_s[tid] = 0u;
+        if (tid == 0) nrec_s = 0u;
         __syncthreads();
-        load_tables(E, r, p.primary + (size_t)layer * E, REP ? p.replicas + (size_t)layer * E * r : nullptr, T);
-        for (int i = tid; i < P * 32; i += kEvalThreads) cnt[i] = 0u;
+        long long t0, t1;
+        item_tokens(g, mb, sl, t0, t1);
+        const int n = (int)(t1 - t0);
+        const int16_t* base = p.indices + (size_t)layer * (size_t)g.N * (size_t)k;
+        unsigned char* cost_l = (OUT && p.cost) ? p.cost + (size_t)layer * g.N + t0 : nullptr;
+        signed char* serve_l = (OUT && p.serve) ? p.serve + ((size_t)layer * g.N + t0) * k : nullptr;
+        M* rec_set = RECS ? reinterpret_cast<M*>(p.rec.set) + (size_t)item * g.slice : nullptr;
+        unsigned* rec_rank = RECS ? p.rec.rank + (size_t)item * g.slice : nullptr;
+        unsigned* rec_meta = RECS ? p.rec.meta + (size_t)item * g.slice : nullptr;
+        int home = (hm0 + tid) % P;
+        const int8_t* fam0 = p.family + t0;
+        const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
+
+        for (int ob = tid; ob < n + tid; ob += kEvalThreads * U) {      // uniform trip count across the CTA
+            int f[U];
+            unsigned w[U][NW];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int o = ob + u * kEvalThreads;
+                f[u] = -1;
+                if (o < n) {
+                    f[u] = fam0[o];
+                    if constexpr (KT == 8) {
+                        const uint4 v = __ldg(reinterpret_cast<const uint4*>(rows0) + o);
+                        w[u][0] = v.x; w[u][1] = v.y; w[u][2] = v.z; w[u][3] = v.w;
+                    } else if constexpr (KT == 4) {
+                        const uint2 v = __ldg(reinterpret_cast<const uint2*>(rows0) + o);
+                        w[u][0] = v.x; w[u][1] = v.y;
+                    } else if constexpr (KT > 0) {
+                        const unsigned* rp = rows0 + (size_t)o * NW;
+#pragma unroll
+                        for (int i = 0; i < NW; ++i) w[u][i] = __ldg(rp + i);
+                    }
+                }
+            }
+            M dR[U];                 // accessed set of a deferred token
+            unsigned drank[U];       // ranks of its pending slots (0 = the token is not deferred)
+            unsigned dmeta[U];
+            bool dmulti[U];          // more than one pending slot
+            int ndef = 0;            // this lane's deferred tokens of the batch: one pending slot | several << 16
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int o = ob + u * kEvalThreads;
+                const bool live = (unsigned)f[u] < (unsigned)F;
+                drank[u] = 0u;
+                dmeta[u] = 0u;
+                dmulti[u] = false;
+                dR[u] = 0;
+                if (live) {
+                    unsigned a2[KM];            // byte offsets into tab16
+                    if constexpr (KT > 0) {
+                        unsigned orw = 0u;
+#pragma unroll
+                        for (int i = 0; i < NW; ++i) {
+                            a2[2 * i] = (w[u][i] << 1) & 0x1fffeu;
+                            a2[2 * i + 1] = (w[u][i] >> 15) & 0x1fffeu;
+                            orw |= w[u][i];
+                        }
+                        if (orw & 0xfe00fe00u) {       // an id outside [0,512): clamp to the "not an expert" entry
+#pragma unroll
+                            for (int j = 0; j < KM; ++j) a2[j] = min(a2[j], 1024u);
+                        }
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            a2[j] = (j < k) ? 2u * min((unsigned)(unsigned short)__ldg(base + ((size_t)t0 + o) * k + j), 512u) : 1024u;
+                    }
+                    // all table lookups first, then no branch: a slot that is not a plain expert has row 64, which
+                    // shifts to an empty mask and counts into the sink row
+                    unsigned t[KM];
+#pragma unroll
+                    for (int j = 0; j < KM; ++j) t[j] = slds_u16(tb + a2[j]);
+                    M R = 0;
+                    unsigned ranks = 0u;
+#pragma unroll
+                    for (int j = 0; j < KM; ++j) {
+                        const unsigned row = t[j] & 0x7fu;
+                        R |= bit_or_zero<M>(row);
+                        sred_inc(cl + row * 128u);
+                        if (RECS && j < 8) ranks |= ((t[j] >> 8) & 15u) << (4 * j);
+                    }
+                    if constexpr (OUT) {
+                        if (serve_l) {
+                            signed char* out = serve_l + (size_t)o * k;
+#pragma unroll
+                            for (int j = 0; j < KM; ++j)
+                                if (j < k) out[j] = (t[j] & kT16Bad) ? (signed char)-1 : (signed char)(t[j] & 0x3fu);
+                        }
+                    }
+                    unsigned packed = 1u << 22;          // one token of family f
+                    if (!RECS || ranks == 0u) {
+                        const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~((M)1 << home));
+                        packed |= (unsigned)max(0, nR - 1) | ((unsigned)rem << 11);
+                        if (OUT && cost_l) cost_l[o] = (unsigned char)rem;
+                    } else {
+                        dR[u] = R;
+                        drank[u] = ranks;
+                        dmeta[u] = (unsigned)o | ((unsigned)f[u] << 13) | ((unsigned)home << 16);
+                        const unsigned nz = (ranks | (ranks >> 1) | (ranks >> 2) | (ranks >> 3)) & 0x11111111u;
+                        dmulti[u] = (nz & (nz - 1u)) != 0u;
+                        ndef += dmulti[u] ? 0x10000 : 1;
+                    }
+                    sred_add(al + (unsigned)f[u] * 128u, packed);
+                } else if (o < n) {
+                    if (OUT && cost_l) cost_l[o] = 0;
+                    if (OUT && serve_l)
+                        for (int j = 0; j < k; ++j) serve_l[(size_t)o * k + j] = -1;
+                }
+                if (stepP) {
+                    home += stepP;
+                    if (home >= P) home -= P;
+                }
+            }
+            if constexpr (RECS) {
+                // records of this batch: one warp-wide reservation (tokens with one pending slot | with several, 16 bits
+                // each: an item has at most 8192 tokens), then every lane writes its own
+                if (__any_sync(0xffffffffu, ndef != 0)) {
+                    int inc = ndef;
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) {
+                        const int v = __shfl_up_sync(0xffffffffu, inc, d);
+                        if (lane >= d) inc += v;
+                    }
+                    const int total = __shfl_sync(0xffffffffu, inc, 31);
+                    unsigned wbase = 0u;
+                    if (lane == 31) wbase = atomicAdd(&nrec_s, (unsigned)total);
+                    wbase = __shfl_sync(0xffffffffu, wbase, 31);
+                    const unsigned mine = wbase + (unsigned)(inc - ndef);
+                    unsigned pos1 = mine & 0xffffu;                               // singles: upwards from entry 0
+                    unsigned pos2 = (unsigned)g.slice - 1u - (mine >> 16);        // several: downwards from the last entry
+#pragma unroll
+                    for (int u = 0; u < U; ++u) {
+                        if (drank[u]) {
+                            const unsigned pos = dmulti[u] ? pos2-- : pos1++;
+                            rec_set[pos] = dR[u];
+                            rec_rank[pos] = drank[u];
+                            rec_meta[pos] = dmeta[u];
+                        }
+                    }
+                }
+            }
+        }
+        // item epilogue: per-family sums of this thread -> CTA, per-partition columns -> row
+#pragma unroll
+        for (int fq = 0; fq < 8; ++fq) {
+            if (fq < F) {
+                const unsigned av = acc[fq * 32];
+                acc[fq * 32] = 0u;
+                const unsigned s = __reduce_add_sync(0xffffffffu, av & 0x7ffu);
+                const unsigned q = __reduce_add_sync(0xffffffffu, (av >> 11) & 0x7ffu);
+                const unsigned c = __reduce_add_sync(0xffffffffu, av >> 22);
+                if (lane == 0) {
+                    if (s) atomicAdd(&comm_s[fq], s);
+                    if (q) atomicAdd(&comm_s[8 + fq], q);
+                    if (c) atomicAdd(&fam_s[fq], c);
+                }
+            }
+        }
+        __syncthreads();
+        unsigned* row = p.rows + (size_t)item * g.W;
+        for (int m = tid >> 5; m < P; m += kEvalThreads / 32) {
+            const unsigned s = __reduce_add_sync(0xffffffffu, cnt[m * 32 + lane]);
+            cnt[m * 32 + lane] = 0u;
+            if (lane == 0) row[m] = layer_ovf ? 0u : s;     // overflow: everything but the token counts is redone later
+        }
+        if (tid < F) {
+            row[P + tid] = layer_ovf ? 0u : comm_s[tid];
+            row[P + F + tid] = layer_ovf ? 0u : comm_s[8 + tid];
+            row[P + 2 * F + tid] = fam_s[tid];
+        }
+        if (tid == 0) {
+            row[P + 3 * F] = layer_ovf ? kOverflow : (nrec_s & 0xffffu);
+            row[P + 3 * F + 1] = layer_ovf ? 0u : (nrec_s >> 16);
+        }
+        // next item
+        hm0 += hstep;
+        if (hm0 >= P) hm0 -= P;
+        if (++sl == g.spm) {
+            sl = 0;
+            if (++mb == g.nmb) { mb = 0; ++layer; }
+            hm0 = (int)((g.token_offset + mb * g.B) % P);
+        }
+    }
+}
+
+struct ChainParams {
+    EvalGeom g;
+    const int16_t* indices;
+    const int8_t* family;
+    const int8_t* primary;
+    const int8_t* replicas;
+    const unsigned* rows;
+    RecArrays rec;
+    float theta;
+    double rho;
+    double* load_state;                // [L,P] in/out or null
+    unsigned long long* load;          // [L,P] out
+    unsigned long long* comm_span;     // [L,F] out
+    unsigned long long* comm_remote;   // [L,F] out
+    unsigned long long* ntok;          // [F] out
+    unsigned char* cost;
+    signed char* serve;
+    int groups;                        // clusters in the grid; cluster c owns layers c, c + groups, ...
+};
+
+// One cluster of CS CTAs per layer (CLUSTER = false: a plain CTA).  CTA `rank` takes the rank-th share of every
+// item's records; the integer dispatch counts of a micro-batch are exchanged through distributed shared
+// memory (two alternating buffers, one cluster barrier per micro-batch).
+template <typename M, bool OUT, bool CLUSTER>
+__global__ void __launch_bounds__(kChainThreads, 1) eval_chain_kernel(const ChainParams p) {
+    tacg_pdl_prologue();
+    extern __shared__ __align__(16) unsigned char csm[];
+    const EvalGeom& g = p.g;
+    const int P = g.P, E = g.E, F = g.F, r = g.r, k = g.k;
+    LayerTables T;
+    size_t off = 0;
+    T.S = reinterpret_cast<double*>(csm + off);            off += 64 * sizeof(double);
+    T.cand = csm + off;                                    off += ((size_t)E * kCandStride + 15) & ~(size_t)15;
+    T.rep = reinterpret_cast<signed char*>(csm + off);     off += ((size_t)E * r + 15) & ~(size_t)15;
+    unsigned* cnt = reinterpret_cast<unsigned*>(csm + off);   off += sizeof(unsigned) * (size_t)P * 32;
+    unsigned* accb = reinterpret_cast<unsigned*>(csm + off);  off += sizeof(unsigned) * (kChainThreads / 32) * 8 * 32;
+    unsigned short* replist = reinterpret_cast<unsigned short*>(csm + off);   // [E] ids of the replicated experts
+    __shared__ unsigned char ptab_s[kPtab];
+    __shared__ unsigned char rank8[kPtab];
+    __shared__ __align__(16) unsigned char candr[(kMaxRank + 1) * kCandStride];   // candidate tables by rank
+    __shared__ double Ls[64];                  // EMA state of this layer
+    __shared__ unsigned long long ltot[64];    // cumulative integer load of this layer
+    __shared__ unsigned long long csum[24];    // span | remote | tokens per family: rows of the scan kernel
+    __shared__ unsigned long long dsum[16];    // span | remote of the deferred tokens handled by THIS CTA
+    __shared__ unsigned exch[2][64];           // this CTA's dispatch counts of the micro-batch (even / odd)
+    __shared__ unsigned wsum[kChainThreads / 32 + 1];
+    __shared__ unsigned long long feas_s;
+    __shared__ __align__(16) unsigned long long candm[(kMaxRank + 1) * 4];   // by rank: one-hot masks (type M) of the first four candidates
+    __shared__ unsigned bigq_s;                                 // ranks that list more than four candidates
+    __shared__ unsigned pre1[33], pre2[33];                     // records of up to 32 slices, prefix sums
+    __shared__ unsigned nrec1[32], nrec2[32];                   // records per slice (one pending slot | several)
+    __shared__ unsigned ovf_s[32];
+    T.ptab = ptab_s;
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    int rank = 0, CS = 1;
+    if constexpr (CLUSTER) {
+        cg::cluster_group cgl = cg::this_cluster();
+        rank = (int)cgl.block_rank();
+        CS = (int)cgl.num_blocks();
+    }
+    const int cluster_id = blockIdx.x / CS;
+    const unsigned cl = saddr(cnt + lane);
+    unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;
+    const unsigned al = saddr(acc);
+    const unsigned cmb = saddr(candm), pb1 = saddr(pre1), pb2 = saddr(pre2), nb1 = saddr(nrec1), nb2 = saddr(nrec2);
+    const int W = g.W;
+    const int ncols = P + 3 * F;               // row words summed by threads 0..ncols-1
+
+    for (int layer = cluster_id; layer < g.L; layer += p.groups) {
+        __syncthreads();
+        load_ptab(E, r, p.primary + (size_t)layer * E, p.replicas + (size_t)layer * E * r, T.ptab, T.rep);
+        for (int i = tid; i < P * 32; i += kChainThreads) cnt[i] = 0u;
+#pragma unroll
+        for (int f = 0; f < 8; ++f) acc[f * 32] = 0u;
         if (tid < 64) {
             Ls[tid] = (p.load_state && tid < P) ? p.load_state[(size_t)layer * P + tid] : 0.0;
             ltot[tid] = 0ull;
         }
-        if (tid < 16) comm_s[tid] = 0ull;
-        if (tid < 8) fam_s[tid] = 0u;
+        if (tid < 24) csum[tid] = 0ull;
+        if (tid < 16) dsum[tid] = 0ull;
         __syncthreads();
-        // per family, over this thread's tokens: span (bits 0-10) | remote (11-21) | token count (22-31)
-#pragma unroll
-        for (int g = 0; g < 8; ++g) acc[g * 32] = 0u;
-        int since = 0;                      // tokens added to acc since the last flush (uniform per warp)
+        const int nrep = build_ranks(E, T.ptab, rank8, replist, wsum);
+        const int16_t* base = p.indices + (size_t)layer * (size_t)g.N * (size_t)k;
+        const unsigned* rows_l = p.rows + (size_t)layer * g.ipl * W;
+        const size_t rec_l = (size_t)layer * g.ipl * g.slice;
+
+        // per-family sums of this thread's deferred tokens -> CTA.  16-bit fields: a thread takes at most 9 tokens
+        // per item, each <= 16, so they are flushed at least every 256 items
         auto flush_acc = [&]() {
 #pragma unroll
-            for (int g = 0; g < 8; ++g) {
-                if (g < F) {
-                    const unsigned av = acc[g * 32];
-                    const unsigned s = __reduce_add_sync(0xffffffffu, av & 0x7ffu);
-                    const unsigned q = __reduce_add_sync(0xffffffffu, (av >> 11) & 0x7ffu);
+            for (int fq = 0; fq < 8; ++fq) {
+                if (fq < F) {
+                    const unsigned av = acc[fq * 32];
+                    acc[fq * 32] = 0u;
+                    const unsigned sp = __reduce_add_sync(0xffffffffu, av & 0xffffu);
+                    const unsigned rq = __reduce_add_sync(0xffffffffu, av >> 16);
                     if (lane == 0) {
-                        if (s) atomicAdd(&comm_s[g], (unsigned long long)s);
-                        if (q) atomicAdd(&comm_s[8 + g], (unsigned long long)q);
-                    }
-                    if (layer == 0) {               // tokens per family, counted once (family is shared by all layers)
-                        const unsigned c = __reduce_add_sync(0xffffffffu, av >> 22);
-                        if (lane == 0 && c) atomicAdd(&fam_s[g], c);
-                    }
-                    acc[g * 32] = 0u;
-                }
-            }
-            since = 0;
-        };
-        const int16_t* base = p.indices + (size_t)layer * (size_t)p.N * (size_t)k;
-        unsigned char* cost_l = (OUT && p.cost) ? p.cost + (size_t)layer * p.N : nullptr;
-        signed char* serve_l = (OUT && p.serve) ? p.serve + (size_t)layer * p.N * k : nullptr;
-        long long slice0 = 0;               // first token of the slice being processed (for the queued outputs)
-        int qn = 0;                         // tokens waiting in this warp's queue (warp-uniform)
-        // loads, communication cost and outputs of one token whose serve bytes are final; returns span | remote << 11 | 1 << 22
-        auto finish_packed = [&](unsigned long long svp, M R, int hm, int o) -> unsigned {
-#pragma unroll
-            for (int j = 0; j < KM; ++j)
-                if (j < 8) atomicAdd(cnt_lane + (unsigned)((svp >> (8 * j)) & 0xffull) * 32, 1u);
-            const M notHome = ~((M)1 << hm);
-            int nR, rem;
-            if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
-            else { nR = __popc(R); rem = __popc(R & notHome); }
-            if (OUT && cost_l) cost_l[slice0 + o] = (unsigned char)rem;
-            if (OUT && serve_l) {
-                signed char* out = serve_l + ((size_t)slice0 + o) * k;
-#pragma unroll
-                for (int j = 0; j < KM; ++j)
-                    if (j < 8) out[j] = (signed char)((svp >> (8 * j)) & 0xffull);
-            }
-            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 11) | (1u << 22);
-        };
-        // same for a token whose serving partitions are in registers (no replicated slot)
-        auto finish_sv = [&](const int (&sv)[KM], M R, int hm, int o) -> unsigned {
-#pragma unroll
-            for (int j = 0; j < KM; ++j)
-                if (j < k) atomicAdd(cnt_lane + sv[j] * 32, 1u);
-            const M notHome = ~((M)1 << hm);
-            int nR, rem;
-            if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
-            else { nR = __popc(R); rem = __popc(R & notHome); }
-            if (OUT && cost_l) cost_l[slice0 + o] = (unsigned char)rem;
-            if (OUT && serve_l) {
-                signed char* out = serve_l + ((size_t)slice0 + o) * k;
-#pragma unroll
-                for (int j = 0; j < KM; ++j)
-                    if (j < k) out[j] = (signed char)sv[j];
-            }
-            return (unsigned)max(0, nR - 1) | ((unsigned)rem << 11) | (1u << 22);
-        };
-        // resolves the replicated slots of the last `nact` queued tokens, one token per lane
-        auto drain = [&](int nact) {
-            __syncwarp();
-            if (lane < nact) {
-                const unsigned* q = wqueue + (qn - nact + lane) * kDeferWords;
-                unsigned ww[KT > 0 ? KT / 2 : 1];
-#pragma unroll
-                for (int i = 0; i < (KT > 0 ? KT / 2 : 1); ++i) ww[i] = q[i];
-                int e[KM];
-                if constexpr (KT > 0) unpack_ids<KT>(ww, e);
-                const unsigned meta = q[4];
-                const int hm = (int)(meta & 0xffu), fq = (int)(meta >> 8);
-                unsigned long long svp = 0ull;
-                unsigned pend = 0u;
-                M R = 0;
-                if constexpr (KM <= 8) {
-#pragma unroll
-                    for (int j = 0; j < KM; ++j) {          // pass 1 again, on packed serve bytes
-                        const unsigned in = T.ptab[e[j]];
-                        const unsigned isrep = in >> 7;
-                        svp |= (unsigned long long)(in & 63u) << (8 * j);
-                        R |= (M)(isrep ^ 1u) << (in & 63u);
-                        pend |= isrep << j;
-                    }
-                    R = serve_pending_packed<KM, M>(e, pend, hm, R, T, svp);
-                }
-                const unsigned packed = finish_packed(svp, R, hm, (int)q[5]);
-                atomicAdd(&acc[fq * 32], packed);         // queued tokens are live: fq < F
-            }
-            qn -= nact;
-            __syncwarp();
-        };
-
-        for (long long mb = 0; mb < p.nmb; ++mb) {
-            // steps 1-3: snapshot, guard, candidate tables
-            if (REP) {
-                if (tid < 64) T.S[tid] = Ls[tid];
-                __syncthreads();
-                if (tid == 0) feas_s = load_guard(T.S, P, p.theta);
-                __syncthreads();
-                build_candidates(E, r, T, feas_s);
-                __syncthreads();
-            }
-            // step 4: this CTA's slice of the micro-batch
-            const long long mb_begin = mb * p.B;
-            const long long mb_end = min(p.N, mb_begin + p.B);
-            const long long len = mb_end - mb_begin;
-            const long long per = ((len + p.cpl - 1) / p.cpl + 31) / 32 * 32;
-            const long long t0 = mb_begin + (long long)part * per;
-            const long long t1 = min(mb_end, t0 + per);
-            const int n = t1 > t0 ? (int)(t1 - t0) : 0;            // tokens of the slice (per <= 2^31 checked on the host)
-            slice0 = t0;
-            int home = (int)((p.token_offset + t0 + tid) % P);
-            M notHome = ~((M)1 << home);            // constant over the slice when P divides the CTA width (stepP == 0)
-            const int8_t* fam0 = p.family + t0;
-            const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
-            for (int ob = tid; ob < n + tid; ob += kEvalThreads * U) {      // uniform trip count across the CTA
-                int f[U];
-                unsigned w[U][KT > 0 ? KT / 2 : 1];
-#pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const int o = ob + u * kEvalThreads;
-                    f[u] = -1;
-                    if (o < n) {
-                        f[u] = fam0[o];
-                        if constexpr (KT == 8) {
-                            const uint4 v = __ldg(reinterpret_cast<const uint4*>(rows0) + o);
-                            w[u][0] = v.x; w[u][1] = v.y; w[u][2] = v.z; w[u][3] = v.w;
-                        } else if constexpr (KT == 4) {
-                            const uint2 v = __ldg(reinterpret_cast<const uint2*>(rows0) + o);
-                            w[u][0] = v.x; w[u][1] = v.y;
-                        } else if constexpr (KT > 0) {
-                            const unsigned* rp = rows0 + (size_t)o * (KT / 2);
-#pragma unroll
-                            for (int i = 0; i < KT / 2; ++i) w[u][i] = __ldg(rp + i);
-                        }
+                        if (sp) atomicAdd(&dsum[fq], (unsigned long long)sp);
+                        if (rq) atomicAdd(&dsum[8 + fq], (unsigned long long)rq);
                     }
                 }
+            }
+        };
+        // record counts of up to 32 slices starting at s0 (one pending slot | several) and their prefix sums; one warp
+        auto load_counts = [&](const unsigned* rows_mb, int s0, int ns, int ln) {
+            unsigned n1 = 0u, n2 = 0u;
+            if (ln < ns) {
+                n1 = rows_mb[(size_t)(s0 + ln) * W + ncols];
+                n2 = rows_mb[(size_t)(s0 + ln) * W + ncols + 1];
+                if (n1 == kOverflow) { n1 = 0u; n2 = 0u; ovf_s[ln] = 1u; } else ovf_s[ln] = 0u;
+            }
+            nrec1[ln] = n1;
+            nrec2[ln] = n2;
+            unsigned a1 = n1, a2 = n2;
 #pragma unroll
-                for (int u = 0; u < U; ++u) {
-                    const int o = ob + u * kEvalThreads;
-                    const bool live = (unsigned)f[u] < (unsigned)F;
-                    unsigned packed = 0;
-                    bool defer = false;
-                    unsigned pend = 0u;
-                    if (live) {
-                        int e[KM], sv[KM];
-                        M R;
-                        bool fast = false;
-                        if constexpr (KT > 0) {
-                            unpack_ids<KT>(w[u], e);
-                            unsigned hi = (unsigned)e[0];       // a negative id is a huge unsigned value
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned v1 = __shfl_up_sync(0xffffffffu, a1, d), v2 = __shfl_up_sync(0xffffffffu, a2, d);
+                if (ln >= d) { a1 += v1; a2 += v2; }
+            }
+            pre1[ln + 1] = a1;
+            pre2[ln + 1] = a2;
+            if (ln == 0) { pre1[0] = 0u; pre2[0] = 0u; }
+        };
+        for (long long mb = 0; mb < g.nmb; ++mb) {
+            const unsigned* rows_mb = rows_l + (size_t)mb * g.spm * W;
+            // the scan kernel's sums of this micro-batch (independent of the chain: read them early)
+            unsigned long long mine = 0ull;
+            if (tid < ncols)
+                for (int s = 0; s < g.spm; ++s) mine += rows_mb[(size_t)s * W + tid];
+            // steps 1-3: snapshot, guard, candidate tables of the replicated experts; the second warp fetches the
+            // record counts of the first 32 slices meanwhile
+            if (tid < 64) T.S[tid] = Ls[tid];
+            __syncthreads();
+            if (tid == 0) feas_s = load_guard(T.S, P, p.theta);
+            if (tid == 0) bigq_s = 0u;
+            if (tid >= 32 && tid < 64) load_counts(rows_mb, 0, min(32, g.spm), tid - 32);
+            __syncthreads();
+            const unsigned long long feas = feas_s;
+            for (int i = tid; i < nrep; i += kChainThreads) {
+                const int e = (int)replist[i];
+                unsigned char* out = T.cand + e * kCandStride;
+                build_candidate(e, r, T, feas, out);
+                if (i < kMaxRank) {
+                    // by rank: the one-hot masks of the first four candidates (entries beyond the count repeat the first)
+                    const int n = out[0];
+                    M* cm = reinterpret_cast<M*>(candm) + (i + 1) * 4;
 #pragma unroll
-                            for (int j = 1; j < KT; ++j) hi = max(hi, (unsigned)e[j]);
-                            fast = hi < (unsigned)E;
-                        } else {
-#pragma unroll
-                            for (int j = 0; j < 16; ++j)
-                                e[j] = (j < k) ? (int)__ldg(base + ((size_t)t0 + o) * k + j) : -1;
-                        }
-                        bool done = true;
-                        if constexpr (kQueued) {
-                            if (fast) {
-                                // pass 1; a token with replicated slots waits in the warp's queue (only its ids are kept)
-                                M R1 = 0;
-#pragma unroll
-                                for (int j = 0; j < KM; ++j) {
-                                    const unsigned in = T.ptab[e[j]];
-                                    const unsigned isrep = in >> 7;
-                                    sv[j] = (int)(in & 63u);
-                                    R1 |= (M)(isrep ^ 1u) << (in & 63u);
-                                    pend |= isrep;
-                                }
-                                defer = pend != 0u;
-                                done = false;
-                                if (!defer) packed = finish_sv(sv, R1, home, o);
-                            }
-                        }
-                        if (done) {
-                            if (fast) {
-                                R = serve_fast<KM, REP, M>(e, home, T, sv);
-#pragma unroll
-                                for (int j = 0; j < KM; ++j) atomicAdd(cnt_lane + sv[j] * 32, 1u);
-                            } else {
-                                R = serve_token<KM, M>(e, k, E, home, T, sv);
-#pragma unroll
-                                for (int j = 0; j < KM; ++j)
-                                    if (j < k && sv[j] >= 0) atomicAdd(cnt_lane + sv[j] * 32, 1u);
-                            }
-                            int nR, rem;
-                            if constexpr (sizeof(M) == 8) { nR = __popcll(R); rem = __popcll(R & notHome); }
-                            else { nR = __popc(R); rem = __popc(R & notHome); }
-                            packed = (unsigned)max(0, nR - 1) | ((unsigned)rem << 11) | (1u << 22);
-                            if (OUT && cost_l) cost_l[t0 + o] = (unsigned char)rem;
-                            if (OUT && serve_l) {
-                                signed char* out = serve_l + ((size_t)t0 + o) * k;
-#pragma unroll
-                                for (int j = 0; j < KM; ++j)
-                                    if (j < k) out[j] = (signed char)sv[j];
-                            }
-                        }
-                    } else if (o < n) {
-                        if (OUT && cost_l) cost_l[t0 + o] = 0;
-                        if (OUT && serve_l)
-                            for (int j = 0; j < k; ++j) serve_l[((size_t)t0 + o) * k + j] = -1;
+                    for (int q = 0; q < 4; ++q) cm[q] = (M)1 << out[1 + (q < n ? q : 0)];
+                    if (n > 4) atomicOr(&bigq_s, 1u << (i + 1));
+                    unsigned* dst = reinterpret_cast<unsigned*>(candr + (i + 1) * kCandStride);
+                    const unsigned* src = reinterpret_cast<const unsigned*>(out);
+                    dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+                }
+            }
+            __syncthreads();
+            const unsigned bigq = bigq_s;
+            // one pending slot: rank q of the replicated expert, loc = accessed set so far | home; returns the pick
+            auto pick_slot = [&](unsigned q, M loc) -> M {
+                M m1, m2, m3, m4;
+                if constexpr (sizeof(M) == 4) {
+                    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(m1), "=r"(m2), "=r"(m3), "=r"(m4) : "r"(cmb + q * 16u));
+                } else {
+                    asm volatile("ld.shared.v2.u64 {%0,%1}, [%2];" : "=l"(m1), "=l"(m2) : "r"(cmb + q * 32u));
+                    asm volatile("ld.shared.v2.u64 {%0,%1}, [%2];" : "=l"(m3), "=l"(m4) : "r"(cmb + q * 32u + 16u));
+                }
+                M pm = (loc & m1) ? m1 : ((loc & m2) ? m2 : ((loc & m3) ? m3 : ((loc & m4) ? m4 : m1)));
+                if (((bigq >> q) & 1u) && !(loc & (m1 | m2 | m3 | m4)))          // more than four candidates listed
+                    pm = (M)1 << pick_candidate<M>(candr + q * kCandStride, loc);
+                return pm;
+            };
+            // step 4: the pending slots of this micro-batch.  The records of up to 32 slices form one index space per
+            // record class, so that a thread's loads from different slices are in flight together.
+            for (int s0 = 0; s0 < g.spm; s0 += 32) {
+                const int ns = min(32, g.spm - s0);
+                if (s0 > 0) {
+                    __syncthreads();
+                    if (tid < 32) load_counts(rows_mb, s0, ns, tid);
+                    __syncthreads();
+                }
+                const size_t ro0 = rec_l + ((size_t)mb * g.spm + s0) * (size_t)g.slice;
+                const M* rset = reinterpret_cast<const M*>(p.rec.set) + ro0;
+                const unsigned* rrank = p.rec.rank + ro0;
+                const unsigned* rmeta = p.rec.meta + ro0;
+                const unsigned stride = (unsigned)CS * kChainThreads;
+                const unsigned slice = (unsigned)g.slice;
+                // per-token outputs of a record at entry x (OUT only): token index from the slice and the offset
+                auto token_of = [&](unsigned x, unsigned meta) -> size_t {
+                    long long t0, t1;
+                    item_tokens(g, mb, s0 + (int)(x / slice), t0, t1);
+                    return (size_t)layer * g.N + t0 + (meta & 0x1fffu);
+                };
+                // one record: its pending slots in slot order (lowest nibble first), then the communication cost
+                auto resolve = [&](M R, unsigned rk, unsigned meta, unsigned x) {
+                    const M hb = (M)1 << ((meta >> 16) & 63u);
+                    while (rk) {
+                        const int sh = (__ffs(rk) - 1) & ~3;
+                        const M pm = pick_slot((rk >> sh) & 15u, R | hb);
+                        rk &= ~(15u << sh);
+                        R |= pm;
+                        const int pick = sizeof(M) == 8 ? 63 - __clzll((long long)pm) : 31 - __clz((int)pm);
+                        sred_inc(cl + (unsigned)pick * 128u);
+                        if (OUT && p.serve) p.serve[token_of(x, meta) * k + (sh >> 2)] = (signed char)pick;
                     }
-                    // packed is 0 unless f[u] is a family < F
-                    if (packed) atomicAdd(&acc[f[u] * 32], packed);
-                    if constexpr (kQueued) {
-                        const unsigned dm = __ballot_sync(0xffffffffu, defer);
-                        if (defer) {
-                            unsigned* q = wqueue + (qn + __popc(dm & ((1u << lane) - 1u))) * kDeferWords;
-#pragma unroll
-                            for (int i = 0; i < KT / 2; ++i) q[i] = w[u][i];
-                            q[4] = (unsigned)home | ((unsigned)f[u] << 8);
-                            q[5] = (unsigned)o;
+                    const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~hb);
+                    if (OUT && p.cost) p.cost[token_of(x, meta)] = (unsigned char)rem;
+                    sred_add(al + ((meta >> 13) & 7u) * 128u, (unsigned)max(0, nR - 1) | ((unsigned)rem << 16));
+                };
+#pragma unroll 1
+                for (int cls = 0; cls < 2; ++cls) {
+                    const unsigned pb = cls ? pb2 : pb1;               // shared address of the prefix sums
+                    const unsigned tot = slds_u32(pb + 4u * ns);
+                    // entry of flat index gi; the slice index only moves forward
+                    unsigned sl = 0u, lo_sl = 0u, hi_sl = slds_u32(pb + 4u);
+                    auto locate = [&](unsigned gi) -> unsigned {
+                        while (gi >= hi_sl) {
+                            ++sl;
+                            lo_sl = hi_sl;
+                            hi_sl = slds_u32(pb + 4u * (sl + 1u));
                         }
-                        qn += __popc(dm);
-                        if (qn >= 32) drain(32);
-                    }
-                    if (stepP) {
-                        home += stepP;
-                        if (home >= P) home -= P;
-                        notHome = ~((M)1 << home);
+                        const unsigned within = gi - lo_sl;
+                        return sl * slice + (cls ? slice - 1u - within : within);
+                    };
+                    for (unsigned g0 = (unsigned)rank * kChainThreads + tid; g0 < tot; g0 += 2u * stride) {
+                        // two records per round, all six loads in flight before the first is used
+                        unsigned x[2], rk[2], me[2];
+                        M Rs[2];
+#pragma unroll
+                        for (int q = 0; q < 2; ++q) {
+                            const unsigned gq = g0 + (unsigned)q * stride;
+                            x[q] = gq < tot ? locate(gq) : x[0];
+                        }
+#pragma unroll
+                        for (int q = 0; q < 2; ++q) {
+                            Rs[q] = rset[x[q]];
+                            rk[q] = rrank[x[q]];
+                            me[q] = rmeta[x[q]];
+                        }
+#pragma unroll
+                        for (int q = 0; q < 2; ++q)
+                            if (g0 + (unsigned)q * stride < tot) resolve(Rs[q], rk[q], me[q], x[q]);
                     }
                 }
-                since += kQueued ? 2 * U : U;     // a queued token adds to acc when it is drained
-                if (since >= 120) flush_acc();      // 11-bit fields: 124 tokens x (span <= 15, remote <= 16) fit
+                // items left to this kernel: their tokens are served here, from the trace
+                for (int s = s0; s < s0 + ns; ++s) {
+                    if (!ovf_s[s - s0]) continue;
+                    long long t0, t1;
+                    item_tokens(g, mb, s, t0, t1);
+                    const unsigned hb0 = (unsigned)((g.token_offset + t0) % P);
+                    const long long n = t1 - t0;
+                    const long long lo = n * rank / CS, hi = n * (rank + 1) / CS;
+                    for (long long o = lo + tid; o < hi; o += kChainThreads) {
+                        const int fq = p.family[t0 + o];
+                        if ((unsigned)fq >= (unsigned)F) continue;
+                        int e[16], sv[16];
+#pragma unroll
+                        for (int j = 0; j < 16; ++j) e[j] = (j < k) ? (int)__ldg(base + ((size_t)t0 + o) * k + j) : -1;
+                        const int home = (int)((hb0 + o) % P);
+                        const M R = serve_token<16, M>(e, k, E, home, T, sv);
+#pragma unroll
+                        for (int j = 0; j < 16; ++j)
+                            if (j < k && sv[j] >= 0) sred_inc(cl + (unsigned)sv[j] * 128u);
+                        const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~((M)1 << home));
+                        if (OUT && p.cost) p.cost[(size_t)layer * g.N + t0 + o] = (unsigned char)rem;
+                        if (OUT && p.serve)
+                            for (int j = 0; j < k; ++j) p.serve[((size_t)layer * g.N + t0 + o) * k + j] = (signed char)sv[j];
+                        sred_add(al + (unsigned)fq * 128u, (unsigned)max(0, nR - 1) | ((unsigned)rem << 16));
+                    }
+                }
+                // 16-bit fields: a thread takes at most 32 * 8192 / 1024 tokens of <= 16 each per round
+                flush_acc();
             }
-            if constexpr (kQueued) {
-                while (qn > 0) drain(min(qn, 32));
-            }
-            flush_acc();
             // step 5: integer dispatch counts of the micro-batch, then Eq. 15
             __syncthreads();
-            for (int m = tid >> 5; m < P; m += kEvalThreads / 32) {
-                const unsigned s = __reduce_add_sync(0xffffffffu, cnt[m * 32 + lane]);
+            const int par = (int)(mb & 1);
+            for (int m = tid >> 5; m < P; m += kChainThreads / 32) {
+                const unsigned sm = __reduce_add_sync(0xffffffffu, cnt[m * 32 + lane]);
                 cnt[m * 32 + lane] = 0u;
-                if (lane == 0) dsum[m] = (unsigned long long)s;
+                if (lane == 0) exch[par][m] = sm;
             }
-            __syncthreads();
-            // Without replicas nothing depends on the snapshot (and the whole trace is one micro-batch): a CTA only
-            // writes its own row of partial sums, never waits and never touches an accumulated output;
-            // fairness_kernel adds the rows of a layer and applies Eq. 15.
-            const bool ema_here = REP;
-            if constexpr (REP) {
-                if (p.cpl > 1) {
-                    unsigned long long* dl = p.delta + ((size_t)layer * p.nmb + mb) * P;
-                    if (tid < P && dsum[tid]) atomicAdd(&dl[tid], dsum[tid]);
-                    __threadfence();
-                    __syncthreads();
-                    if (tid == 0) {
-                        atomicAdd(&p.barrier[layer], 1u);
-                        const unsigned target = (unsigned)((mb + 1) * p.cpl);
-                        volatile unsigned* bar = p.barrier + layer;
-                        while (*bar < target) __nanosleep(20);
-                        __threadfence();
-                    }
-                    __syncthreads();
-                    if (tid < P) dsum[tid] = __ldcg(&dl[tid]);
-                    __syncthreads();
+            if constexpr (CLUSTER) cg::this_cluster().sync();
+            else __syncthreads();
+            if (tid < P) {
+                unsigned long long d = mine;
+                if constexpr (CLUSTER) {
+                    cg::cluster_group cgl = cg::this_cluster();
+                    for (int q = 0; q < CS; ++q) d += cgl.map_shared_rank(&exch[par][0], q)[tid];
+                } else {
+                    d += exch[par][tid];
                 }
-            } else {
-                if (tid < P) ltot[tid] += dsum[tid];
-            }
-            if (ema_here && tid < P) {
-                const unsigned long long d = dsum[tid];
                 Ls[tid] = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
                 ltot[tid] += d;
+            } else if (tid < ncols) {
+                csum[tid - P] += mine;
             }
             __syncthreads();
         }
-        // layer epilogue: communication sums and, from part 0, loads and the final state
-        if constexpr (REP) {
-            if (layer == 0 && tid < F && fam_s[tid]) atomicAdd(&p.ntok[tid], (unsigned long long)fam_s[tid]);
-            if (tid < F) {
-                if (comm_s[tid]) atomicAdd(&p.comm_span[(size_t)layer * F + tid], comm_s[tid]);
-                if (comm_s[8 + tid]) atomicAdd(&p.comm_remote[(size_t)layer * F + tid], comm_s[8 + tid]);
-            }
-            if (part == 0 && tid < P) {
+        // layer epilogue: rank 0 adds the deferred tokens' communication sums of its peers and writes the outputs
+        if constexpr (CLUSTER) cg::this_cluster().sync();
+        if (rank == 0) {
+            if (tid < P) {
                 p.load[(size_t)layer * P + tid] = ltot[tid];
                 if (p.load_state) p.load_state[(size_t)layer * P + tid] = Ls[tid];
-            }
-        } else {
-            unsigned long long* row = p.partial + ((size_t)layer * p.cpl + part) * (size_t)(P + 3 * F);
-            if (tid < P) row[tid] = ltot[tid];
-            if (tid < F) {
-                row[P + tid] = comm_s[tid];
-                row[P + F + tid] = comm_s[8 + tid];
-                row[P + 2 * F + tid] = layer == 0 ? (unsigned long long)fam_s[tid] : 0ull;
+            } else if (tid >= 64 && tid < 64 + 2 * F) {
+                const int which = (tid - 64) / F, f = (tid - 64) % F;
+                unsigned long long v = csum[which * F + f];
+                if constexpr (CLUSTER) {
+                    cg::cluster_group cgl = cg::this_cluster();
+                    for (int q = 0; q < CS; ++q) v += cgl.map_shared_rank(&dsum[0], q)[which * 8 + f];
+                } else {
+                    v += dsum[which * 8 + f];
+                }
+                (which ? p.comm_remote : p.comm_span)[(size_t)layer * F + f] = v;
+            } else if (layer == 0 && tid >= 128 && tid < 128 + F) {
+                p.ntok[tid - 128] = csum[2 * F + (tid - 128)];
             }
         }
+        if constexpr (CLUSTER) cg::this_cluster().sync();     // peers keep their sums until rank 0 has read them
     }
 }
 
@@ -637,13 +872,14 @@ eval_kernel(EvalParams p) {
 // One CTA per output row (row L = loads summed over layers), 64 x 16 threads: thread (m, q) adds the
 // layers q, q+16, ... of partition m, so no thread walks more than L/16 dependent loads; the
 // statistics are then computed by one thread from the P sums in the fixed order m = 0..P-1.
-// partial != nullptr (the no-replica path): the CTAs of the evaluation kernel left one row of partial sums each
-// (loads | span | remote | tokens per family); row l < L adds the rows of its layer, applies Eq. 15 (one
-// micro-batch: the same two fp64 operations the evaluation kernel applies) and writes load, load_state, comm_span,
-// comm_remote and, from layer 0, ntok; row L sums the loads of all layers.
+// rows != nullptr (the no-replica path): the scan kernel left one row of partial sums per item
+// (loads | span | remote | tokens per family | -); row l < L adds the `ipl` rows of its layer, applies Eq. 15
+// (one micro-batch: the same two fp64 operations the chain kernel applies) and writes load, load_state,
+// comm_span, comm_remote and, from layer 0, ntok; row L sums the loads of all layers.
 __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __restrict__ load, int L, int P,
-                                                       float* __restrict__ out, const unsigned long long* __restrict__ partial,
-                                                       int cpl, int F, double rho, double* __restrict__ load_state,
+                                                       float* __restrict__ out, const unsigned* __restrict__ rows,
+                                                       long long ipl, int W, int F, double rho,
+                                                       double* __restrict__ load_state,
                                                        unsigned long long* __restrict__ comm_span,
                                                        unsigned long long* __restrict__ comm_remote,
                                                        unsigned long long* __restrict__ ntok) {
@@ -654,17 +890,16 @@ __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __re
     const int row = blockIdx.x;
     const int m = threadIdx.x & 63, q = threadIdx.x >> 6;
     unsigned long long v = 0, csum = 0;
-    if (partial) {
-        // thread (m, q) adds the CTA rows q, q+16, ...: no thread walks more than cpl/16 dependent loads
-        const size_t W = (size_t)(P + 3 * F);
+    if (rows) {
+        // thread (m, q) adds the item rows q, q+16, ...
         if (row < L) {
-            const unsigned long long* rows = partial + (size_t)row * cpl * W;
-            for (int c = q; c < cpl; c += 16) {
-                if (m < P) v += rows[(size_t)c * W + m];
-                if (m < 3 * F) csum += rows[(size_t)c * W + P + m];
+            const unsigned* rl = rows + (size_t)row * ipl * W;
+            for (long long c = q; c < ipl; c += 16) {
+                if (m < P) v += rl[(size_t)c * W + m];
+                if (m < 3 * F) csum += rl[(size_t)c * W + P + m];
             }
         } else if (m < P) {
-            for (long long i = q; i < (long long)L * cpl; i += 16) v += partial[(size_t)i * W + m];
+            for (long long i = q; i < (long long)L * ipl; i += 16) v += rows[(size_t)i * W + m];
         }
         if (m < 24) cpart[q][m] = csum;
     } else if (m < P) {
@@ -678,14 +913,14 @@ __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __re
 #pragma unroll
         for (int z = 0; z < 16; ++z) t += part[z][m];
         x[m] = (double)t;
-        if (partial && row < L && m < P) {
+        if (rows && row < L && m < P) {
             load[(size_t)row * P + m] = t;
             if (load_state) {
                 const double Ls = load_state[(size_t)row * P + m];
                 load_state[(size_t)row * P + m] = __dadd_rn(__dmul_rn(rho, Ls), (double)t);   // no FMA (Q19)
             }
         }
-    } else if (q == 1 && partial && row < L && m < 3 * F) {
+    } else if (q == 1 && rows && row < L && m < 3 * F) {
         unsigned long long t = 0;
 #pragma unroll
         for (int z = 0; z < 16; ++z) t += cpart[z][m];
@@ -714,6 +949,11 @@ __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __re
     }
 }
 
+size_t select_smem_bytes(int E, int r) {
+    return 64 * sizeof(double) + kPtab + (((size_t)E * kCandStride + 15) & ~(size_t)15) +
+           (((size_t)E * (r > 0 ? r : 1) + 15) & ~(size_t)15);
+}
+
 // gesr_select: serve for one given snapshot; grid = (token blocks, layer)
 template <int KT>
 __global__ void __launch_bounds__(kEvalThreads)
@@ -723,15 +963,20 @@ select_kernel(const int16_t* __restrict__ indices, long long N, int k, int E, in
     extern __shared__ __align__(16) unsigned char ssm[];
     constexpr int KM = KT > 0 ? KT : 16;
     LayerTables T;
-    carve_tables(ssm, E, r, T);
+    size_t off = 0;
+    T.S = reinterpret_cast<double*>(ssm + off);            off += 64 * sizeof(double);
+    T.ptab = ssm + off;                                    off += kPtab;
+    T.cand = ssm + off;                                    off += ((size_t)E * kCandStride + 15) & ~(size_t)15;
+    T.rep = reinterpret_cast<signed char*>(ssm + off);
     __shared__ unsigned long long feas_s;
     const int layer = blockIdx.y;
-    load_tables(E, r, primary + (size_t)layer * E, replicas ? replicas + (size_t)layer * E * r : nullptr, T);
+    load_ptab(E, replicas ? r : 0, primary + (size_t)layer * E, replicas ? replicas + (size_t)layer * E * r : nullptr,
+              T.ptab, T.rep);
     if (threadIdx.x < 64) T.S[threadIdx.x] = threadIdx.x < P ? snapshot[(size_t)layer * P + threadIdx.x] : 0.0;
     __syncthreads();
     if (threadIdx.x == 0) feas_s = load_guard(T.S, P, theta);
     __syncthreads();
-    build_candidates(E, r, T, feas_s);
+    build_candidates(E, replicas ? r : 0, T, feas_s);
     __syncthreads();
     const int16_t* base = indices + (size_t)layer * (size_t)N * (size_t)k;
     const long long stride = (long long)gridDim.x * kEvalThreads;
@@ -754,100 +999,87 @@ select_kernel(const int16_t* __restrict__ indices, long long N, int k, int E, in
     }
 }
 
-// clears the accumulated outputs and the barrier scratch in one launch
-__global__ void eval_zero_kernel(unsigned long long* a, size_t na, unsigned long long* b, size_t nb,
-                                 unsigned long long* c, size_t nc, unsigned long long* d, size_t nd,
-                                 unsigned long long* s, size_t ns) {
-    tacg_pdl_prologue();
-    const size_t stride = (size_t)gridDim.x * blockDim.x;
-    const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (size_t i = i0; i < na; i += stride) a[i] = 0ull;
-    for (size_t i = i0; i < nb; i += stride) b[i] = 0ull;
-    for (size_t i = i0; i < nc; i += stride) c[i] = 0ull;
-    for (size_t i = i0; i < nd; i += stride) d[i] = 0ull;
-    for (size_t i = i0; i < ns; i += stride) s[i] = 0ull;
+struct EvalCall {
+    tacg_ctx* ctx;
+    ScanParams sp;
+    ChainParams cp;
+    bool rep, out;
+};
+
+template <int KT, bool REP, typename M, bool OUT>
+int launch_scan(EvalCall& c) {
+    tacg_ctx* ctx = c.ctx;
+    auto kern = eval_scan_kernel<KT, REP, M, OUT>;
+    const size_t smem = sizeof(unsigned) * (kSink + 1) * 32 + sizeof(unsigned) * (kEvalThreads / 32) * 8 * 32;
+    const long long T = (long long)c.sp.g.L * c.sp.g.ipl;
+    const int grid = (int)max(1ll, min(T, (long long)ctx->sm_count * 2));
+    TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kEvalThreads), smem, ctx->stream, c.sp));
+    TACG_LAUNCH_CHECK(ctx);
+    return TACG_OK;
 }
 
-size_t eval_smem_bytes(int E, int P, int r) {
-    return tables_bytes(E, r) + 64 * sizeof(unsigned long long) + sizeof(unsigned) * (size_t)P * 32 +
-           (r > 0 ? sizeof(unsigned) * (size_t)(kEvalThreads / 32) * kDeferCap * kDeferWords : 0) +
-           sizeof(unsigned) * (size_t)(kEvalThreads / 32) * 8 * 32;
+template <typename M, bool OUT>
+int launch_chain(EvalCall& c) {
+    tacg_ctx* ctx = c.ctx;
+    const EvalGeom& g = c.cp.g;
+    const size_t smem = 64 * sizeof(double) + (((size_t)g.E * kCandStride + 15) & ~(size_t)15) +
+                        (((size_t)g.E * g.r + 15) & ~(size_t)15) + sizeof(unsigned) * (size_t)g.P * 32 +
+                        sizeof(unsigned) * (kChainThreads / 32) * 8 * 32 + sizeof(unsigned short) * (size_t)g.E + 16;
+    // cluster size: as many CTAs per layer as the SM count allows, up to 16 (non-portable above 8)
+    int cs = 1;
+    while (cs < 16 && (long long)g.L * cs * 2 <= ctx->sm_count) cs *= 2;
+    // a micro-batch with few records gains nothing from more CTAs
+    while (cs > 1 && min(g.B, g.N) < (long long)cs * 2048) cs /= 2;
+    c.cp.groups = min(g.L, max(1, ctx->sm_count / cs));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(c.cp.groups * cs);
+    cfg.blockDim = dim3(kChainThreads);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cs;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (cs > 1) {
+        auto kern = eval_chain_kernel<M, OUT, true>;
+        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        if (cs > 8) TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        TACG_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, c.cp));
+    } else {
+        auto kern = eval_chain_kernel<M, OUT, false>;
+        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        cfg.numAttrs = 0;
+        TACG_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, c.cp));
+    }
+    TACG_LAUNCH_CHECK(ctx);
+    return TACG_OK;
 }
 
 template <int KT>
-int launch_eval_t(tacg_ctx* ctx, EvalParams& p) {
-    const size_t smem = eval_smem_bytes(p.E, p.P, p.r);
-    const bool rep = p.replicas != nullptr && p.r > 0;
-    const bool out = p.cost != nullptr || p.serve != nullptr;
-    void (*kern)(EvalParams);
-    if (p.P <= 32) {
-        kern = rep ? (out ? eval_kernel<KT, true, unsigned, true> : eval_kernel<KT, true, unsigned, false>)
-                   : (out ? eval_kernel<KT, false, unsigned, true> : eval_kernel<KT, false, unsigned, false>);
-    } else {
-        kern = rep ? (out ? eval_kernel<KT, true, unsigned long long, true> : eval_kernel<KT, true, unsigned long long, false>)
-                   : (out ? eval_kernel<KT, false, unsigned long long, true> : eval_kernel<KT, false, unsigned long long, false>);
+int launch_eval_t(EvalCall& c) {
+    const bool wide = c.sp.g.P > 32;
+    int rc;
+    if (c.rep) {
+        if (wide) rc = c.out ? launch_scan<KT, true, unsigned long long, true>(c) : launch_scan<KT, true, unsigned long long, false>(c);
+        else rc = c.out ? launch_scan<KT, true, unsigned, true>(c) : launch_scan<KT, true, unsigned, false>(c);
+        if (rc != TACG_OK) return rc;
+        if (wide) return c.out ? launch_chain<unsigned long long, true>(c) : launch_chain<unsigned long long, false>(c);
+        return c.out ? launch_chain<unsigned, true>(c) : launch_chain<unsigned, false>(c);
     }
-    int occ = 0;
-    // the largest shapes (E = 512, P = 64, r = 8) need a little more than the 48 KB default
-    TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    TACG_CUDA_TRY(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kEvalThreads, smem));
-    if (occ < 1) occ = 1;
-    const int max_grid = ctx->sm_count * occ;
-    // CTAs per layer: spread the grid over the layers; never more CTAs than 512-token slices of a micro-batch
-    long long cpl = max(1, max_grid / p.L);
-    // (one token per thread and micro-batch is still worth a CTA: with few layers the per-micro-batch
-    //  latency chain dominates, measured on config 5: 64 CTAs 2.7 ms, 96-128 CTAs 2.5 ms)
-    const long long slices = max(1ll, (min(p.B, p.N) + kEvalThreads - 1) / kEvalThreads);
-    if (cpl > slices) cpl = slices;
-    p.cpl = (int)cpl;
-    if ((min(p.B, p.N) + cpl - 1) / cpl + 32 > 0x7fffffffll) {
-        snprintf(ctx->detail, sizeof(ctx->detail), "eval: more than 2^31 tokens per CTA slice");
-        return TACG_ERR_SHAPE;
-    }
-    p.groups = (int)min((long long)p.L, (long long)max_grid / cpl);
-    const int grid = p.groups * p.cpl;
-    const bool waits = rep && p.cpl > 1 && p.nmb > 1;     // CTAs of a group meet at a barrier per micro-batch
-    size_t off = 0;
-    if (rep) {
-        const size_t o_delta = off; off += tacg_align_up(sizeof(unsigned long long) * (size_t)p.L * (size_t)p.nmb * p.P, 256);
-        const size_t o_bar = off;   off += tacg_align_up(sizeof(unsigned) * (size_t)p.L, 256);
-        char* base = static_cast<char*>(tacg_scratch(ctx, off));
-        if (!base) return TACG_ERR_CUDA;
-        p.delta = reinterpret_cast<unsigned long long*>(base + o_delta);
-        p.barrier = reinterpret_cast<unsigned*>(base + o_bar);
-        p.partial = nullptr;
-        const size_t ns = p.cpl > 1 ? off / sizeof(unsigned long long) : 0;
-        const int zgrid = (int)max((size_t)1, min((size_t)ctx->sm_count, (ns + 1023) / 1024));
-        TACG_CUDA_TRY(ctx, tacg_launch_pdl(eval_zero_kernel, dim3(zgrid), dim3(1024), 0, ctx->stream, p.comm_span,
-                                           (size_t)p.L * p.F, p.comm_remote, (size_t)p.L * p.F, p.load, (size_t)p.L * p.P,
-                                           p.ntok, (size_t)p.F, reinterpret_cast<unsigned long long*>(base), ns));
-        TACG_LAUNCH_CHECK(ctx);
-    } else {
-        // every (layer, part) row is written by exactly one CTA, so nothing needs clearing
-        off = sizeof(unsigned long long) * (size_t)p.L * (size_t)p.cpl * (size_t)(p.P + 3 * p.F);
-        char* base = static_cast<char*>(tacg_scratch(ctx, off));
-        if (!base) return TACG_ERR_CUDA;
-        p.partial = reinterpret_cast<unsigned long long*>(base);
-        p.delta = nullptr; p.barrier = nullptr;
-    }
-    tacg_prof_scope prof(ctx, TACG_PROF_EVAL);
-    if (waits) {
-        void* args[] = {&p};
-        TACG_CUDA_TRY(ctx, cudaLaunchCooperativeKernel((const void*)kern, dim3(grid), dim3(kEvalThreads), args, smem,
-                                                       ctx->stream));
-        ctx->launches += 1;
-    } else {
-        TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kEvalThreads), smem, ctx->stream, p));
-        TACG_LAUNCH_CHECK(ctx);
-    }
-    return TACG_OK;
+    if (wide) rc = c.out ? launch_scan<KT, false, unsigned long long, true>(c) : launch_scan<KT, false, unsigned long long, false>(c);
+    else rc = c.out ? launch_scan<KT, false, unsigned, true>(c) : launch_scan<KT, false, unsigned, false>(c);
+    return rc;
 }
 
 template <int KT>
 int launch_select_t(tacg_ctx* ctx, const int16_t* indices, int64_t N, int k, int L, int E, int P,
                     const int8_t* primary, const int8_t* replicas, int r, const double* snapshot, float theta,
                     int64_t token_offset, int8_t* serve) {
-    const size_t smem = tables_bytes(E, r);
+    const size_t smem = select_smem_bytes(E, r);
     const long long blocks = (N + kEvalThreads - 1) / kEvalThreads;
     const int gx = (int)max(1ll, min(blocks, (long long)max(1, ctx->sm_count * 8 / L)));
     select_kernel<KT><<<dim3(gx, L), kEvalThreads, smem, ctx->stream>>>(
@@ -884,39 +1116,80 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(load, 0, sizeof(uint64_t) * (size_t)L * P, ctx->stream));
         TACG_CUDA_TRY(ctx, cudaMemsetAsync(ntok, 0, sizeof(uint64_t) * (size_t)F, ctx->stream));
     }
-    const unsigned long long* fin_partial = nullptr;   // set when the fairness kernel still has the CTA rows to add
-    int fin_cpl = 0;
+    const unsigned* fin_rows = nullptr;   // set when the fairness kernel still has the item rows to add
+    long long fin_ipl = 0;
+    int fin_W = 0;
     if (N > 0) {
-        EvalParams p;
-        p.indices = indices; p.family = family; p.N = N; p.k = k; p.L = L; p.E = E; p.F = F; p.P = P; p.r = r;
-        p.primary = primary; p.replicas = replicas; p.theta = theta; p.rho = rho;
-        const bool use_rep = replicas != nullptr && r > 0;
-        p.B = (!use_rep || microbatch <= 0 || microbatch > N) ? N : microbatch;
-        p.nmb = (N + p.B - 1) / p.B;
-        p.token_offset = token_offset;
-        p.load_state = load_state;
-        p.load = reinterpret_cast<unsigned long long*>(load);
-        p.comm_span = reinterpret_cast<unsigned long long*>(comm_span);
-        p.comm_remote = reinterpret_cast<unsigned long long*>(comm_remote);
-        p.ntok = reinterpret_cast<unsigned long long*>(ntok);
-        p.cost = cost_per_token;
-        p.serve = reinterpret_cast<signed char*>(serve);
-        p.delta = nullptr; p.barrier = nullptr; p.partial = nullptr; p.cpl = 1; p.groups = 1;
+        EvalCall c;
+        c.ctx = ctx;
+        c.rep = replicas != nullptr && r > 0;
+        c.out = cost_per_token != nullptr || serve != nullptr;
+        EvalGeom g;
+        g.N = N; g.k = k; g.L = L; g.E = E; g.F = F; g.P = P; g.r = c.rep ? r : 0;
+        g.B = (!c.rep || microbatch <= 0 || microbatch > N) ? N : microbatch;
+        g.nmb = (N + g.B - 1) / g.B;
+        // slice: as large as the record format allows (the per-item epilogue is amortised over 16 tokens per
+        // thread); smaller only when the whole trace would otherwise give the scan grid fewer than two items per CTA
+        long long slice = kSlice;
+        if ((long long)L * N < (long long)kSlice * ctx->sm_count * 4)
+            slice = std::max(1ll, (long long)L * N / ((long long)ctx->sm_count * 4));
+        slice = std::min((long long)kSlice, std::min(g.B, slice));
+        slice = std::max(512ll, (slice + 511) / 512 * 512);
+        g.slice = (int)slice;
+        g.spm = (int)((g.B + slice - 1) / slice);
+        g.ipl = g.nmb * g.spm;
+        g.W = (int)tacg_align_up((size_t)P + 3 * (size_t)F + 2, 4);
+        g.token_offset = token_offset;
+        const int kt = tacg_pick_kt(k, indices);
+        const size_t items = (size_t)L * (size_t)g.ipl;
+        const size_t nrec = (c.rep && kt > 0) ? items * (size_t)g.slice : 0;      // one record per token at most
+        const size_t set_bytes = P > 32 ? sizeof(unsigned long long) : sizeof(unsigned);
+        const size_t o_set = tacg_align_up(items * g.W * sizeof(unsigned), 256);
+        const size_t o_rank = o_set + tacg_align_up(nrec * set_bytes, 256);
+        const size_t o_meta = o_rank + tacg_align_up(nrec * sizeof(unsigned), 256);
+        const size_t total = o_meta + tacg_align_up(nrec * sizeof(unsigned), 256);
+        char* sbase = static_cast<char*>(tacg_scratch(ctx, total));
+        if (!sbase) return TACG_ERR_CUDA;
+        c.sp.g = g;
+        c.sp.indices = indices; c.sp.family = family; c.sp.primary = primary; c.sp.replicas = c.rep ? replicas : nullptr;
+        c.sp.rows = reinterpret_cast<unsigned*>(sbase);
+        c.sp.rec.set = sbase + o_set;
+        c.sp.rec.rank = reinterpret_cast<unsigned*>(sbase + o_rank);
+        c.sp.rec.meta = reinterpret_cast<unsigned*>(sbase + o_meta);
+        c.sp.cost = cost_per_token;
+        c.sp.serve = reinterpret_cast<signed char*>(serve);
+        c.cp.g = g;
+        c.cp.indices = indices; c.cp.family = family; c.cp.primary = primary; c.cp.replicas = replicas;
+        c.cp.rows = c.sp.rows; c.cp.rec = c.sp.rec;
+        c.cp.theta = theta; c.cp.rho = rho; c.cp.load_state = load_state;
+        c.cp.load = reinterpret_cast<unsigned long long*>(load);
+        c.cp.comm_span = reinterpret_cast<unsigned long long*>(comm_span);
+        c.cp.comm_remote = reinterpret_cast<unsigned long long*>(comm_remote);
+        c.cp.ntok = reinterpret_cast<unsigned long long*>(ntok);
+        c.cp.cost = cost_per_token;
+        c.cp.serve = reinterpret_cast<signed char*>(serve);
+        c.cp.groups = 1;
         int rc;
-        switch (tacg_pick_kt(k, indices)) {
-            case 2: rc = launch_eval_t<2>(ctx, p); break;
-            case 4: rc = launch_eval_t<4>(ctx, p); break;
-            case 6: rc = launch_eval_t<6>(ctx, p); break;
-            case 8: rc = launch_eval_t<8>(ctx, p); break;
-            default: rc = launch_eval_t<0>(ctx, p); break;
+        {
+            tacg_prof_scope prof(ctx, TACG_PROF_EVAL);
+            switch (kt) {
+                case 2: rc = launch_eval_t<2>(c); break;
+                case 4: rc = launch_eval_t<4>(c); break;
+                case 6: rc = launch_eval_t<6>(c); break;
+                case 8: rc = launch_eval_t<8>(c); break;
+                default: rc = launch_eval_t<0>(c); break;
+            }
         }
         if (rc != TACG_OK) return rc;
-        fin_partial = p.partial;
-        fin_cpl = p.cpl;
+        if (!c.rep) {
+            fin_rows = c.sp.rows;
+            fin_ipl = g.ipl;
+            fin_W = g.W;
+        }
     }
     TACG_CUDA_TRY(ctx, tacg_launch_pdl(fairness_kernel, dim3(L + 1), dim3(1024), 0, ctx->stream,
-                                       reinterpret_cast<unsigned long long*>(load), L, P, fairness, fin_partial, fin_cpl, F,
-                                       rho, load_state, reinterpret_cast<unsigned long long*>(comm_span),
+                                       reinterpret_cast<unsigned long long*>(load), L, P, fairness, fin_rows, fin_ipl, fin_W,
+                                       F, rho, load_state, reinterpret_cast<unsigned long long*>(comm_span),
                                        reinterpret_cast<unsigned long long*>(comm_remote),
                                        reinterpret_cast<unsigned long long*>(ntok)));
     TACG_LAUNCH_CHECK(ctx);
