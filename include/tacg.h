@@ -86,6 +86,17 @@ const char* tacg_version(void);
 int tacg_profile_enable(tacg_ctx* ctx, int on);
 int tacg_profile_read(tacg_ctx* ctx, int slot, double* total_ms, int64_t* launches);
 
+/* Measured denominators for the roofline figures (the int8 tensor peak and the
+ * shared-memory atomic peak are not in MEASURED_PEAKS.json, so the library measures them): runs a
+ * micro-benchmark on every SM of the ctx device (one CTA per SM, a few milliseconds, synchronises the
+ * ctx stream) and returns the throughput per second and per clock and SM (from the kernel's own cycle
+ * counter).  Units: increments for the two atomic cases, integer operations (2 per multiply-add) for
+ * the tensor case.  `which` outside the list: TACG_ERR_SHAPE. */
+#define TACG_PEAK_ATOMS_SPREAD 0 /* shared-memory atomic increments, the 32 lanes of a warp on 32 different banks */
+#define TACG_PEAK_ATOMS_RANDOM 1 /* shared-memory atomic increments on uniformly random words of a 128 KB table */
+#define TACG_PEAK_I8_TENSOR    2 /* tcgen05.mma kind::i8, M=128 N=256 K=32, back to back, s32 accumulator in TMEM */
+int tacg_measure_peak(tacg_ctx* ctx, int which, double* per_second, double* per_clk_sm);
+
 /* S1+S2 -- per-family usage and co-activation counts
  * ("usage vector u ... coactivation matrix A ... frequency of expert pairs selected
  * by the same token", per layer and task family).

@@ -22,10 +22,12 @@ TACG_PATH_AUTO = 0x00
 TACG_PATH_HIST = 0x10
 TACG_PATH_MMA = 0x20
 TACG_PROF_COACT, TACG_PROF_AFFINITY, TACG_PROF_EVAL = 0, 1, 2
+TACG_PEAK_ATOMS_SPREAD, TACG_PEAK_ATOMS_RANDOM, TACG_PEAK_I8_TENSOR = 0, 1, 2
 
 EXPORTS = (
     "tacg_create", "tacg_destroy", "tacg_strerror", "tacg_last_detail", "tacg_last_path",
-    "tacg_launch_count", "tacg_version", "tacg_profile_enable", "tacg_profile_read", "tacg_coact_accumulate", "tacg_affinity_swapgain",
+    "tacg_launch_count", "tacg_version", "tacg_profile_enable", "tacg_profile_read", "tacg_measure_peak",
+    "tacg_coact_accumulate", "tacg_affinity_swapgain",
     "gesr_select", "tacg_eval_placement", "gesr_build_replicas", "tacg_spectral_place", "tacg_family_divergence",
 )
 
@@ -65,6 +67,7 @@ def lib():
         L.tacg_version.restype = C.c_char_p
         L.tacg_profile_enable.argtypes = [vp, i32]
         L.tacg_profile_read.argtypes = [vp, i32, C.POINTER(f64), C.POINTER(i64)]
+        L.tacg_measure_peak.argtypes = [vp, i32, C.POINTER(f64), C.POINTER(f64)]
         L.tacg_coact_accumulate.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, vp, vp, vp, u32]
         L.tacg_affinity_swapgain.argtypes = [vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, f32, f32, f32,
                                              vp, vp, vp, vp]
@@ -148,6 +151,12 @@ class Context:
         ms, n = C.c_double(0.0), C.c_int64(0)
         self.check(lib().tacg_profile_read(self._h, int(slot), C.byref(ms), C.byref(n)), "tacg_profile_read")
         return ms.value, n.value
+
+    def measure_peak(self, which: int):
+        """(units per second, units per clock and SM) of one of the TACG_PEAK_* micro-benchmarks."""
+        a, b = C.c_double(0.0), C.c_double(0.0)
+        self.check(lib().tacg_measure_peak(self._h, int(which), C.byref(a), C.byref(b)), "tacg_measure_peak")
+        return a.value, b.value
 
     def check(self, rc: int, where: str):
         if rc != 0:
