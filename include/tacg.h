@@ -194,7 +194,8 @@ int gesr_build_replicas(tacg_ctx* ctx,
  * exact (sums in increasing expert id, fp64).  labels0 (optional) receives the Stage-1 labels and
  * embed (optional) the embedding; an eigenvector's sign and the basis inside a repeated eigenvalue
  * are not unique, the labels do not depend on them.  TACG_ERR_SHAPE for E > 512, P > min(64, E),
- * E > P*capacity, jitter < 0 or kmeans_iters < 1. */
+ * E > P*capacity, jitter <= 0 (with jitter = 0 an expert that never co-activates would have degree 0 and
+ * D^-1/2 would not exist) or kmeans_iters < 1. */
 int tacg_spectral_place(tacg_ctx* ctx,
                         const float* W,          /* dev [L,E,E] graph of tacg_affinity_swapgain */
                         int L, int E, int P, int capacity,

@@ -88,9 +88,13 @@ def version() -> str:
     return lib().tacg_version().decode()
 
 
-def _ptr(t: Optional[torch.Tensor], dtype=None, name="tensor"):
+def _ptr(t: Optional[torch.Tensor], dtype=None, name="tensor", numel: Optional[int] = None):
+    """Device pointer of a tensor after checking where it lives, its layout, its dtype and (numel given) that it
+    holds at least the elements the C call will touch -- a short tensor would be an out-of-bounds device access."""
     if t is None:
         return None
+    if numel is not None and t.numel() < int(numel):
+        raise ValueError(f"{name} has {t.numel()} elements, the call needs {int(numel)}")
     if not t.is_cuda:
         raise ValueError(f"{name} must be a CUDA tensor (the library has no CPU path)")
     if not t.is_contiguous():
@@ -98,6 +102,12 @@ def _ptr(t: Optional[torch.Tensor], dtype=None, name="tensor"):
     if dtype is not None and t.dtype != dtype:
         raise ValueError(f"{name} must be {dtype}, got {t.dtype}")
     return C.c_void_p(t.data_ptr())
+
+
+def _within_limits(k=1, L=1, E=1, F=1, P=1, r=0, N=0) -> bool:
+    """The ABI limits of include/tacg.h.  Outside them the library itself refuses the call (TACG_ERR_SHAPE) before
+    touching any buffer, so the binding leaves the error to it and checks buffer sizes only inside them."""
+    return 1 <= k <= 16 and L >= 1 and 1 <= E <= 512 and 1 <= F <= 8 and 1 <= P <= 64 and 0 <= r <= 8 and N >= 0
 
 
 class Context:
@@ -162,60 +172,91 @@ class Context:
         if rc != 0:
             raise TacgError(rc, where, self.detail())
 
+    def _enter(self):
+        """The library enqueues on the stream the context was created with; torch allocates (and frees) the caller's
+        tensors on the CURRENT stream.  Using the context under another stream would race silently, so refuse."""
+        if self.stream is not None and torch.cuda.current_stream(self.device) != self.stream:
+            raise ValueError("this tacg Context is bound to another CUDA stream than the current one: create one "
+                             "Context per stream (tacg.Context(device, stream))")
+
     # ---- raw calls: same names and argument order as include/tacg.h ----
     def tacg_coact_accumulate(self, indices, family, N, k, L, E, F, D, Cm, ntok, flags=0) -> int:
+        self._enter()
+        ok = _within_limits(k=k, L=L, E=E, F=F, N=N)
+        n = lambda v: v if ok else None
         return lib().tacg_coact_accumulate(
-            self._h, _ptr(indices, torch.int16, "indices"), _ptr(family, torch.int8, "family"),
-            int(N), int(k), int(L), int(E), int(F), _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"),
-            _ptr(ntok, torch.int64, "ntok"), int(flags))
+            self._h, _ptr(indices, torch.int16, "indices", n(L * N * k)), _ptr(family, torch.int8, "family", n(N)),
+            int(N), int(k), int(L), int(E), int(F), _ptr(D, torch.int32, "D", n(L * F * E)),
+            _ptr(Cm, torch.int32, "C", n(L * F * E * E)), _ptr(ntok, torch.int64, "ntok", n(F)), int(flags))
 
     def tacg_affinity_swapgain(self, D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps,
                                pref, W, aff, gain) -> int:
+        self._enter()
+        ok = _within_limits(L=L, E=E, F=F, P=max(P, 1))
+        n = lambda v: v if ok else None
         return lib().tacg_affinity_swapgain(
-            self._h, _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"), _ptr(ntok, torch.int64, "ntok"),
-            int(L), int(E), int(F), int(P), int(capacity), _ptr(primary, torch.int8, "primary"),
-            float(alpha), float(tau), float(eps), _ptr(pref, torch.float32, "pref"),
-            _ptr(W, torch.float32, "W"), _ptr(aff, torch.float32, "aff"), _ptr(gain, torch.float32, "gain"))
+            self._h, _ptr(D, torch.int32, "D", n(L * F * E)), _ptr(Cm, torch.int32, "C", n(L * F * E * E)),
+            _ptr(ntok, torch.int64, "ntok", n(F)), int(L), int(E), int(F), int(P), int(capacity),
+            _ptr(primary, torch.int8, "primary", n(L * E)), float(alpha), float(tau), float(eps),
+            _ptr(pref, torch.float32, "pref", n(L * E * F)), _ptr(W, torch.float32, "W", n(L * E * E)),
+            _ptr(aff, torch.float32, "aff", n(L * E * P)), _ptr(gain, torch.float32, "gain", n(L * E * E)))
 
     def gesr_build_replicas(self, D, Cm, ntok, L, E, F, P, capacity, primary, alpha, tau, eps, lambda1, lambda2,
                             n_rep, r, replicas, terms) -> int:
+        self._enter()
+        ok = _within_limits(L=L, E=E, F=F, P=P, r=r)
+        n = lambda v: v if ok else None
         return lib().gesr_build_replicas(
-            self._h, _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"), _ptr(ntok, torch.int64, "ntok"),
-            int(L), int(E), int(F), int(P), int(capacity), _ptr(primary, torch.int8, "primary"),
-            float(alpha), float(tau), float(eps), float(lambda1), float(lambda2), int(n_rep), int(r),
-            _ptr(replicas, torch.int8, "replicas"), _ptr(terms, torch.float32, "terms"))
+            self._h, _ptr(D, torch.int32, "D", n(L * F * E)), _ptr(Cm, torch.int32, "C", n(L * F * E * E)),
+            _ptr(ntok, torch.int64, "ntok", n(F)), int(L), int(E), int(F), int(P), int(capacity),
+            _ptr(primary, torch.int8, "primary", n(L * E)), float(alpha), float(tau), float(eps), float(lambda1),
+            float(lambda2), int(n_rep), int(r), _ptr(replicas, torch.int8, "replicas", n(L * E * max(r, 0))),
+            _ptr(terms, torch.float32, "terms", n(L * E * 4)))
 
     def tacg_family_divergence(self, D, Cm, ntok, L, E, F, topk, frob, jaccard) -> int:
+        self._enter()
+        ok = _within_limits(L=L, E=E, F=F)
+        n = lambda v: v if ok else None
         return lib().tacg_family_divergence(
-            self._h, _ptr(D, torch.int32, "D"), _ptr(Cm, torch.int32, "C"), _ptr(ntok, torch.int64, "ntok"),
-            int(L), int(E), int(F), int(topk), _ptr(frob, torch.float32, "frob"), _ptr(jaccard, torch.float32, "jaccard"))
+            self._h, _ptr(D, torch.int32, "D", n(L * F * E)), _ptr(Cm, torch.int32, "C", n(L * F * E * E)),
+            _ptr(ntok, torch.int64, "ntok", n(F)), int(L), int(E), int(F), int(topk),
+            _ptr(frob, torch.float32, "frob", n((L + 1) * F * F)), _ptr(jaccard, torch.float32, "jaccard", n((L + 1) * F * F)))
 
     def tacg_spectral_place(self, W, L, E, P, capacity, jitter, kmeans_iters, labels_in, primary, labels0, embed) -> int:
+        self._enter()
+        ok = _within_limits(L=L, E=E, P=P)
+        n = lambda v: v if ok else None
         return lib().tacg_spectral_place(
-            self._h, _ptr(W, torch.float32, "W"), int(L), int(E), int(P), int(capacity), float(jitter),
-            int(kmeans_iters), _ptr(labels_in, torch.int8, "labels_in"), _ptr(primary, torch.int8, "primary"),
-            _ptr(labels0, torch.int8, "labels0"), _ptr(embed, torch.float64, "embed"))
+            self._h, _ptr(W, torch.float32, "W", n(L * E * E)), int(L), int(E), int(P), int(capacity), float(jitter),
+            int(kmeans_iters), _ptr(labels_in, torch.int8, "labels_in", n(L * E)), _ptr(primary, torch.int8, "primary", n(L * E)),
+            _ptr(labels0, torch.int8, "labels0", n(L * E)), _ptr(embed, torch.float64, "embed", n(L * E * P)))
 
     def gesr_select(self, indices, N, k, L, E, P, primary, replicas, r, load_snapshot, theta,
                     token_offset, serve, flags=0) -> int:
+        self._enter()
+        ok = _within_limits(k=k, L=L, E=E, P=P, r=r, N=N)
+        n = lambda v: v if ok else None
         return lib().gesr_select(
-            self._h, _ptr(indices, torch.int16, "indices"), int(N), int(k), int(L), int(E), int(P),
-            _ptr(primary, torch.int8, "primary"), _ptr(replicas, torch.int8, "replicas"), int(r),
-            _ptr(load_snapshot, torch.float64, "load_snapshot"), float(theta), int(token_offset),
-            _ptr(serve, torch.int8, "serve"), int(flags))
+            self._h, _ptr(indices, torch.int16, "indices", n(L * N * k)), int(N), int(k), int(L), int(E), int(P),
+            _ptr(primary, torch.int8, "primary", n(L * E)), _ptr(replicas, torch.int8, "replicas", n(L * E * max(r, 0))), int(r),
+            _ptr(load_snapshot, torch.float64, "load_snapshot", n(L * P)), float(theta), int(token_offset),
+            _ptr(serve, torch.int8, "serve", n(L * N * k)), int(flags))
 
     def tacg_eval_placement(self, indices, family, N, k, L, E, F, P, primary, replicas, r, theta, rho,
                             microbatch, token_offset, load_state, load, comm_span, comm_remote, ntok,
                             fairness, cost_per_token, serve, flags=0) -> int:
+        self._enter()
+        ok = _within_limits(k=k, L=L, E=E, F=F, P=P, r=r, N=N)
+        n = lambda v: v if ok else None
         return lib().tacg_eval_placement(
-            self._h, _ptr(indices, torch.int16, "indices"), _ptr(family, torch.int8, "family"),
-            int(N), int(k), int(L), int(E), int(F), int(P), _ptr(primary, torch.int8, "primary"),
-            _ptr(replicas, torch.int8, "replicas"), int(r), float(theta), float(rho), int(microbatch),
-            int(token_offset), _ptr(load_state, torch.float64, "load_state"),
-            _ptr(load, torch.int64, "load"), _ptr(comm_span, torch.int64, "comm_span"),
-            _ptr(comm_remote, torch.int64, "comm_remote"), _ptr(ntok, torch.int64, "ntok"),
-            _ptr(fairness, torch.float32, "fairness"), _ptr(cost_per_token, torch.uint8, "cost_per_token"),
-            _ptr(serve, torch.int8, "serve"), int(flags))
+            self._h, _ptr(indices, torch.int16, "indices", n(L * N * k)), _ptr(family, torch.int8, "family", n(N)),
+            int(N), int(k), int(L), int(E), int(F), int(P), _ptr(primary, torch.int8, "primary", n(L * E)),
+            _ptr(replicas, torch.int8, "replicas", n(L * E * max(r, 0))), int(r), float(theta), float(rho), int(microbatch),
+            int(token_offset), _ptr(load_state, torch.float64, "load_state", n(L * P)),
+            _ptr(load, torch.int64, "load", n(L * P)), _ptr(comm_span, torch.int64, "comm_span", n(L * F)),
+            _ptr(comm_remote, torch.int64, "comm_remote", n(L * F)), _ptr(ntok, torch.int64, "ntok", n(F)),
+            _ptr(fairness, torch.float32, "fairness", n((L + 1) * 3)), _ptr(cost_per_token, torch.uint8, "cost_per_token", n(L * N)),
+            _ptr(serve, torch.int8, "serve", n(L * N * k)), int(flags))
 
 
 # ---- convenience wrappers: allocate outputs with torch, call, return a dict ----

@@ -4,8 +4,9 @@
 //   coact_hist_kernel      persistent, one CTA per SM.  A CTA owns a contiguous range of
 //                          (layer, token-chunk) items and keeps a PRIVATE strict-upper-triangular
 //                          uint32 pair histogram in shared memory (all F families when they fit,
-//                          else one family per CTA with the tokens of that family compacted through
-//                          a per-warp queue).  Four bank-spread copies of the bins when they fit; for
+//                          else one family per CTA: the F CTAs of a group walk the same token range at
+//                          the same time, each through its family's token list, which three small
+//                          kernels build once per call -- the labels are shared by all layers).  Four bank-spread copies of the bins when they fit; for
 //                          k = 8 a small token-set table short-cuts repeated expert sets.  The
 //                          histogram is written once per (CTA, layer) to a scratch slot.
 //   coact_finalize_kernel  grid (E/8, L*F), one warp per output row: sums the slots of the layer (L2
@@ -28,7 +29,7 @@ constexpr int kThreads = 1024;           // one CTA per SM
 constexpr int kWarps = kThreads / 32;
 constexpr int kBatch = 4;                 // tokens per thread whose loads are issued together
 constexpr int kRun = 4;                   // items (of kThreads tokens) walked together
-constexpr int kQueue = 160;              // per-warp token queue of the family-filter mode (<= 31 + 128 entries)
+constexpr int kRunFam = 16;               // the same in family mode, where a CTA takes one token in F
 
 struct HistParams {
     const int16_t* indices;
@@ -46,6 +47,8 @@ struct HistParams {
     int slot_words;     // Fs*(tri+E+1) rounded up to 4
     int memo_off;       // byte offset of the token-set table in shared memory, 0 = no table
     int memo_ts;        // table entries per family (power of two)
+    const unsigned* perm;   // family mode: [F][N] tokens of each family in increasing order
+    const unsigned* boff;   // family mode: [F][cps+1] tokens of family f before item (block of `chunk` tokens) b
 };
 
 // R(i) + j is the bin of the pair i < j in a row-major strict upper triangle of an E x E matrix:
@@ -184,7 +187,6 @@ __device__ __forceinline__ void count_token(const int16_t* __restrict__ row, int
 }
 
 // smem layout (words): [Fs][tri] pair bins | [Fs][E] corr | [Fs] ntok (layer 0 only) | pad to slot_words
-//                      | (filter mode) per-warp queues of token offsets
 // CP (non-filter mode only): bank-spread copies of the pair bins, one per quarter warp.
 template <int KT, bool FILTER, int CP>
 __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParams p) {
@@ -217,12 +219,83 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
         m.mask = (unsigned)(p.memo_ts - 1);
         return m;
     };
+    // Tokens that miss the token-set table diverge from those that hit it (28 increments against one), so their
+    // sorted sets wait in a per-warp queue and are expanded 32 at a time, every lane busy.
+    const int lane = tid & 31;
+    unsigned long long* qkey = reinterpret_cast<unsigned long long*>(mcnt + mentries + (mentries & 1)) + (tid >> 5) * 64;
+    unsigned char* qfam = reinterpret_cast<unsigned char*>(
+                              reinterpret_cast<unsigned long long*>(mcnt + mentries + (mentries & 1)) + (kThreads / 32) * 64) +
+                          (tid >> 5) * 64;
+    int qn = 0;                         // entries waiting in this warp's queue (warp-uniform)
+    // pair increments of one sorted set (ids as bytes of `key`), `c` times
+    auto expand_key = [&](unsigned long long key, unsigned c, unsigned* hf) {
+        if constexpr (KT >= 2) {
+            int s[KT];
+#pragma unroll
+            for (int a = 0; a < KT; ++a) s[a] = (int)((key >> (8 * a)) & 0xffull);
+#pragma unroll
+            for (int a = 0; a + 1 < KT; ++a) {
+                unsigned* rowp = hf + tri_row(s[a], p.E) * CP;
+#pragma unroll
+                for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b] * CP, c);
+            }
+        }
+    };
+    // one token (live = it exists and is not padding) of family slot fl; every lane of the warp calls this together
+    auto process = [&](bool live, const unsigned (&w)[KT >= 2 ? KT / 2 : 1], int fl) {
+        if constexpr (KT >= 2) {
+            if (!mentries) {
+                if (live) count_packed<KT, CP>(w, p.E, hist_lane + (size_t)fl * p.tri * CP, corr + fl * p.E);
+                return;
+            }
+            unsigned long long key = 0ull;
+            bool miss = false;
+            if (live) {
+                int e[KT], s[KT];
+#pragma unroll
+                for (int i = 0; i < KT / 2; ++i) {
+                    e[2 * i] = (int)(short)(w[i] & 0xffffu);
+                    e[2 * i + 1] = (int)w[i] >> 16;
+                }
+#pragma unroll
+                for (int a = 0; a < KT; ++a) s[a] = e[a];
+                sort_ids<KT>(s);
+                bool fast = s[0] >= 0 && s[KT - 1] < p.E;
+#pragma unroll
+                for (int a = 0; a + 1 < KT; ++a) fast = fast && (s[a] != s[a + 1]);
+                if (fast) {
+#pragma unroll
+                    for (int a = 0; a < KT; ++a) key |= (unsigned long long)(unsigned)s[a] << (8 * a);
+                    const MemoTable memo = memo_of(fl);
+                    const unsigned h = (unsigned)((key * 0x9E3779B97F4A7C15ull) >> 40) & memo.mask;
+                    // plain read first: once a set is in the table a hit costs one load and one increment
+                    unsigned long long prev = *reinterpret_cast<volatile unsigned long long*>(memo.keys + h);
+                    if (prev == 0ull) prev = atomicCAS(memo.keys + h, 0ull, key);
+                    if (prev == 0ull || prev == key) atomicAdd(memo.cnt + h, 1u);
+                    else miss = true;
+                } else {
+                    slow_token<KT, CP>(e, KT, p.E, hist_lane + (size_t)fl * p.tri * CP, corr + fl * p.E);
+                }
+            }
+            const unsigned mm = __ballot_sync(0xffffffffu, miss);
+            if (mm) {
+                if (miss) {
+                    const int pos = qn + __popc(mm & ((1u << lane) - 1u));
+                    qkey[pos] = key;
+                    qfam[pos] = (unsigned char)fl;
+                }
+                qn += __popc(mm);
+                __syncwarp();
+                if (qn >= 32) {
+                    qn -= 32;
+                    expand_key(qkey[qn + lane], 1u, hist_lane + (size_t)qfam[qn + lane] * p.tri * CP);
+                    __syncwarp();
+                }
+            }
+        }
+    };
     __syncthreads();
 
-    // filter mode: per-warp queue of matching token offsets (relative to the layer's token 0)
-    unsigned* wq = hsm + p.slot_words + (tid >> 5) * kQueue;
-    int qn = 0;                         // warp-uniform
-    const int lane = tid & 31;
 
     // Items are walked in runs of up to kRun consecutive items of one layer, so that a thread has
     // kBatch tokens in flight while group boundaries stay at the finer item granularity.
@@ -235,27 +308,15 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
         if (item == hi) l = -1;
         if (l != layer) {
             const int16_t* lbase = p.indices + (size_t)layer * (size_t)p.N * k;
-            if (FILTER) {               // drain the partial queue of this layer
-                if (lane < qn) count_token<KT>(lbase + (size_t)wq[lane] * k, k, p.E, hsm, corr, memo_of(0));
-                qn = 0;
-            }
+            if (lane < qn) expand_key(qkey[lane], 1u, hist_lane + (size_t)qfam[lane] * p.tri * CP);   // the rest of the queue
+            qn = 0;
             __syncthreads();
             if constexpr (KT >= 2) {
                 // expand the token-set table: count x every pair of the key
                 for (int i = tid; i < mentries; i += kThreads) {
                     const unsigned c = mcnt[i];
                     if (c) {
-                        const unsigned long long key = mkeys[i];
-                        unsigned* hf = hsm + (size_t)(i / p.memo_ts) * p.tri * CP + (CP > 1 ? (tid & (CP - 1)) : 0);
-                        int s[KT];
-#pragma unroll
-                        for (int a = 0; a < KT; ++a) s[a] = (int)((key >> (8 * a)) & 0xffull);
-#pragma unroll
-                        for (int a = 0; a + 1 < KT; ++a) {
-                            unsigned* rowp = hf + tri_row(s[a], p.E) * CP;
-#pragma unroll
-                            for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b] * CP, c);
-                        }
+                        expand_key(mkeys[i], c, hsm + (size_t)(i / p.memo_ts) * p.tri * CP + (CP > 1 ? (tid & (CP - 1)) : 0));
                         mkeys[i] = 0ull;
                         mcnt[i] = 0u;
                     }
@@ -286,7 +347,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             if (l < 0) break;
             layer = l;
         }
-        const int run = (int)min((long long)min(kRun, p.cps - ci), hi - item);
+        const int run = (int)min((long long)min(FILTER ? kRunFam : kRun, p.cps - ci), hi - item);
         const long long t0 = (long long)ci * p.chunk;
         const long long t1 = min(p.N, t0 + (long long)run * p.chunk);
         ci += run;
@@ -295,7 +356,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
         if (!FILTER) {
             if constexpr (KT >= 2) {
                 // kBatch tokens per thread with all their loads in flight before the first increment
-                for (long long tb = t0 + tid; tb < t1; tb += (long long)kThreads * kBatch) {
+                for (long long tb = t0 + tid; tb - lane < t1; tb += (long long)kThreads * kBatch) {   // warp-uniform trip count
                     int f[kBatch];
                     unsigned w[kBatch][KT / 2];
 #pragma unroll
@@ -309,9 +370,9 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
                     }
 #pragma unroll
                     for (int u = 0; u < kBatch; ++u) {
-                        if ((unsigned)f[u] >= (unsigned)p.F) continue;      // padding token / past the end
-                        if (l == 0) atomicAdd(&sntok[f[u]], 1u);
-                        count_packed<KT, CP>(w[u], p.E, hist_lane + (size_t)f[u] * p.tri * CP, corr + f[u] * p.E, memo_of(f[u]));
+                        const bool live = (unsigned)f[u] < (unsigned)p.F;    // not a padding token, not past the end
+                        if (live && l == 0) atomicAdd(&sntok[f[u]], 1u);
+                        process(live, w[u], live ? f[u] : 0);
                     }
                 }
             } else {
@@ -323,34 +384,28 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
                 }
             }
         } else {
-            // each thread scans 4 consecutive tokens per step; a warp covers 128
-            for (long long tb = t0 + (long long)(tid >> 5) * 128; tb < t1; tb += (long long)kWarps * 128) {
-                const long long ta = tb + lane * 4;
-                unsigned m = 0;
+            // family mode: the tokens of family fg among [t0, t1) are a contiguous piece of the family's list
+            const int b0 = ci - run;
+            const unsigned* bo = p.boff + (size_t)fg * (p.cps + 1);
+            const unsigned j0 = bo[b0], j1 = bo[b0 + run];
+            const unsigned* __restrict__ list = p.perm + (size_t)fg * (size_t)p.N;
+            if (l == 0 && tid == 0) sntok[0] += j1 - j0;
+            if constexpr (KT >= 2) {
+                for (unsigned jb = j0 + tid; jb - lane < j1; jb += kThreads * kBatch) {     // warp-uniform trip count
+                    unsigned w[kBatch][KT / 2];
+                    bool live[kBatch];
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (ta + u < t1 && (int)p.family[ta + u] == fg) m |= 1u << u;
-                const int c = __popc(m);
-                int inc = c;            // inclusive warp scan
+                    for (int u = 0; u < kBatch; ++u) {
+                        const unsigned j = jb + u * kThreads;
+                        live[u] = j < j1;
+                        if (live[u]) load_raw<KT>(lbase + (size_t)__ldg(list + j) * KT, w[u]);
+                    }
 #pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const int v = __shfl_up_sync(0xffffffffu, inc, d);
-                    if (lane >= d) inc += v;
+                    for (int u = 0; u < kBatch; ++u) process(live[u], w[u], 0);
                 }
-                const int total = __shfl_sync(0xffffffffu, inc, 31);
-                int pos = qn + inc - c;
-#pragma unroll
-                for (int u = 0; u < 4; ++u)
-                    if (m & (1u << u)) wq[pos++] = (unsigned)(ta + u);
-                qn += total;
-                if (l == 0 && lane == 0 && total) atomicAdd(&sntok[0], (unsigned)total);
-                __syncwarp();
-                while (qn >= 32) {
-                    qn -= 32;
-                    const unsigned t = wq[qn + lane];
-                    count_token<KT>(lbase + (size_t)t * k, k, p.E, hsm, corr, memo_of(0));
-                }
-                __syncwarp();
+            } else {
+                for (unsigned j = j0 + tid; j < j1; j += kThreads)
+                    count_token<KT>(lbase + (size_t)__ldg(list + j) * k, k, p.E, hsm, corr);
             }
         }
     }
@@ -424,6 +479,77 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
     }
 }
 
+// ---- family mode: the tokens of every family as an increasing list, with the list position of every block of
+// kThreads tokens (= one work item), built once per call in three small launches.
+// (1) boff[f][b] = tokens of family f in block b
+__global__ void __launch_bounds__(kThreads)
+part_count_kernel(const int8_t* __restrict__ family, long long N, int F, int nb, unsigned* __restrict__ boff) {
+    tacg_pdl_prologue();
+    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const int f = t < N ? (int)family[t] : -1;
+    for (int ff = 0; ff < F; ++ff) {
+        const int c = __syncthreads_count(f == ff);
+        if (threadIdx.x == 0) boff[(size_t)ff * (nb + 1) + blockIdx.x] = (unsigned)c;
+    }
+}
+
+// (2) in place: boff[f][b] = tokens of family f before block b, boff[f][nb] = all of them; one CTA per family
+__global__ void __launch_bounds__(kThreads) part_scan_kernel(int nb, unsigned* __restrict__ boff) {
+    tacg_pdl_prologue();
+    __shared__ unsigned tsum[kThreads];
+    unsigned* row = boff + (size_t)blockIdx.x * (nb + 1);
+    const int per = (nb + kThreads - 1) / kThreads;
+    const int b0 = min(nb, (int)threadIdx.x * per), b1 = min(nb, b0 + per);
+    unsigned s = 0;
+    for (int b = b0; b < b1; ++b) s += row[b];
+    tsum[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {                        // exclusive scan of the 1024 thread sums by one warp
+        unsigned carry = 0;
+        for (int c = 0; c < kThreads; c += 32) {
+            const unsigned v = tsum[c + threadIdx.x];
+            unsigned inc = v;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned u = __shfl_up_sync(0xffffffffu, inc, d);
+                if ((int)threadIdx.x >= d) inc += u;
+            }
+            tsum[c + threadIdx.x] = carry + inc - v;
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+        if (threadIdx.x == 0) row[nb] = carry;
+    }
+    __syncthreads();
+    unsigned run = tsum[threadIdx.x];
+    for (int b = b0; b < b1; ++b) {
+        const unsigned c = row[b];
+        row[b] = run;
+        run += c;
+    }
+}
+
+// (3) perm[f][boff[f][b] + rank of the token among its family's tokens of block b] = token
+__global__ void __launch_bounds__(kThreads)
+part_scatter_kernel(const int8_t* __restrict__ family, long long N, int F, int nb, const unsigned* __restrict__ boff,
+                    unsigned* __restrict__ perm) {
+    tacg_pdl_prologue();
+    __shared__ unsigned wc[8][kWarps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
+    const int f = t < N ? (int)family[t] : -1;
+    unsigned rank = 0;
+    for (int ff = 0; ff < F; ++ff) {
+        const unsigned b = __ballot_sync(0xffffffffu, f == ff);
+        if (lane == 0) wc[ff][warp] = __popc(b);
+        if (f == ff) rank = __popc(b & ((1u << lane) - 1u));
+    }
+    __syncthreads();
+    if ((unsigned)f < (unsigned)F) {
+        for (int w = 0; w < warp; ++w) rank += wc[f][w];
+        perm[(size_t)f * (size_t)N + boff[(size_t)f * (nb + 1) + blockIdx.x] + rank] = (unsigned)t;
+    }
+}
+
 // Fallback: global atomics on D and C (any E <= 512).  The caller zeroes and counts ntok.
 __global__ void __launch_bounds__(512)
 coact_global_kernel(const int16_t* __restrict__ indices, const int8_t* __restrict__ family, long long N, int k, int L,
@@ -481,10 +607,9 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     const size_t limit = (size_t)ctx->smem_optin;
     const size_t all_words = tacg_align_up((size_t)F * (p.tri + E + 1), 4);
     const size_t one_words = tacg_align_up((size_t)(p.tri + E + 1), 4);
-    const size_t queue_bytes = sizeof(unsigned) * kWarps * kQueue;
     bool filter;
     if (all_words * 4 <= limit) filter = false;
-    else if (one_words * 4 + queue_bytes <= limit && N < (1ll << 32)) filter = true;
+    else if (one_words * 4 <= limit && N < (1ll << 32)) filter = true;
     else {
         // neither layout fits: global atomics
         if (zero_first) {
@@ -511,12 +636,19 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     const long long min_items = max(2ll, (long long)p.slot_words * 4 / 12800);
     p.groups = (int)max(1ll, min((long long)(ctx->sm_count / p.nfg), max(1ll, p.T / min_items)));
     const size_t slots = (size_t)(p.groups + L - 1) * p.nfg;
-    p.scratch = static_cast<unsigned*>(tacg_scratch(ctx, slots * p.slot_words * sizeof(unsigned)));
-    if (!p.scratch) return TACG_ERR_CUDA;
+    // family mode: the family token lists and their block offsets live behind the slots
+    const size_t o_perm = tacg_align_up(slots * p.slot_words * sizeof(unsigned), 256);
+    const size_t o_boff = o_perm + (filter ? tacg_align_up(sizeof(unsigned) * (size_t)F * (size_t)N, 256) : 0);
+    const size_t total = o_boff + (filter ? sizeof(unsigned) * (size_t)F * ((size_t)p.cps + 1) : 0);
+    char* sbase = static_cast<char*>(tacg_scratch(ctx, total));
+    if (!sbase) return TACG_ERR_CUDA;
+    p.scratch = reinterpret_cast<unsigned*>(sbase);
+    p.perm = reinterpret_cast<unsigned*>(sbase + o_perm);
+    p.boff = reinterpret_cast<unsigned*>(sbase + o_boff);
     // four bank-spread copies of the pair bins when they fit (non-filter mode)
     const size_t bins_bytes = sizeof(unsigned) * (size_t)p.Fs * p.tri;
     const bool copies = !filter && (size_t)p.slot_words * 4 + 3 * bins_bytes + 16 <= limit;
-    size_t smem = (size_t)p.slot_words * 4 + (filter ? queue_bytes : 0) + (copies ? 3 * bins_bytes + 16 : 0);
+    size_t smem = (size_t)p.slot_words * 4 + (copies ? 3 * bins_bytes + 16 : 0);
     // token-set table: ids as bytes (E <= 256), packed loaders, 1024 entries per family.  Measured on
     // B200: it pays at k = 8 (28 increments saved per hit: config 3 706 -> 516 us) and loses at k = 6
     // (15 saved, the 64-bit CAS and the key packing cost more: config 2 71 -> 77 us), so k = 8 only.
@@ -524,7 +656,8 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     p.memo_ts = 1024;
     if (E <= 256 && tacg_pick_kt(k, indices) == 8) {
         const size_t off = tacg_align_up(smem, 16);
-        const size_t need = (size_t)p.Fs * p.memo_ts * (sizeof(unsigned long long) + sizeof(unsigned));
+        const size_t need = (size_t)p.Fs * p.memo_ts * (sizeof(unsigned long long) + sizeof(unsigned)) + 8 +
+                            (size_t)(kThreads / 32) * 64 * (sizeof(unsigned long long) + 1);     // table + the warps' miss queues
         if (off + need <= limit) {
             p.memo_off = (int)off;
             smem = off + need;
@@ -532,6 +665,18 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     }
     const int grid = p.groups * p.nfg;
     tacg_prof_scope prof(ctx, TACG_PROF_COACT);
+    if (filter) {
+        unsigned* perm = const_cast<unsigned*>(p.perm);
+        unsigned* boff = const_cast<unsigned*>(p.boff);
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_count_kernel, dim3(p.cps), dim3(kThreads), 0, ctx->stream, family,
+                                           (long long)N, F, p.cps, boff));
+        TACG_LAUNCH_CHECK(ctx);
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_scan_kernel, dim3(F), dim3(kThreads), 0, ctx->stream, p.cps, boff));
+        TACG_LAUNCH_CHECK(ctx);
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_scatter_kernel, dim3(p.cps), dim3(kThreads), 0, ctx->stream, family,
+                                           (long long)N, F, p.cps, (const unsigned*)boff, perm));
+        TACG_LAUNCH_CHECK(ctx);
+    }
     int rc = filter ? launch_hist_k<true, 1>(ctx, p, smem, grid)
                     : (copies ? launch_hist_k<false, 4>(ctx, p, smem, grid) : launch_hist_k<false, 1>(ctx, p, smem, grid));
     if (rc != TACG_OK) return rc;

@@ -50,6 +50,7 @@ constexpr int kEvalThreads = 512;    // eval_scan_kernel, select_kernel
 constexpr int kEvalBatch = 4;        // tokens per thread with their loads in flight together
 constexpr int kSlice = 8192;         // most tokens of a scan item (13-bit offsets in the records, 16 per thread)
 constexpr int kChainThreads = 1024;
+constexpr long long kSeqBelow = 1024; // micro-batches shorter than this go to the one-warp-per-layer kernel
 constexpr int kCandStride = 12;      // bytes per expert in the candidate table: [0] = count, [1..9] = partitions
 constexpr unsigned kRepFlag = 0x80u; // ptab bit: the expert has at least one replica
 constexpr unsigned kBadFlag = 0x40u; // ptab bit: not an expert (empty slot, id outside [0,E))
@@ -949,6 +950,128 @@ __global__ void __launch_bounds__(1024) fairness_kernel(unsigned long long* __re
     }
 }
 
+// The literal Eq. 15 (the load state decays after EVERY token) and any other short
+// micro-batch: one warp per layer walks the micro-batches in order, lanes over the tokens of a micro-batch,
+// the whole state in the warp's shared memory.  No other warp is ever waited for, so a trace of a million
+// tokens per layer at B = 1 is a second of work instead of a million grid barriers.
+struct SeqParams {
+    EvalGeom g;
+    const int16_t* indices;
+    const int8_t* family;
+    const int8_t* primary;
+    const int8_t* replicas;
+    float theta;
+    double rho;
+    double* load_state;
+    unsigned long long* load;
+    unsigned long long* comm_span;
+    unsigned long long* comm_remote;
+    unsigned long long* ntok;
+    unsigned char* cost;
+    signed char* serve;
+};
+
+template <typename M>
+__global__ void __launch_bounds__(32) eval_seq_kernel(const SeqParams p) {
+    tacg_pdl_prologue();
+    extern __shared__ __align__(16) unsigned char qsm[];
+    const EvalGeom& g = p.g;
+    const int P = g.P, E = g.E, F = g.F, r = g.r, k = g.k;
+    LayerTables T;
+    size_t off = 0;
+    T.S = reinterpret_cast<double*>(qsm + off);            off += 64 * sizeof(double);
+    double* Ls = reinterpret_cast<double*>(qsm + off);     off += 64 * sizeof(double);
+    unsigned long long* ltot = reinterpret_cast<unsigned long long*>(qsm + off);   off += 64 * sizeof(unsigned long long);
+    unsigned long long* comm = reinterpret_cast<unsigned long long*>(qsm + off);   off += 24 * sizeof(unsigned long long);
+    unsigned* cnt = reinterpret_cast<unsigned*>(qsm + off);                         off += 64 * sizeof(unsigned);
+    unsigned short* replist = reinterpret_cast<unsigned short*>(qsm + off);         off += ((size_t)E * 2 + 15) & ~(size_t)15;
+    T.ptab = qsm + off;                                    off += kPtab + 12;
+    T.cand = qsm + off;                                    off += ((size_t)E * kCandStride + 15) & ~(size_t)15;
+    T.rep = reinterpret_cast<signed char*>(qsm + off);
+    __shared__ unsigned long long feas_s;
+    __shared__ int nrep_s;
+    const int lane = threadIdx.x;
+    const int layer = blockIdx.x;
+    load_ptab(E, r, p.primary + (size_t)layer * E, p.replicas + (size_t)layer * E * r, T.ptab, T.rep);
+    for (int m = lane; m < 64; m += 32) {
+        Ls[m] = (p.load_state && m < P) ? p.load_state[(size_t)layer * P + m] : 0.0;
+        ltot[m] = 0ull;
+        cnt[m] = 0u;
+    }
+    if (lane < 24) comm[lane] = 0ull;
+    if (lane == 0) nrep_s = 0;
+    __syncwarp();
+    for (int e = lane; e < E; e += 32)
+        if (T.ptab[e] & kRepFlag) replist[atomicAdd(&nrep_s, 1)] = (unsigned short)e;
+    __syncwarp();
+    const int nrep = nrep_s;
+    const int16_t* base = p.indices + (size_t)layer * (size_t)g.N * (size_t)k;
+    unsigned long long span[8] = {0, 0, 0, 0, 0, 0, 0, 0}, remote[8] = {0, 0, 0, 0, 0, 0, 0, 0}, seen[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (long long mb = 0; mb < g.nmb; ++mb) {
+        // steps 1-3: snapshot, guard, candidate tables
+        for (int m = lane; m < 64; m += 32) T.S[m] = Ls[m];
+        __syncwarp();
+        if (lane == 0) feas_s = load_guard(T.S, P, p.theta);
+        __syncwarp();
+        const unsigned long long feas = feas_s;
+        for (int i = lane; i < nrep; i += 32) build_candidate((int)replist[i], r, T, feas, T.cand + (int)replist[i] * kCandStride);
+        __syncwarp();
+        // step 4: the tokens of the micro-batch, one per lane
+        const long long t0 = mb * g.B, t1 = min(g.N, t0 + g.B);
+        for (long long t = t0 + lane; t < t1; t += 32) {
+            const int fq = p.family[t];
+            if ((unsigned)fq >= (unsigned)F) {
+                if (p.cost) p.cost[(size_t)layer * g.N + t] = 0;
+                if (p.serve)
+                    for (int j = 0; j < k; ++j) p.serve[((size_t)layer * g.N + t) * k + j] = -1;
+                continue;
+            }
+            int e[16], sv[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) e[j] = (j < k) ? (int)__ldg(base + (size_t)t * k + j) : -1;
+            const int home = (int)((g.token_offset + t) % P);
+            const M R = serve_token<16, M>(e, k, E, home, T, sv);
+#pragma unroll
+            for (int j = 0; j < 16; ++j)
+                if (j < k && sv[j] >= 0) atomicAdd(&cnt[sv[j]], 1u);
+            const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~((M)1 << home));
+            if (p.cost) p.cost[(size_t)layer * g.N + t] = (unsigned char)rem;
+            if (p.serve)
+                for (int j = 0; j < k; ++j) p.serve[((size_t)layer * g.N + t) * k + j] = (signed char)sv[j];
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+                if (q == fq) { span[q] += (unsigned)max(0, nR - 1); remote[q] += (unsigned)rem; seen[q] += 1; }
+        }
+        __syncwarp();
+        // step 5: Eq. 15
+        for (int m = lane; m < P; m += 32) {
+            const unsigned d = cnt[m];
+            cnt[m] = 0u;
+            Ls[m] = __dadd_rn(__dmul_rn(p.rho, Ls[m]), (double)d);   // no FMA (Q19)
+            ltot[m] += d;
+        }
+        __syncwarp();
+    }
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        if (q < F) {
+            atomicAdd(&comm[q], span[q]);
+            atomicAdd(&comm[8 + q], remote[q]);
+            atomicAdd(&comm[16 + q], seen[q]);
+        }
+    }
+    __syncwarp();
+    for (int m = lane; m < P; m += 32) {
+        p.load[(size_t)layer * P + m] = ltot[m];
+        if (p.load_state) p.load_state[(size_t)layer * P + m] = Ls[m];
+    }
+    if (lane < F) {
+        p.comm_span[(size_t)layer * F + lane] = comm[lane];
+        p.comm_remote[(size_t)layer * F + lane] = comm[8 + lane];
+        if (layer == 0) p.ntok[lane] = comm[16 + lane];
+    }
+}
+
 size_t select_smem_bytes(int E, int r) {
     return 64 * sizeof(double) + kPtab + (((size_t)E * kCandStride + 15) & ~(size_t)15) +
            (((size_t)E * (r > 0 ? r : 1) + 15) & ~(size_t)15);
@@ -1128,6 +1251,32 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         g.N = N; g.k = k; g.L = L; g.E = E; g.F = F; g.P = P; g.r = c.rep ? r : 0;
         g.B = (!c.rep || microbatch <= 0 || microbatch > N) ? N : microbatch;
         g.nmb = (N + g.B - 1) / g.B;
+        g.k = k; g.token_offset = token_offset;
+        if (c.rep && g.B < kSeqBelow) {
+            // short micro-batches (down to the literal per-token Eq. 15): one warp per layer, nothing to exchange
+            SeqParams q;
+            g.spm = 1; g.slice = 512; g.ipl = g.nmb; g.W = 0;
+            q.g = g;
+            q.indices = indices; q.family = family; q.primary = primary; q.replicas = replicas;
+            q.theta = theta; q.rho = rho; q.load_state = load_state;
+            q.load = reinterpret_cast<unsigned long long*>(load);
+            q.comm_span = reinterpret_cast<unsigned long long*>(comm_span);
+            q.comm_remote = reinterpret_cast<unsigned long long*>(comm_remote);
+            q.ntok = reinterpret_cast<unsigned long long*>(ntok);
+            q.cost = cost_per_token;
+            q.serve = reinterpret_cast<signed char*>(serve);
+            const size_t smem = 64 * 8 * 3 + 24 * 8 + 64 * 4 + (((size_t)E * 2 + 15) & ~(size_t)15) + kPtab + 12 +
+                                (((size_t)E * kCandStride + 15) & ~(size_t)15) + (((size_t)E * r + 15) & ~(size_t)15);
+            tacg_prof_scope prof(ctx, TACG_PROF_EVAL);
+            if (P > 32) {
+                TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(eval_seq_kernel<unsigned long long>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                TACG_CUDA_TRY(ctx, tacg_launch_pdl(eval_seq_kernel<unsigned long long>, dim3(L), dim3(32), smem, ctx->stream, q));
+            } else {
+                TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(eval_seq_kernel<unsigned>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                TACG_CUDA_TRY(ctx, tacg_launch_pdl(eval_seq_kernel<unsigned>, dim3(L), dim3(32), smem, ctx->stream, q));
+            }
+            TACG_LAUNCH_CHECK(ctx);
+        } else {
         // slice: as large as the record format allows (the per-item epilogue is amortised over 16 tokens per
         // thread); smaller only when the whole trace would otherwise give the scan grid fewer than two items per CTA
         long long slice = kSlice;
@@ -1185,6 +1334,7 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
             fin_rows = c.sp.rows;
             fin_ipl = g.ipl;
             fin_W = g.W;
+        }
         }
     }
     TACG_CUDA_TRY(ctx, tacg_launch_pdl(fairness_kernel, dim3(L + 1), dim3(1024), 0, ctx->stream,

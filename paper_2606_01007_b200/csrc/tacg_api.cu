@@ -227,7 +227,8 @@ int tacg_spectral_place(tacg_ctx* ctx, const float* W, int L, int E, int P, int 
     if (!W || !primary) return fail(ctx, TACG_ERR_NULL, "spectral_place: NULL pointer");
     if (P < 1 || P > 64 || P > E || capacity < 1 || (int64_t)E > (int64_t)P * capacity)
         return fail(ctx, TACG_ERR_SHAPE, "spectral_place: P outside [1, min(64,E)] or E > P*capacity");
-    if (!(jitter >= 0.0) || kmeans_iters < 1) return fail(ctx, TACG_ERR_SHAPE, "spectral_place: jitter < 0 or kmeans_iters < 1");
+    // jitter = 0 would give an expert that never co-activates degree 0 and a NaN in D^-1/2 A D^-1/2
+    if (!(jitter > 0.0) || kmeans_iters < 1) return fail(ctx, TACG_ERR_SHAPE, "spectral_place: jitter <= 0 or kmeans_iters < 1");
     TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     return tacg_launch_spectral(ctx, W, L, E, P, capacity, jitter, kmeans_iters, labels_in, primary, labels0, embed);
 }

@@ -3,8 +3,7 @@
 These are the consumers of the hot path, not part of it: a capacity-preserving best-swap
 local search driven by the GPU swap gains (the "only if the move improves" test of
 PAPER.md:124 applied to every pair), the whole offline stage of the method chained on the device
-(`tacg_gesr_placement`: counts -> graph -> spectral-then-repair -> replicas), and the GESR replica table with
-the canonical lambda1 = lambda2 = 0 (centrality only).  All
+(`tacg_gesr_placement`: counts -> graph -> spectral-then-repair -> replicas by gesr_build_replicas).  All
 E x E arithmetic stays in tacg_affinity_swapgain; the host only takes argmaxes.
 """
 from __future__ import annotations
@@ -60,30 +59,6 @@ def local_search(ctx: "_b.Context", D, Cm, ntok, P: int, capacity: int, alpha: f
         if not any_swap:
             break
     return primary, swaps
-
-
-def replica_table(ctx: "_b.Context", D, Cm, ntok, P: int, capacity: int, primary: np.ndarray, n_rep: int, r: int,
-                  alpha: float = 0.25, tau: float = 1.0, eps: float = 1e-6) -> np.ndarray:
-    """GESR offline step with lambda1 = lambda2 = 0: generic experts = top n_rep by centrality
-    (row sum of the pooled graph; Ahat = W at alpha = 0 is Abar up to a positive factor), their
-    secondaries = the r non-primary partitions with the largest affinity (Eq. 12).  Ties -> lower id."""
-    L, F, E = D.shape
-    rep = np.full((L, E, max(r, 0)), -1, dtype=np.int8)
-    if r <= 0 or n_rep <= 0:
-        return rep
-    dev = D.device
-    pooled = _b.tacg_affinity_swapgain(ctx, D, Cm, ntok, P, capacity, None, alpha=0.0, tau=tau, eps=eps, want=("W",))
-    cent = pooled["W"].double().sum(dim=2).cpu().numpy()
-    out = _b.tacg_affinity_swapgain(ctx, D, Cm, ntok, P, capacity, torch.from_numpy(primary.astype(np.int8)).to(dev),
-                                    alpha=alpha, tau=tau, eps=eps, want=("aff",))
-    aff = out["aff"].cpu().numpy()
-    for l in range(L):
-        order = sorted(range(E), key=lambda e: (-cent[l, e], e))
-        for e in order[:n_rep]:
-            cands = sorted((m for m in range(P) if m != int(primary[l, e])), key=lambda m: (-aff[l, e, m], m))
-            for i, m in enumerate(cands[:r]):
-                rep[l, e, i] = m
-    return rep
 
 
 def tacg_gesr_placement(ctx: "_b.Context", D, Cm, ntok, P: int, capacity: int, n_rep: int, r: int,

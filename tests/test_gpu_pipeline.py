@@ -52,7 +52,8 @@ def test_pipeline_local_search_and_eval(tacg, ctx, cfg_id, N, L):
     assert (j1[swaps > 0] > j0[swaps > 0]).all()
     # the replica table passes the library's own validation and the evaluation matches the oracle
     r = max(cfg.r, 1)
-    replicas = placement.replica_table(ctx, co["D"], co["C"], co["ntok"], cfg.P, cfg.capacity, primary, 4, r)
+    replicas = tacg.gesr_build_replicas(ctx, co["D"], co["C"], co["ntok"], cfg.P, cfg.capacity,
+                                        torch.from_numpy(primary).cuda(), 4, r)[0].cpu().numpy()
     got = tacg.tacg_eval_placement(ctx, ei.cuda(), ef.cuda(), cfg.E, cfg.F, cfg.P, torch.from_numpy(primary).cuda(),
                                    torch.from_numpy(replicas).cuda(), theta=0.15, rho=0.995,
                                    microbatch=cfg.microbatch, flags=tacg.TACG_VALIDATE)

@@ -116,7 +116,12 @@ def test_spectral_place_degenerate_and_refusals(tacg, ctx):
     W = _random_graph(1, 5, 9)
     got = tacg.tacg_spectral_place(ctx, torch.from_numpy(W).cuda(), 1, 5)
     assert (got["primary"].cpu().numpy() == 0).all()
+    # an expert that never co-activates (an all-zero row and column of W): isolated, still placed like the oracle places it
+    W = _random_graph(1, 8, 3)
+    W[0, 5, :] = 0.0
+    W[0, :, 5] = 0.0
+    _check_full(tacg, ctx, W, 2, 4)
     Wd = torch.from_numpy(_random_graph(1, 8, 1)).cuda()
-    for P, cap, jit, iters in ((9, 1, 1e-6, 10), (2, 3, 1e-6, 10), (2, 4, -1.0, 10), (2, 4, 1e-6, 0), (65, 1, 1e-6, 10)):
+    for P, cap, jit, iters in ((9, 1, 1e-6, 10), (2, 3, 1e-6, 10), (2, 4, -1.0, 10), (2, 4, 0.0, 10), (2, 4, 1e-6, 0), (65, 1, 1e-6, 10)):
         with pytest.raises(tacg.TacgError):
             tacg.tacg_spectral_place(ctx, Wd, P, cap, jitter=jit, kmeans_iters=iters)
