@@ -428,7 +428,7 @@ def main():
     af_ms, af_n = ctx.profile_read(tacg.TACG_PROF_AFFINITY)
     ev_ms, ev_n = ctx.profile_read(tacg.TACG_PROF_EVAL)
     abytes, co_avg_ms, achieved, frac, used_path = coact_roofline(tacg, ctx, cfg, co_ms, co_n, peak)
-    kernel_names = {"hist": "coact_hist_kernel+coact_finalize_kernel",
+    kernel_names = {"hist": "coact_hist_kernel+coact_finalize_kernel" + ("+part_count/scan/scatter_kernel" if cfg.E > 160 else ""),
                     "mma": "coact_mma_kernel+coact_mma_finalize_kernel"}
     roofline = {
         "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": frac,

@@ -2,7 +2,7 @@
  * placement (arxiv/paper_2606_01007), hand-written CUDA for sm_100a (B200).
  *
  * Citations are PAPER.md:<line> (the paper text) and SURVEY.md section 8; the
- * readings Q1..Q28 taken where the paper is silent are listed in DESIGN.md.
+ * readings Q1..Q39 taken where the paper is silent are listed in DESIGN.md section 3.
  *
  * Conventions (all entry points)
  *   - Every pointer marked "dev" is DEVICE memory owned and allocated by the
@@ -50,7 +50,7 @@ typedef enum tacg_status {
 /* flags of tacg_coact_accumulate */
 #define TACG_ZERO_FIRST 0x1u /* zero D, C and ntok on the stream before accumulating */
 #define TACG_VALIDATE   0x2u /* check indices / family (coact) or primary / replicas (eval, select) on device */
-#define TACG_PATH_AUTO  0x00u /* pick the co-activation kernel by shape */
+#define TACG_PATH_AUTO  0x00u /* pick the co-activation kernel by shape (DESIGN.md 5.2 "Path choice") */
 #define TACG_PATH_HIST  0x10u /* force the shared-memory / global atomic histogram kernel */
 #define TACG_PATH_MMA   0x20u /* force the tcgen05 kind::i8 X^T X kernel; TACG_ERR_SHAPE if the shape is unsupported */
 #define TACG_PATH_MASK  0x30u

@@ -21,6 +21,8 @@ SO = os.path.join(HERE, "libtacg.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+if os.environ.get("TACG_CHECKED") == "1":      # bounds assertions in the kernels (tacg_common.cuh); use with --force
+    FLAGS.append("-DTACG_CHECKED")
 
 
 def _stale(target: str, deps) -> bool:

@@ -96,7 +96,10 @@ __device__ __forceinline__ void slow_token(const int (&e)[KMAX], int k, int E, u
             const int j = e[b];
             if (b == a || (unsigned)j >= (unsigned)E || j == i) continue;
             ++cnt;
-            if (b > a) atomicAdd(&hist[(tri_row(min(i, j), E) + max(i, j)) * CP], 1u);
+            if (b > a) {
+                TACG_ASSERT(tri_row(min(i, j), E) + max(i, j) >= 0 && tri_row(min(i, j), E) + max(i, j) < E * (E - 1) / 2);
+                atomicAdd(&hist[(tri_row(min(i, j), E) + max(i, j)) * CP], 1u);
+            }
         }
         if (km1 - cnt) atomicAdd(&corr[i], (unsigned)(km1 - cnt));
     }
@@ -163,7 +166,10 @@ __device__ __forceinline__ void count_packed(const unsigned (&w)[KT / 2], int E,
         for (int a = 0; a + 1 < KT; ++a) {
             unsigned* rowp = hist + tri_row(s[a], E) * CP;
 #pragma unroll
-            for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b] * CP, 1u);
+            for (int b = a + 1; b < KT; ++b) {
+                TACG_ASSERT(tri_row(s[a], E) + s[b] >= 0 && tri_row(s[a], E) + s[b] < E * (E - 1) / 2);
+                atomicAdd(rowp + s[b] * CP, 1u);
+            }
         }
         return;
     }
@@ -237,7 +243,10 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             for (int a = 0; a + 1 < KT; ++a) {
                 unsigned* rowp = hf + tri_row(s[a], p.E) * CP;
 #pragma unroll
-                for (int b = a + 1; b < KT; ++b) atomicAdd(rowp + s[b] * CP, c);
+                for (int b = a + 1; b < KT; ++b) {
+                    TACG_ASSERT(s[a] < s[b] && s[b] < p.E && tri_row(s[a], p.E) + s[b] < p.tri);
+                    atomicAdd(rowp + s[b] * CP, c);
+                }
             }
         }
     };
@@ -281,6 +290,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             if (mm) {
                 if (miss) {
                     const int pos = qn + __popc(mm & ((1u << lane) - 1u));
+                    TACG_ASSERT(pos >= 0 && pos < 64);
                     qkey[pos] = key;
                     qfam[pos] = (unsigned char)fl;
                 }
@@ -388,6 +398,7 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             const int b0 = ci - run;
             const unsigned* bo = p.boff + (size_t)fg * (p.cps + 1);
             const unsigned j0 = bo[b0], j1 = bo[b0 + run];
+            TACG_ASSERT(b0 >= 0 && b0 + run <= p.cps && j0 <= j1 && (long long)j1 <= p.N);
             const unsigned* __restrict__ list = p.perm + (size_t)fg * (size_t)p.N;
             if (l == 0 && tid == 0) sntok[0] += j1 - j0;
             if constexpr (KT >= 2) {
@@ -546,6 +557,7 @@ part_scatter_kernel(const int8_t* __restrict__ family, long long N, int F, int n
     __syncthreads();
     if ((unsigned)f < (unsigned)F) {
         for (int w = 0; w < warp; ++w) rank += wc[f][w];
+        TACG_ASSERT((long long)boff[(size_t)f * (nb + 1) + blockIdx.x] + rank < N);
         perm[(size_t)f * (size_t)N + boff[(size_t)f * (nb + 1) + blockIdx.x] + rank] = (unsigned)t;
     }
 }

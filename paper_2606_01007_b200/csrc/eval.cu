@@ -440,6 +440,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
 #pragma unroll
                     for (int j = 0; j < KM; ++j) {
                         const unsigned row = t[j] & 0x7fu;
+                        TACG_ASSERT(a2[j] <= 1024u && (row < (unsigned)P || row == (unsigned)kSink));
                         R |= bit_or_zero<M>(row);
                         sred_inc(cl + row * 128u);
                         if (RECS && j < 8) ranks |= ((t[j] >> 8) & 15u) << (4 * j);
@@ -497,6 +498,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                     for (int u = 0; u < U; ++u) {
                         if (drank[u]) {
                             const unsigned pos = dmulti[u] ? pos2-- : pos1++;
+                            TACG_ASSERT(pos < (unsigned)g.slice && pos1 <= pos2 + 2u);
                             rec_set[pos] = dR[u];
                             rec_rank[pos] = drank[u];
                             rec_meta[pos] = dmeta[u];
@@ -745,10 +747,12 @@ __global__ void __launch_bounds__(kChainThreads, 1) eval_chain_kernel(const Chai
                     const M hb = (M)1 << ((meta >> 16) & 63u);
                     while (rk) {
                         const int sh = (__ffs(rk) - 1) & ~3;
+                        TACG_ASSERT(((rk >> sh) & 15u) >= 1u && (int)((rk >> sh) & 15u) <= nrep);
                         const M pm = pick_slot((rk >> sh) & 15u, R | hb);
                         rk &= ~(15u << sh);
                         R |= pm;
                         const int pick = sizeof(M) == 8 ? 63 - __clzll((long long)pm) : 31 - __clz((int)pm);
+                        TACG_ASSERT(pick >= 0 && pick < P);
                         sred_inc(cl + (unsigned)pick * 128u);
                         if (OUT && p.serve) p.serve[token_of(x, meta) * k + (sh >> 2)] = (signed char)pick;
                     }
@@ -769,6 +773,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) eval_chain_kernel(const Chai
                             hi_sl = slds_u32(pb + 4u * (sl + 1u));
                         }
                         const unsigned within = gi - lo_sl;
+                        TACG_ASSERT(sl < (unsigned)ns && within < slice);
                         return sl * slice + (cls ? slice - 1u - within : within);
                     };
                     for (unsigned g0 = (unsigned)rank * kChainThreads + tid; g0 < tot; g0 += 2u * stride) {

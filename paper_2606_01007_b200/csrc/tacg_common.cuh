@@ -106,6 +106,16 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
 
 // ---- device helpers ----
 #ifdef __CUDACC__
+// Bounds assertions of the kernels' shared-memory and scratch indices.  compute-sanitizer is closed on the B200 pool
+// this library is developed on, so the checks it would make are written into the kernels and switched on with
+// TACG_CHECKED=1 python -m paper_2606_01007_b200.build --force (device assert: a violation aborts the launch and the
+// next CUDA call returns an error, which every test then reports); they compile to nothing otherwise.
+#ifdef TACG_CHECKED
+#include <cassert>
+#define TACG_ASSERT(x) assert(x)
+#else
+#define TACG_ASSERT(x) ((void)0)
+#endif
 // Programmatic dependent launch: the kernels of one step are launched with tacg_launch_pdl and begin with
 // tacg_pdl_prologue(), which blocks until the PREVIOUS kernel of the stream has completed and its memory is
 // visible.  Everything after the prologue is ordered exactly as with plain stream serialisation; what is saved

@@ -10,7 +10,7 @@
 Everything numeric runs in the library (tacg_coact_accumulate, tacg_affinity_swapgain, tacg_spectral_place,
 gesr_build_replicas, tacg_eval_placement); this module only sorts a count vector and formats reports.
 
-    python -m paper_2606_01007_b200.harness --config 2 [--tokens 65536] [--layers 4]     # JSON report on stdout
+    python -m paper_2606_01007_b200.harness --config 2 [--tokens 65536] [--layers 4] [--gap] [--no-skew]   # JSON on stdout
 """
 from __future__ import annotations
 
@@ -101,6 +101,7 @@ def main():
     ap.add_argument("--tokens", type=int, default=65536, help="tokens per layer of the calibration and online traces")
     ap.add_argument("--layers", type=int, default=4)
     ap.add_argument("--gap", action="store_true", help="also the per-token against micro-batch comparison (f4)")
+    ap.add_argument("--no-skew", action="store_true", help="skip the 13-workload sweep")
     args = ap.parse_args()
     base = tracegen.get_config(args.config)
     cfg = tracegen.scaled(base, N=args.tokens, N_eval=args.tokens, L=min(base.L, args.layers))
@@ -110,7 +111,7 @@ def main():
         co = _b.tacg_coact_accumulate(ctx, bi, bf, cfg.E, cfg.F)
         placements = build_placements(ctx, cfg, co["D"], co["C"], co["ntok"])
         out = {"config": cfg.name, "tokens": args.tokens, "layers": cfg.L,
-               "skew": skew_report(ctx, cfg, params, placements, args.tokens, cfg.seed + 11)}
+               "skew": {} if args.no_skew else skew_report(ctx, cfg, params, placements, args.tokens, cfg.seed + 11)}
         if args.gap and "tacg+gesr" in placements:
             ei, ef = tracegen.gen_trace(cfg, params, eval_trace=True, device="cuda")
             pr, rp = placements["tacg+gesr"]

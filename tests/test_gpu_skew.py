@@ -1,4 +1,4 @@
-"""The paper's skew sweep: one placement, thirteen online family
+"""The paper's skew sweep (section 4.3, PAPER.md:383 the 13-workload suite): one placement, thirteen online family
 streams.  Only the family labels change, which is exactly what moves work between the family
 bins of the counting kernels and between the per-family accumulators of the evaluator, so every
 stream is a parity case for both: counts and evaluation bit-exact against the C oracle.
