@@ -192,6 +192,38 @@ __device__ __forceinline__ void count_token(const int16_t* __restrict__ row, int
     }
 }
 
+// Eight ids, two per word, sorted into the eight bytes of a key (smallest id in the lowest byte).
+// Lanes: the low halves of the four words are one sequence, the high halves another; both are sorted with the same
+// five word-wide compare-exchanges, then merged as a bitonic sequence whose compare-exchanges are again word-wide
+// after two byte permutes.  ok = every id is in [0, 256) and no two are equal (else the caller takes the slow path).
+__device__ __forceinline__ unsigned long long sort8_key(const unsigned (&w)[4], bool& ok) {
+    unsigned a = w[0], b = w[1], c = w[2], d = w[3], t;
+    const unsigned orw = (a | b) | (c | d);
+    // 4-sorter on the words: (0,1) (2,3) (0,2) (1,3) (1,2)
+    t = __vminu2(a, b); b = __vmaxu2(a, b); a = t;
+    t = __vminu2(c, d); d = __vmaxu2(c, d); c = t;
+    t = __vminu2(a, c); c = __vmaxu2(a, c); a = t;
+    t = __vminu2(b, d); d = __vmaxu2(b, d); b = t;
+    t = __vminu2(b, c); c = __vmaxu2(b, c); b = t;
+    // x = low lane ascending, y = high lane ascending; pair x_i with y_(3-i)
+    const unsigned x01 = __byte_perm(a, b, 0x5410), x23 = __byte_perm(c, d, 0x5410);
+    const unsigned y32 = __byte_perm(d, c, 0x7632), y10 = __byte_perm(b, a, 0x7632);
+    const unsigned l01 = __vminu2(x01, y32), h01 = __vmaxu2(x01, y32);
+    const unsigned l23 = __vminu2(x23, y10), h23 = __vmaxu2(x23, y10);
+    const unsigned pl = __vminu2(l01, l23), ql = __vmaxu2(l01, l23);     // lower four: (0,2) (1,3)
+    const unsigned ph = __vminu2(h01, h23), qh = __vmaxu2(h01, h23);     // upper four
+    const unsigned t0 = __byte_perm(pl, ql, 0x5410), t1 = __byte_perm(pl, ql, 0x7632);
+    const unsigned u0 = __byte_perm(ph, qh, 0x5410), u1 = __byte_perm(ph, qh, 0x7632);
+    const unsigned lo_e = __vminu2(t0, t1), lo_o = __vmaxu2(t0, t1);     // (s0, s2), (s1, s3)
+    const unsigned hi_e = __vminu2(u0, u1), hi_o = __vmaxu2(u0, u1);     // (s4, s6), (s5, s7)
+    const unsigned k0 = __byte_perm(lo_e, lo_o, 0x6240), k1 = __byte_perm(hi_e, hi_o, 0x6240);
+    // neighbours equal <=> a zero byte in key ^ (key >> 8) (the top byte compares s7 with 0: s7 = 0 means all equal)
+    const unsigned d0 = k0 ^ __funnelshift_r(k0, k1, 8), d1 = k1 ^ (k1 >> 8);
+    const unsigned z = ((d0 - 0x01010101u) & ~d0) | ((d1 - 0x01010101u) & ~d1);
+    ok = (orw & 0xff00ff00u) == 0u && (z & 0x80808080u) == 0u;
+    return (unsigned long long)k0 | ((unsigned long long)k1 << 32);
+}
+
 // smem layout (words): [Fs][tri] pair bins | [Fs][E] corr | [Fs] ntok (layer 0 only) | pad to slot_words
 // CP (non-filter mode only): bank-spread copies of the pair bins, one per quarter warp.
 template <int KT, bool FILTER, int CP>
@@ -260,21 +292,27 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             unsigned long long key = 0ull;
             bool miss = false;
             if (live) {
-                int e[KT], s[KT];
+                bool fast;
+                if constexpr (KT == 8) {
+                    // sorted set as eight bytes without unpacking: the ids stay two per word and every min / max
+                    // (VIMNMX.U16x2) orders two pairs at once
+                    key = sort8_key(w, fast);
+                    fast = fast && (int)(key >> 56) < p.E;
+                } else {
+                    int s[KT];
 #pragma unroll
-                for (int i = 0; i < KT / 2; ++i) {
-                    e[2 * i] = (int)(short)(w[i] & 0xffffu);
-                    e[2 * i + 1] = (int)w[i] >> 16;
+                    for (int i = 0; i < KT / 2; ++i) {
+                        s[2 * i] = (int)(short)(w[i] & 0xffffu);
+                        s[2 * i + 1] = (int)w[i] >> 16;
+                    }
+                    sort_ids<KT>(s);
+                    fast = s[0] >= 0 && s[KT - 1] < p.E;
+#pragma unroll
+                    for (int a = 0; a + 1 < KT; ++a) fast = fast && (s[a] != s[a + 1]);
+#pragma unroll
+                    for (int a = 0; a < KT; ++a) key |= (unsigned long long)(unsigned)(s[a] & 0xff) << (8 * a);
                 }
-#pragma unroll
-                for (int a = 0; a < KT; ++a) s[a] = e[a];
-                sort_ids<KT>(s);
-                bool fast = s[0] >= 0 && s[KT - 1] < p.E;
-#pragma unroll
-                for (int a = 0; a + 1 < KT; ++a) fast = fast && (s[a] != s[a + 1]);
                 if (fast) {
-#pragma unroll
-                    for (int a = 0; a < KT; ++a) key |= (unsigned long long)(unsigned)s[a] << (8 * a);
                     const MemoTable memo = memo_of(fl);
                     const unsigned h = (unsigned)((key * 0x9E3779B97F4A7C15ull) >> 40) & memo.mask;
                     // plain read first: once a set is in the table a hit costs one load and one increment
@@ -283,6 +321,12 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
                     if (prev == 0ull || prev == key) atomicAdd(memo.cnt + h, 1u);
                     else miss = true;
                 } else {
+                    int e[KT];
+#pragma unroll
+                    for (int i = 0; i < KT / 2; ++i) {
+                        e[2 * i] = (int)(short)(w[i] & 0xffffu);
+                        e[2 * i + 1] = (int)w[i] >> 16;
+                    }
                     slow_token<KT, CP>(e, KT, p.E, hist_lane + (size_t)fl * p.tri * CP, corr + fl * p.E);
                 }
             }
