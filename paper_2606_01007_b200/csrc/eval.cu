@@ -10,7 +10,7 @@
 //                      <= 8192 tokens); per token the primary map is looked up in a 16-bit table, the
 //                      slots of experts without replicas are counted (lane-private shared-memory
 //                      counters, no branch) and, when the token has no replicated slot, its communication
-//                      cost is final.  A token WITH replicated slots leaves one 12-byte record (accessed
+//                      cost is final.  A token WITH replicated slots leaves one 16-byte record (accessed
 //                      set so far | the rank of the replicated expert in each slot | home, family,
 //                      offset).  Every item writes one row of partial sums
 //                      (loads | span | remote | tokens per family | records).
@@ -49,7 +49,8 @@ namespace {
 constexpr int kEvalThreads = 512;    // eval_scan_kernel, select_kernel
 constexpr int kEvalBatch = 4;        // tokens per thread with their loads in flight together
 constexpr int kSlice = 8192;         // most tokens of a scan item (13-bit offsets in the records, 16 per thread)
-constexpr int kChainThreads = 1024;
+constexpr int kChainThreads = 512;    // two CTAs per SM, so that clusters of 4 at L = 58 still use every SM
+constexpr unsigned kRecFlight = 4;    // records a chain thread loads before it resolves the first
 constexpr long long kSeqBelow = 1024; // micro-batches shorter than this go to the one-warp-per-layer kernel
 constexpr int kCandStride = 12;      // bytes per expert in the candidate table: [0] = count, [1..9] = partitions
 constexpr unsigned kRepFlag = 0x80u; // ptab bit: the expert has at least one replica
@@ -241,16 +242,19 @@ __device__ __forceinline__ void item_tokens(const EvalGeom& g, long long mb, int
     if (t1 < t0) t1 = t0;
 }
 
-// Records of the deferred tokens of an item, three parallel arrays of g.slice entries per item (tokens with
-// one pending slot from entry 0 upwards, tokens with several from the last entry downwards):
-//   set   M          accessed set after pass 1 (partitions of the slots without replicas)
-//   rank  unsigned   4 bits per slot: rank of the replicated expert in that slot, 0 = not pending
-//   meta  unsigned   offset in the item (13) | family (3) | home (6)
-struct RecArrays {
-    void* set;
-    unsigned* rank;
-    unsigned* meta;
-};
+// Records of the deferred tokens of an item, g.slice 16-byte entries per item (tokens with one pending slot from entry
+// 0 upwards, tokens with several from the last entry downwards), one load or store each:
+//   x, y  accessed set after pass 1 (partitions of the slots without replicas), low and high word
+//   z     4 bits per slot: rank of the replicated expert in that slot, 0 = not pending
+//   w     offset in the item (13) | family (3) | home (6)
+typedef uint4 Rec;
+template <typename M> __device__ __forceinline__ Rec make_rec(M R, unsigned rank, unsigned meta) {
+    return make_uint4((unsigned)R, (unsigned)((unsigned long long)R >> 32), rank, meta);
+}
+template <typename M> __device__ __forceinline__ M rec_set(const Rec& v) {
+    if constexpr (sizeof(M) == 8) return (unsigned long long)v.x | ((unsigned long long)v.y << 32);
+    else return v.x;
+}
 
 // 1 << s with PTX semantics: a shift count >= the register width gives 0 (the sink row 64 is no partition)
 template <typename M> __device__ __forceinline__ M bit_or_zero(unsigned s);
@@ -289,7 +293,7 @@ struct ScanParams {
     const int8_t* primary;
     const int8_t* replicas;   // null: no replicas
     unsigned* rows;           // [L*ipl][W]
-    RecArrays rec;            // [L*ipl][slice] each (replicas only)
+    Rec* rec;                 // [L*ipl][slice] (replicas only)
     unsigned char* cost;      // [L,N] or null
     signed char* serve;       // [L,N,k] or null
 };
@@ -369,9 +373,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
         const int16_t* base = p.indices + (size_t)layer * (size_t)g.N * (size_t)k;
         unsigned char* cost_l = (OUT && p.cost) ? p.cost + (size_t)layer * g.N + t0 : nullptr;
         signed char* serve_l = (OUT && p.serve) ? p.serve + ((size_t)layer * g.N + t0) * k : nullptr;
-        M* rec_set = RECS ? reinterpret_cast<M*>(p.rec.set) + (size_t)item * g.slice : nullptr;
-        unsigned* rec_rank = RECS ? p.rec.rank + (size_t)item * g.slice : nullptr;
-        unsigned* rec_meta = RECS ? p.rec.meta + (size_t)item * g.slice : nullptr;
+        Rec* recs = RECS ? p.rec + (size_t)item * g.slice : nullptr;
         int home = (hm0 + tid) % P;
         const int8_t* fam0 = p.family + t0;
         const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
@@ -499,9 +501,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                         if (drank[u]) {
                             const unsigned pos = dmulti[u] ? pos2-- : pos1++;
                             TACG_ASSERT(pos < (unsigned)g.slice && pos1 <= pos2 + 2u);
-                            rec_set[pos] = dR[u];
-                            rec_rank[pos] = drank[u];
-                            rec_meta[pos] = dmeta[u];
+                            recs[pos] = make_rec<M>(dR[u], drank[u], dmeta[u]);
                         }
                     }
                 }
@@ -557,7 +557,7 @@ struct ChainParams {
     const int8_t* primary;
     const int8_t* replicas;
     const unsigned* rows;
-    RecArrays rec;
+    const Rec* rec;
     float theta;
     double rho;
     double* load_state;                // [L,P] in/out or null
@@ -574,7 +574,7 @@ struct ChainParams {
 // item's records; the integer dispatch counts of a micro-batch are exchanged through distributed shared
 // memory (two alternating buffers, one cluster barrier per micro-batch).
 template <typename M, bool OUT, bool CLUSTER>
-__global__ void __launch_bounds__(kChainThreads, 1) eval_chain_kernel(const ChainParams p) {
+__global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const ChainParams p) {
     tacg_pdl_prologue();
     extern __shared__ __align__(16) unsigned char csm[];
     const EvalGeom& g = p.g;
@@ -731,9 +731,7 @@ __global__ void __launch_bounds__(kChainThreads, 1) eval_chain_kernel(const Chai
                     __syncthreads();
                 }
                 const size_t ro0 = rec_l + ((size_t)mb * g.spm + s0) * (size_t)g.slice;
-                const M* rset = reinterpret_cast<const M*>(p.rec.set) + ro0;
-                const unsigned* rrank = p.rec.rank + ro0;
-                const unsigned* rmeta = p.rec.meta + ro0;
+                const Rec* recs = p.rec + ro0;
                 const unsigned stride = (unsigned)CS * kChainThreads;
                 const unsigned slice = (unsigned)g.slice;
                 // per-token outputs of a record at entry x (OUT only): token index from the slice and the offset
@@ -776,24 +774,20 @@ __global__ void __launch_bounds__(kChainThreads, 1) eval_chain_kernel(const Chai
                         TACG_ASSERT(sl < (unsigned)ns && within < slice);
                         return sl * slice + (cls ? slice - 1u - within : within);
                     };
-                    for (unsigned g0 = (unsigned)rank * kChainThreads + tid; g0 < tot; g0 += 2u * stride) {
-                        // two records per round, all six loads in flight before the first is used
-                        unsigned x[2], rk[2], me[2];
-                        M Rs[2];
+                    for (unsigned g0 = (unsigned)rank * kChainThreads + tid; g0 < tot; g0 += kRecFlight * stride) {
+                        // kRecFlight records per round, all their loads in flight before the first is used
+                        unsigned x[kRecFlight];
+                        Rec v[kRecFlight];
 #pragma unroll
-                        for (int q = 0; q < 2; ++q) {
+                        for (int q = 0; q < kRecFlight; ++q) {
                             const unsigned gq = g0 + (unsigned)q * stride;
                             x[q] = gq < tot ? locate(gq) : x[0];
                         }
 #pragma unroll
-                        for (int q = 0; q < 2; ++q) {
-                            Rs[q] = rset[x[q]];
-                            rk[q] = rrank[x[q]];
-                            me[q] = rmeta[x[q]];
-                        }
+                        for (int q = 0; q < kRecFlight; ++q) v[q] = recs[x[q]];
 #pragma unroll
-                        for (int q = 0; q < 2; ++q)
-                            if (g0 + (unsigned)q * stride < tot) resolve(Rs[q], rk[q], me[q], x[q]);
+                        for (int q = 0; q < kRecFlight; ++q)
+                            if (g0 + (unsigned)q * stride < tot) resolve(rec_set<M>(v[q]), v[q].z, v[q].w, x[q]);
                     }
                 }
                 // items left to this kernel: their tokens are served here, from the trace
@@ -1154,11 +1148,12 @@ int launch_chain(EvalCall& c) {
                         (((size_t)g.E * g.r + 15) & ~(size_t)15) + sizeof(unsigned) * (size_t)g.P * 32 +
                         sizeof(unsigned) * (kChainThreads / 32) * 8 * 32 + sizeof(unsigned short) * (size_t)g.E + 16;
     // cluster size: as many CTAs per layer as the SM count allows, up to 16 (non-portable above 8)
+    const int slots = 2 * ctx->sm_count;           // resident CTAs (two per SM)
     int cs = 1;
-    while (cs < 16 && (long long)g.L * cs * 2 <= ctx->sm_count) cs *= 2;
+    while (cs < 16 && (long long)g.L * cs * 2 <= slots) cs *= 2;
     // a micro-batch with few records gains nothing from more CTAs
     while (cs > 1 && min(g.B, g.N) < (long long)cs * 2048) cs /= 2;
-    c.cp.groups = min(g.L, max(1, ctx->sm_count / cs));
+    c.cp.groups = min(g.L, max(1, slots / cs));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3(c.cp.groups * cs);
@@ -1297,19 +1292,14 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         const int kt = tacg_pick_kt(k, indices);
         const size_t items = (size_t)L * (size_t)g.ipl;
         const size_t nrec = (c.rep && kt > 0) ? items * (size_t)g.slice : 0;      // one record per token at most
-        const size_t set_bytes = P > 32 ? sizeof(unsigned long long) : sizeof(unsigned);
-        const size_t o_set = tacg_align_up(items * g.W * sizeof(unsigned), 256);
-        const size_t o_rank = o_set + tacg_align_up(nrec * set_bytes, 256);
-        const size_t o_meta = o_rank + tacg_align_up(nrec * sizeof(unsigned), 256);
-        const size_t total = o_meta + tacg_align_up(nrec * sizeof(unsigned), 256);
+        const size_t o_rec = tacg_align_up(items * g.W * sizeof(unsigned), 256);
+        const size_t total = o_rec + nrec * sizeof(Rec);
         char* sbase = static_cast<char*>(tacg_scratch(ctx, total));
         if (!sbase) return TACG_ERR_CUDA;
         c.sp.g = g;
         c.sp.indices = indices; c.sp.family = family; c.sp.primary = primary; c.sp.replicas = c.rep ? replicas : nullptr;
         c.sp.rows = reinterpret_cast<unsigned*>(sbase);
-        c.sp.rec.set = sbase + o_set;
-        c.sp.rec.rank = reinterpret_cast<unsigned*>(sbase + o_rank);
-        c.sp.rec.meta = reinterpret_cast<unsigned*>(sbase + o_meta);
+        c.sp.rec = reinterpret_cast<Rec*>(sbase + o_rec);
         c.sp.cost = cost_per_token;
         c.sp.serve = reinterpret_cast<signed char*>(serve);
         c.cp.g = g;
