@@ -280,6 +280,11 @@ __device__ __forceinline__ unsigned slds_u32(unsigned a) {
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
 }
+__device__ __forceinline__ unsigned slds_u8(unsigned a) {
+    unsigned v;
+    asm("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
 __device__ __forceinline__ unsigned slds_u16(unsigned a) {
     unsigned short v;
     asm("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a));
@@ -330,7 +335,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
     const unsigned cl = saddr(cnt + lane);                                  // this lane's counter column
     unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;                    // this thread's family words
     const unsigned al = saddr(acc);
-    const unsigned tb = saddr(tab16);
+    const unsigned tb = saddr(tab16), pb8 = saddr(ptab);
     const int stepP = kEvalThreads % P;
 
     for (int i = tid; i < (kSink + 1) * 32; i += kEvalThreads) cnt[i] = 0u;
@@ -414,35 +419,45 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                 dmulti[u] = false;
                 dR[u] = 0;
                 if (live) {
-                    unsigned a2[KM];            // byte offsets into tab16
+                    unsigned a2[KM];            // byte offsets into the table (tab16 with replicas, else the byte table)
+                    constexpr unsigned SC = REP ? 2u : 1u;      // bytes per table entry
                     if constexpr (KT > 0) {
                         unsigned orw = 0u;
 #pragma unroll
                         for (int i = 0; i < NW; ++i) {
-                            a2[2 * i] = (w[u][i] << 1) & 0x1fffeu;
-                            a2[2 * i + 1] = (w[u][i] >> 15) & 0x1fffeu;
+                            if constexpr (REP) {
+                                a2[2 * i] = (w[u][i] << 1) & 0x1fffeu;
+                                a2[2 * i + 1] = (w[u][i] >> 15) & 0x1fffeu;
+                            } else {
+                                a2[2 * i] = w[u][i] & 0xffffu;
+                                a2[2 * i + 1] = w[u][i] >> 16;
+                            }
                             orw |= w[u][i];
                         }
                         if (orw & 0xfe00fe00u) {       // an id outside [0,512): clamp to the "not an expert" entry
 #pragma unroll
-                            for (int j = 0; j < KM; ++j) a2[j] = min(a2[j], 1024u);
+                            for (int j = 0; j < KM; ++j) a2[j] = min(a2[j], 512u * SC);
                         }
                     } else {
 #pragma unroll
                         for (int j = 0; j < 16; ++j)
-                            a2[j] = (j < k) ? 2u * min((unsigned)(unsigned short)__ldg(base + ((size_t)t0 + o) * k + j), 512u) : 1024u;
+                            a2[j] = (j < k) ? SC * min((unsigned)(unsigned short)__ldg(base + ((size_t)t0 + o) * k + j), 512u) : 512u * SC;
                     }
                     // all table lookups first, then no branch: a slot that is not a plain expert has row 64, which
-                    // shifts to an empty mask and counts into the sink row
+                    // shifts to an empty mask and counts into the sink row.  Without replicas the byte table already
+                    // holds the row: the partition, or kBadFlag = 64 = the sink.
                     unsigned t[KM];
 #pragma unroll
-                    for (int j = 0; j < KM; ++j) t[j] = slds_u16(tb + a2[j]);
+                    for (int j = 0; j < KM; ++j) {
+                        if constexpr (REP) t[j] = slds_u16(tb + a2[j]);
+                        else t[j] = slds_u8(pb8 + a2[j]);
+                    }
                     M R = 0;
                     unsigned ranks = 0u;
 #pragma unroll
                     for (int j = 0; j < KM; ++j) {
-                        const unsigned row = t[j] & 0x7fu;
-                        TACG_ASSERT(a2[j] <= 1024u && (row < (unsigned)P || row == (unsigned)kSink));
+                        const unsigned row = REP ? (t[j] & 0x7fu) : t[j];
+                        TACG_ASSERT(a2[j] <= 512u * SC && (row < (unsigned)P || row == (unsigned)kSink));
                         R |= bit_or_zero<M>(row);
                         sred_inc(cl + row * 128u);
                         if (RECS && j < 8) ranks |= ((t[j] >> 8) & 15u) << (4 * j);
@@ -452,7 +467,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                             signed char* out = serve_l + (size_t)o * k;
 #pragma unroll
                             for (int j = 0; j < KM; ++j)
-                                if (j < k) out[j] = (t[j] & kT16Bad) ? (signed char)-1 : (signed char)(t[j] & 0x3fu);
+                                if (j < k) out[j] = ((REP ? (t[j] & kT16Bad) : (t[j] & kBadFlag)) != 0u) ? (signed char)-1 : (signed char)(t[j] & 0x3fu);
                         }
                     }
                     unsigned packed = 1u << 22;          // one token of family f
