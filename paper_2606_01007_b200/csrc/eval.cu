@@ -609,7 +609,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     __shared__ unsigned long long ltot[64];    // cumulative integer load of this layer
     __shared__ unsigned long long csum[24];    // span | remote | tokens per family: rows of the scan kernel
     __shared__ unsigned long long dsum[16];    // span | remote of the deferred tokens handled by THIS CTA
-    __shared__ unsigned exch[2][64];           // this CTA's dispatch counts of the micro-batch (even / odd)
+    __shared__ unsigned exch[2][16][64];       // every cluster rank's dispatch counts of the micro-batch (even / odd):
+                                               // each CTA stores its own row into all its peers before the barrier
     __shared__ unsigned wsum[kChainThreads / 32 + 1];
     __shared__ unsigned long long feas_s;
     __shared__ __align__(16) unsigned long long candm[(kMaxRank + 1) * 4];   // by rank: one-hot masks (type M) of the first four candidates
@@ -702,6 +703,20 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             if (tid == 0) feas_s = load_guard(T.S, P, p.theta);
             if (tid == 0) bigq_s = 0u;
             if (tid >= 32 && tid < 64) load_counts(rows_mb, 0, min(32, g.spm), tid - 32);
+            // The records of the NEXT micro-batch do not depend on the chain: one bulk prefetch per slice and record class
+            // pulls them into L2 now (a single instruction each, issued by one lane of one CTA per slice).
+            if (tid >= 64 && tid < 128 && mb + 1 < g.nmb) {
+                const int sp = tid - 64;                       // slice of the next micro-batch
+                if (sp < g.spm && sp % CS == rank) {
+                    const unsigned* rn = rows_mb + ((size_t)g.spm + sp) * W + ncols;
+                    const unsigned n1 = rn[0], n2 = rn[1];
+                    if (n1 != kOverflow) {
+                        const Rec* rb = p.rec + rec_l + ((size_t)(mb + 1) * g.spm + sp) * (size_t)g.slice;
+                        if (n1) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rb), "r"(n1 * 16u) : "memory");
+                        if (n2) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rb + (g.slice - n2)), "r"(n2 * 16u) : "memory");
+                    }
+                }
+            }
             __syncthreads();
             const unsigned long long feas = feas_s;
             for (int i = tid; i < nrep; i += kChainThreads) {
@@ -840,18 +855,18 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             for (int m = tid >> 5; m < P; m += kChainThreads / 32) {
                 const unsigned sm = __reduce_add_sync(0xffffffffu, cnt[m * 32 + lane]);
                 cnt[m * 32 + lane] = 0u;
-                if (lane == 0) exch[par][m] = sm;
+                if constexpr (CLUSTER) {
+                    // lane q stores this CTA's count into rank q's table: after the barrier every CTA sums local words
+                    if (lane < CS) cg::this_cluster().map_shared_rank(&exch[par][rank][m], lane)[0] = sm;
+                } else {
+                    if (lane == 0) exch[par][0][m] = sm;
+                }
             }
             if constexpr (CLUSTER) cg::this_cluster().sync();
             else __syncthreads();
             if (tid < P) {
                 unsigned long long d = mine;
-                if constexpr (CLUSTER) {
-                    cg::cluster_group cgl = cg::this_cluster();
-                    for (int q = 0; q < CS; ++q) d += cgl.map_shared_rank(&exch[par][0], q)[tid];
-                } else {
-                    d += exch[par][tid];
-                }
+                for (int q = 0; q < CS; ++q) d += exch[par][q][tid];
                 Ls[tid] = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
                 ltot[tid] += d;
             } else if (tid < ncols) {
