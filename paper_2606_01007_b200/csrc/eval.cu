@@ -156,6 +156,72 @@ __device__ __forceinline__ void build_candidate(int e, int r, const LayerTables&
     for (int i = m + 1; i <= 3; ++i) out[i] = out[1];
 }
 
+// load_guard by one whole warp: the same left-to-right fp64 sum (every lane computes it, eight independent loads at a
+// time in front of the dependent additions), then one ballot per 32 partitions instead of a loop.  S has 64 entries.
+__device__ __forceinline__ unsigned long long load_guard_warp(const double* S, int P, float theta, int lane) {
+    double tot = 0.0;
+    for (int m0 = 0; m0 < P; m0 += 8) {
+        double v[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) v[i] = S[min(m0 + i, 63)];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+            if (m0 + i < P) tot = __dadd_rn(tot, v[i]);
+    }
+    const double Lbar = tot / (double)P;
+    const double thr = __dmul_rn(__dadd_rn(1.0, (double)theta), Lbar);
+    unsigned long long fm = __ballot_sync(0xffffffffu, lane < P && S[lane] <= thr);
+    if (P > 32) fm |= (unsigned long long)__ballot_sync(0xffffffffu, lane + 32 < P && S[lane + 32] <= thr) << 32;
+    return fm;
+}
+
+// build_candidate for r <= 3 (at most four candidates) without a data-dependent loop: the position of a candidate in
+// the stable order is the number of kept candidates that are lighter, or as heavy and earlier in slot order.
+__device__ __forceinline__ void build_candidate_small(int e, int r, const LayerTables& T, unsigned long long feas,
+                                                      unsigned char* out) {
+    int c[4];
+    bool ok[4];
+    c[0] = (int)(T.ptab[e] & 63u);
+    ok[0] = true;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int v = a < r ? (int)T.rep[e * r + a] : -1;
+        ok[a + 1] = v >= 0;
+        c[a + 1] = v & 63;
+    }
+    unsigned long long cmask = 0ull;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+        if (ok[i]) cmask |= 1ull << c[i];
+    const bool anyfeas = (cmask & feas) != 0ull;
+    double s[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        ok[i] = ok[i] && (!anyfeas || ((feas >> c[i]) & 1ull));
+        s[i] = T.S[c[i]];
+    }
+    unsigned b[4] = {0u, 0u, 0u, 0u};      // partitions by position
+    int m = 0;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        int pos = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (j != i && ok[j] && (s[j] < s[i] || (j < i && s[j] == s[i]))) ++pos;
+        if (ok[i]) {
+            ++m;
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (pos == q) b[q] = (unsigned)c[i];
+        }
+    }
+    if (m < 2) b[1] = b[0];
+    if (m < 3) b[2] = b[0];
+    unsigned* o = reinterpret_cast<unsigned*>(out);     // entries are 4-byte aligned (kCandStride = 12)
+    o[0] = (unsigned)m | (b[0] << 8) | (b[1] << 16) | (b[2] << 24);
+    o[1] = b[3];
+}
+
 __device__ __forceinline__ void build_candidates(int E, int r, const LayerTables& T, unsigned long long feas) {
     for (int e = threadIdx.x; e < E; e += blockDim.x)
         if (T.ptab[e] & kRepFlag) build_candidate(e, r, T, feas, T.cand + e * kCandStride);
@@ -596,7 +662,6 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     const int P = g.P, E = g.E, F = g.F, r = g.r, k = g.k;
     LayerTables T;
     size_t off = 0;
-    T.S = reinterpret_cast<double*>(csm + off);            off += 64 * sizeof(double);
     T.cand = csm + off;                                    off += ((size_t)E * kCandStride + 15) & ~(size_t)15;
     T.rep = reinterpret_cast<signed char*>(csm + off);     off += ((size_t)E * r + 15) & ~(size_t)15;
     unsigned* cnt = reinterpret_cast<unsigned*>(csm + off);   off += sizeof(unsigned) * (size_t)P * 32;
@@ -613,12 +678,14 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                                                // each CTA stores its own row into all its peers before the barrier
     __shared__ unsigned wsum[kChainThreads / 32 + 1];
     __shared__ unsigned long long feas_s;
+    __shared__ unsigned long long mine_s[64 + 24];   // the scan kernel's sums of the current micro-batch (row words)
     __shared__ __align__(16) unsigned long long candm[(kMaxRank + 1) * 4];   // by rank: one-hot masks (type M) of the first four candidates
     __shared__ unsigned bigq_s;                                 // ranks that list more than four candidates
     __shared__ unsigned pre1[33], pre2[33];                     // records of up to 32 slices, prefix sums
     __shared__ unsigned nrec1[32], nrec2[32];                   // records per slice (one pending slot | several)
     __shared__ unsigned ovf_s[32];
     T.ptab = ptab_s;
+    T.S = Ls;                                  // the snapshot of a micro-batch IS the EMA state at its start
 
     const int tid = threadIdx.x, lane = tid & 31;
     int rank = 0, CS = 1;
@@ -670,14 +737,11 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 }
             }
         };
-        // record counts of up to 32 slices starting at s0 (one pending slot | several) and their prefix sums; one warp
-        auto load_counts = [&](const unsigned* rows_mb, int s0, int ns, int ln) {
-            unsigned n1 = 0u, n2 = 0u;
-            if (ln < ns) {
-                n1 = rows_mb[(size_t)(s0 + ln) * W + ncols];
-                n2 = rows_mb[(size_t)(s0 + ln) * W + ncols + 1];
-                if (n1 == kOverflow) { n1 = 0u; n2 = 0u; ovf_s[ln] = 1u; } else ovf_s[ln] = 0u;
-            }
+        // record counts of up to 32 slices (one pending slot | several) and their prefix sums; one warp
+        auto put_counts = [&](unsigned n1, unsigned n2, int ln) {
+            const bool ovf = n1 == kOverflow;
+            if (ovf) { n1 = 0u; n2 = 0u; }
+            ovf_s[ln] = ovf ? 1u : 0u;
             nrec1[ln] = n1;
             nrec2[ln] = n2;
             unsigned a1 = n1, a2 = n2;
@@ -690,39 +754,73 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             pre2[ln + 1] = a2;
             if (ln == 0) { pre1[0] = 0u; pre2[0] = 0u; }
         };
+        auto load_counts = [&](const unsigned* rows_mb, int s0, int ns, int ln) {
+            unsigned n1 = 0u, n2 = 0u;
+            if (ln < ns) {
+                n1 = rows_mb[(size_t)(s0 + ln) * W + ncols];
+                n2 = rows_mb[(size_t)(s0 + ln) * W + ncols + 1];
+            }
+            put_counts(n1, n2, ln);
+        };
+        // The second warp keeps the record counts of the first 32 slices of this micro-batch and the next in registers
+        // (A, B) and has those of the one after in flight (C): nothing the chain waits for is a miss.
+        const int ns0 = min(32, g.spm);
+        auto fetch_counts = [&](long long mbx, unsigned& n1, unsigned& n2) {
+            n1 = 0u;
+            n2 = 0u;
+            if (mbx < g.nmb && lane < ns0) {
+                const unsigned* rn = rows_l + ((size_t)mbx * g.spm + lane) * W + ncols;
+                n1 = rn[0];
+                n2 = rn[1];
+            }
+        };
+        auto prefetch_rows = [&](long long mb0, long long mb1) {      // rows of micro-batches [mb0, mb1) into L2
+            mb1 = min(mb1, g.nmb);
+            if (mb0 < mb1) {
+                const unsigned* rp = rows_l + (size_t)mb0 * g.spm * W;
+                const unsigned bytes = (unsigned)((mb1 - mb0) * g.spm * W * 4);
+                asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rp), "r"(bytes) : "memory");
+            }
+        };
+        unsigned cA1 = 0u, cA2 = 0u, cB1 = 0u, cB2 = 0u;
+        if (tid >= 32 && tid < 64) {
+            if (lane == 0) prefetch_rows(0, 3);
+            fetch_counts(0, cA1, cA2);
+            fetch_counts(1, cB1, cB2);
+        }
         for (long long mb = 0; mb < g.nmb; ++mb) {
             const unsigned* rows_mb = rows_l + (size_t)mb * g.spm * W;
-            // the scan kernel's sums of this micro-batch (independent of the chain: read them early)
-            unsigned long long mine = 0ull;
-            if (tid < ncols)
-                for (int s = 0; s < g.spm; ++s) mine += rows_mb[(size_t)s * W + tid];
-            // steps 1-3: snapshot, guard, candidate tables of the replicated experts; the second warp fetches the
-            // record counts of the first 32 slices meanwhile
-            if (tid < 64) T.S[tid] = Ls[tid];
-            __syncthreads();
-            if (tid == 0) feas_s = load_guard(T.S, P, p.theta);
-            if (tid == 0) bigq_s = 0u;
-            if (tid >= 32 && tid < 64) load_counts(rows_mb, 0, min(32, g.spm), tid - 32);
-            // The records of the NEXT micro-batch do not depend on the chain: one bulk prefetch per slice and record class
-            // pulls them into L2 now (a single instruction each, issued by one lane of one CTA per slice).
-            if (tid >= 64 && tid < 128 && mb + 1 < g.nmb) {
-                const int sp = tid - 64;                       // slice of the next micro-batch
-                if (sp < g.spm && sp % CS == rank) {
-                    const unsigned* rn = rows_mb + ((size_t)g.spm + sp) * W + ncols;
-                    const unsigned n1 = rn[0], n2 = rn[1];
-                    if (n1 != kOverflow) {
-                        const Rec* rb = p.rec + rec_l + ((size_t)(mb + 1) * g.spm + sp) * (size_t)g.slice;
-                        if (n1) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rb), "r"(n1 * 16u) : "memory");
-                        if (n2) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rb + (g.slice - n2)), "r"(n2 * 16u) : "memory");
-                    }
+            // steps 1-2 by the first warp: guard of the snapshot (the EMA state: it only changes at the end of a
+            // micro-batch).  The second warp meanwhile publishes this micro-batch's record counts.
+            unsigned cC1 = 0u, cC2 = 0u;
+            if (tid < 32) {
+                const unsigned long long fm = load_guard_warp(Ls, P, p.theta, lane);
+                if (lane == 0) { feas_s = fm; bigq_s = 0u; }
+            } else if (tid < 64) {
+                fetch_counts(mb + 2, cC1, cC2);
+                if (lane == 0) prefetch_rows(mb + 3, mb + 4);
+                put_counts(cA1, cA2, lane);
+                // The records of the NEXT micro-batch do not depend on the chain: one bulk prefetch per slice and record
+                // class pulls them into L2 now (a single instruction each, issued by one lane of one CTA per slice).
+                if (mb + 1 < g.nmb && lane < ns0 && lane % CS == rank && cB1 != kOverflow) {
+                    const Rec* rb = p.rec + rec_l + ((size_t)(mb + 1) * g.spm + lane) * (size_t)g.slice;
+                    if (cB1) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rb), "r"(cB1 * 16u) : "memory");
+                    if (cB2) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rb + (g.slice - cB2)), "r"(cB2 * 16u) : "memory");
                 }
+            } else if (tid >= 128 && tid < 128 + ncols) {
+                // the scan kernel's sums of this micro-batch (independent of the chain; read again at step 5)
+                unsigned long long mine = 0ull;
+                for (int s = 0; s < g.spm; ++s) mine += rows_mb[(size_t)s * W + (tid - 128)];
+                mine_s[tid - 128] = mine;
             }
             __syncthreads();
             const unsigned long long feas = feas_s;
+            // step 3: candidate tables of the replicated experts
             for (int i = tid; i < nrep; i += kChainThreads) {
                 const int e = (int)replist[i];
                 unsigned char* out = T.cand + e * kCandStride;
-                build_candidate(e, r, T, feas, out);
+                if (r <= 3) build_candidate_small(e, r, T, feas, out);
+                else build_candidate(e, r, T, feas, out);
                 if (i < kMaxRank) {
                     // by rank: the one-hot masks of the first four candidates (entries beyond the count repeat the first)
                     const int n = out[0];
@@ -865,13 +963,15 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             if constexpr (CLUSTER) cg::this_cluster().sync();
             else __syncthreads();
             if (tid < P) {
-                unsigned long long d = mine;
+                unsigned long long d = mine_s[tid];
                 for (int q = 0; q < CS; ++q) d += exch[par][q][tid];
                 Ls[tid] = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
                 ltot[tid] += d;
             } else if (tid < ncols) {
-                csum[tid - P] += mine;
+                csum[tid - P] += mine_s[tid];
             }
+            cA1 = cB1; cA2 = cB2;
+            cB1 = cC1; cB2 = cC2;
             __syncthreads();
         }
         // layer epilogue: rank 0 adds the deferred tokens' communication sums of its peers and writes the outputs
@@ -1174,7 +1274,7 @@ template <typename M, bool OUT>
 int launch_chain(EvalCall& c) {
     tacg_ctx* ctx = c.ctx;
     const EvalGeom& g = c.cp.g;
-    const size_t smem = 64 * sizeof(double) + (((size_t)g.E * kCandStride + 15) & ~(size_t)15) +
+    const size_t smem = (((size_t)g.E * kCandStride + 15) & ~(size_t)15) +
                         (((size_t)g.E * g.r + 15) & ~(size_t)15) + sizeof(unsigned) * (size_t)g.P * 32 +
                         sizeof(unsigned) * (kChainThreads / 32) * 8 * 32 + sizeof(unsigned short) * (size_t)g.E + 16;
     // cluster size: as many CTAs per layer as the SM count allows, up to 16 (non-portable above 8)
