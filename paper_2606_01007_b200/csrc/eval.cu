@@ -649,12 +649,44 @@ struct ChainParams {
     unsigned char* cost;
     signed char* serve;
     int groups;                        // clusters in the grid; cluster c owns layers c, c + groups, ...
+    int gper;                          // kModeGrid: CTAs per layer
+    unsigned* gsync;                   // kModeGrid: [L][kSyncWords] zeroed before the launch (see layer_barrier)
 };
 
-// One cluster of CS CTAs per layer (CLUSTER = false: a plain CTA).  CTA `rank` takes the rank-th share of every
+// How the CTAs of one layer exchange the dispatch counts of a micro-batch.
+constexpr int kModeSingle = 0;    // one CTA per layer: nothing to exchange
+constexpr int kModeCluster = 1;   // one thread-block cluster per layer: distributed shared memory + the cluster barrier
+constexpr int kModeGrid = 2;      // few layers: more CTAs per layer than a cluster holds, launched cooperatively (all
+                                  // resident); counts through global atomics, one arrival counter per layer
+// per-layer words of ChainParams::gsync: counts[2][64] (cumulative, by micro-batch parity) | sums u64[16] | arrivals
+constexpr int kSyncSums = 128, kSyncBar = 160, kSyncWords = 192;
+
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* ptr) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ptr) : "memory");
+    return v;
+}
+
+// Barrier of the CTAs of one layer (kModeGrid; the launch is cooperative, so all of them are resident): the `n`-th
+// call returns once gper * n arrivals are counted.  What the CTA's threads wrote or added before is visible to every
+// CTA after.  A CTA that waits longer than seconds has met a bug, not a slow peer: it traps instead of hanging the GPU.
+__device__ __forceinline__ void layer_barrier(unsigned* bar, unsigned target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(bar, 1u);
+        const long long t0 = clock64();
+        while (ld_acquire_u32(bar) < target)
+            if (clock64() - t0 > (1ll << 33)) __trap();
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+// One cluster of CS CTAs per layer (MODE: kModeSingle a plain CTA, kModeGrid gper CTAs of a cooperative grid).  CTA `rank` takes the rank-th share of every
 // item's records; the integer dispatch counts of a micro-batch are exchanged through distributed shared
 // memory (two alternating buffers, one cluster barrier per micro-batch).
-template <typename M, bool OUT, bool CLUSTER>
+template <typename M, bool OUT, int MODE>
 __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const ChainParams p) {
     tacg_pdl_prologue();
     extern __shared__ __align__(16) unsigned char csm[];
@@ -674,6 +706,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     __shared__ unsigned long long ltot[64];    // cumulative integer load of this layer
     __shared__ unsigned long long csum[24];    // span | remote | tokens per family: rows of the scan kernel
     __shared__ unsigned long long dsum[16];    // span | remote of the deferred tokens handled by THIS CTA
+    __shared__ unsigned dsum32[16];            // the same for the current round of slices: 32-bit shared atomics are native,
+                                               // 64-bit ones are compare-and-swap loops that 16 warps contend on
     __shared__ unsigned exch[2][16][64];       // every cluster rank's dispatch counts of the micro-batch (even / odd):
                                                // each CTA stores its own row into all its peers before the barrier
     __shared__ unsigned wsum[kChainThreads / 32 + 1];
@@ -689,10 +723,13 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
 
     const int tid = threadIdx.x, lane = tid & 31;
     int rank = 0, CS = 1;
-    if constexpr (CLUSTER) {
+    if constexpr (MODE == kModeCluster) {
         cg::cluster_group cgl = cg::this_cluster();
         rank = (int)cgl.block_rank();
         CS = (int)cgl.num_blocks();
+    } else if constexpr (MODE == kModeGrid) {
+        CS = p.gper;
+        rank = (int)(blockIdx.x % (unsigned)CS);
     }
     const int cluster_id = blockIdx.x / CS;
     const unsigned cl = saddr(cnt + lane);
@@ -713,9 +750,12 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             ltot[tid] = 0ull;
         }
         if (tid < 24) csum[tid] = 0ull;
-        if (tid < 16) dsum[tid] = 0ull;
+        if (tid < 16) { dsum[tid] = 0ull; dsum32[tid] = 0u; }
         __syncthreads();
         const int nrep = build_ranks(E, T.ptab, rank8, replist, wsum);
+        unsigned* gsl = MODE == kModeGrid ? p.gsync + (size_t)layer * kSyncWords : nullptr;
+        unsigned gprev[2] = {0u, 0u};       // kModeGrid: the cumulative counts this thread read last, by parity
+        unsigned nbar = 0u;                 // kModeGrid: barriers of this layer passed so far
         const int16_t* base = p.indices + (size_t)layer * (size_t)g.N * (size_t)k;
         const unsigned* rows_l = p.rows + (size_t)layer * g.ipl * W;
         const size_t rec_l = (size_t)layer * g.ipl * g.slice;
@@ -731,11 +771,16 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     const unsigned sp = __reduce_add_sync(0xffffffffu, av & 0xffffu);
                     const unsigned rq = __reduce_add_sync(0xffffffffu, av >> 16);
                     if (lane == 0) {
-                        if (sp) atomicAdd(&dsum[fq], (unsigned long long)sp);
-                        if (rq) atomicAdd(&dsum[8 + fq], (unsigned long long)rq);
+                        if (sp) atomicAdd(&dsum32[fq], sp);
+                        if (rq) atomicAdd(&dsum32[8 + fq], rq);
                     }
                 }
             }
+        };
+        // a round of at most 32 slices adds less than 2^23 to a 32-bit sum; one thread per entry widens it between barriers
+        auto fold_dsum = [&](int i) {
+            dsum[i] += dsum32[i];
+            dsum32[i] = 0u;
         };
         // record counts of up to 32 slices (one pending slot | several) and their prefix sums; one warp
         auto put_counts = [&](unsigned n1, unsigned n2, int ln) {
@@ -856,6 +901,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 if (s0 > 0) {
                     __syncthreads();
                     if (tid < 32) load_counts(rows_mb, s0, ns, tid);
+                    else if (tid >= 96 && tid < 112) fold_dsum(tid - 96);
                     __syncthreads();
                 }
                 const size_t ro0 = rec_l + ((size_t)mb * g.spm + s0) * (size_t)g.slice;
@@ -953,29 +999,45 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             for (int m = tid >> 5; m < P; m += kChainThreads / 32) {
                 const unsigned sm = __reduce_add_sync(0xffffffffu, cnt[m * 32 + lane]);
                 cnt[m * 32 + lane] = 0u;
-                if constexpr (CLUSTER) {
+                if constexpr (MODE == kModeCluster) {
                     // lane q stores this CTA's count into rank q's table: after the barrier every CTA sums local words
                     if (lane < CS) cg::this_cluster().map_shared_rank(&exch[par][rank][m], lane)[0] = sm;
+                } else if constexpr (MODE == kModeGrid) {
+                    // cumulative per parity: nobody adds to this parity again before every CTA has passed the NEXT
+                    // barrier, that is, after every CTA has read it
+                    if (lane == 0 && sm) atomicAdd(gsl + par * 64 + m, sm);
                 } else {
                     if (lane == 0) exch[par][0][m] = sm;
                 }
             }
-            if constexpr (CLUSTER) cg::this_cluster().sync();
+            if constexpr (MODE == kModeCluster) cg::this_cluster().sync();
+            else if constexpr (MODE == kModeGrid) layer_barrier(gsl + kSyncBar, (unsigned)CS * ++nbar);
             else __syncthreads();
             if (tid < P) {
                 unsigned long long d = mine_s[tid];
-                for (int q = 0; q < CS; ++q) d += exch[par][q][tid];
+                if constexpr (MODE == kModeGrid) {
+                    const unsigned now = __ldcg(gsl + par * 64 + tid);
+                    d += now - gprev[par];
+                    gprev[par] = now;
+                } else {
+                    for (int q = 0; q < CS; ++q) d += exch[par][q][tid];
+                }
                 Ls[tid] = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
                 ltot[tid] += d;
             } else if (tid < ncols) {
                 csum[tid - P] += mine_s[tid];
             }
+            if (tid >= 96 && tid < 112) fold_dsum(tid - 96);
             cA1 = cB1; cA2 = cB2;
             cB1 = cC1; cB2 = cC2;
             __syncthreads();
         }
         // layer epilogue: rank 0 adds the deferred tokens' communication sums of its peers and writes the outputs
-        if constexpr (CLUSTER) cg::this_cluster().sync();
+        if constexpr (MODE == kModeCluster) cg::this_cluster().sync();
+        if constexpr (MODE == kModeGrid) {
+            if (tid < 16 && dsum[tid]) atomicAdd(reinterpret_cast<unsigned long long*>(gsl + kSyncSums) + tid, dsum[tid]);
+            layer_barrier(gsl + kSyncBar, (unsigned)CS * ++nbar);
+        }
         if (rank == 0) {
             if (tid < P) {
                 p.load[(size_t)layer * P + tid] = ltot[tid];
@@ -983,9 +1045,11 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             } else if (tid >= 64 && tid < 64 + 2 * F) {
                 const int which = (tid - 64) / F, f = (tid - 64) % F;
                 unsigned long long v = csum[which * F + f];
-                if constexpr (CLUSTER) {
+                if constexpr (MODE == kModeCluster) {
                     cg::cluster_group cgl = cg::this_cluster();
                     for (int q = 0; q < CS; ++q) v += cgl.map_shared_rank(&dsum[0], q)[which * 8 + f];
+                } else if constexpr (MODE == kModeGrid) {
+                    v += __ldcg(reinterpret_cast<const unsigned long long*>(gsl + kSyncSums) + which * 8 + f);
                 } else {
                     v += dsum[which * 8 + f];
                 }
@@ -994,7 +1058,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 p.ntok[tid - 128] = csum[2 * F + (tid - 128)];
             }
         }
-        if constexpr (CLUSTER) cg::this_cluster().sync();     // peers keep their sums until rank 0 has read them
+        if constexpr (MODE == kModeCluster) cg::this_cluster().sync();     // peers keep their sums until rank 0 has read them
     }
 }
 
@@ -1256,6 +1320,7 @@ struct EvalCall {
     ScanParams sp;
     ChainParams cp;
     bool rep, out;
+    int mode, cs, groups;      // chain_plan
 };
 
 template <int KT, bool REP, typename M, bool OUT>
@@ -1270,6 +1335,29 @@ int launch_scan(EvalCall& c) {
     return TACG_OK;
 }
 
+// How the chain kernel is launched for a geometry: cluster size (or CTAs per layer of a cooperative grid) and mode.
+void chain_plan(const tacg_ctx* ctx, const EvalGeom& g, int& mode, int& cs, int& groups) {
+    // cluster size: as many CTAs per layer as the SM count allows, up to 16 (non-portable above 8)
+    const int slots = 2 * ctx->sm_count;           // resident CTAs (two per SM)
+    const long long tokens = std::min<long long>(g.B, g.N);
+    cs = 1;
+    while (cs < 16 && (long long)g.L * cs * 2 <= slots) cs *= 2;
+    // a micro-batch with few records gains nothing from more CTAs
+    while (cs > 1 && tokens < (long long)cs * 2048) cs /= 2;
+    groups = std::min(g.L, std::max(1, slots / cs));
+    mode = cs > 1 ? kModeCluster : kModeSingle;
+    // few layers and long micro-batches: the largest cluster leaves most SMs idle.  One CTA per SM at most, about 1024
+    // tokens of a micro-batch per CTA.
+    if (cs == 16 && g.L * 32 <= ctx->sm_count && tokens >= 32 * 1024) {
+        const int want = (int)std::min<long long>(ctx->sm_count / g.L, tokens / 1024);
+        if (want > 16) {
+            mode = kModeGrid;
+            cs = want;
+            groups = g.L;
+        }
+    }
+}
+
 template <typename M, bool OUT>
 int launch_chain(EvalCall& c) {
     tacg_ctx* ctx = c.ctx;
@@ -1277,13 +1365,9 @@ int launch_chain(EvalCall& c) {
     const size_t smem = (((size_t)g.E * kCandStride + 15) & ~(size_t)15) +
                         (((size_t)g.E * g.r + 15) & ~(size_t)15) + sizeof(unsigned) * (size_t)g.P * 32 +
                         sizeof(unsigned) * (kChainThreads / 32) * 8 * 32 + sizeof(unsigned short) * (size_t)g.E + 16;
-    // cluster size: as many CTAs per layer as the SM count allows, up to 16 (non-portable above 8)
-    const int slots = 2 * ctx->sm_count;           // resident CTAs (two per SM)
-    int cs = 1;
-    while (cs < 16 && (long long)g.L * cs * 2 <= slots) cs *= 2;
-    // a micro-batch with few records gains nothing from more CTAs
-    while (cs > 1 && min(g.B, g.N) < (long long)cs * 2048) cs /= 2;
-    c.cp.groups = min(g.L, max(1, slots / cs));
+    const int cs = c.cs;
+    c.cp.groups = c.groups;
+    c.cp.gper = cs;
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3(c.cp.groups * cs);
@@ -1291,19 +1375,26 @@ int launch_chain(EvalCall& c) {
     cfg.dynamicSmemBytes = smem;
     cfg.stream = ctx->stream;
     cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = cs;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    if (cs > 1) {
-        auto kern = eval_chain_kernel<M, OUT, true>;
+    if (c.mode == kModeGrid) {
+        // every CTA of a layer waits for the others of that layer: cooperative, so the launch fails unless all fit
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        auto kern = eval_chain_kernel<M, OUT, kModeGrid>;
+        TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        TACG_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, c.cp));
+    } else if (c.mode == kModeCluster) {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = cs;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        auto kern = eval_chain_kernel<M, OUT, kModeCluster>;
         TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         if (cs > 8) TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         TACG_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, c.cp));
     } else {
-        auto kern = eval_chain_kernel<M, OUT, false>;
+        auto kern = eval_chain_kernel<M, OUT, kModeSingle>;
         TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         cfg.numAttrs = 0;
         TACG_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, c.cp));
@@ -1423,9 +1514,15 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         const size_t items = (size_t)L * (size_t)g.ipl;
         const size_t nrec = (c.rep && kt > 0) ? items * (size_t)g.slice : 0;      // one record per token at most
         const size_t o_rec = tacg_align_up(items * g.W * sizeof(unsigned), 256);
-        const size_t total = o_rec + nrec * sizeof(Rec);
+        c.mode = kModeSingle; c.cs = 1; c.groups = 1;
+        if (c.rep) chain_plan(ctx, g, c.mode, c.cs, c.groups);
+        const size_t o_sync = tacg_align_up(o_rec + nrec * sizeof(Rec), 256);
+        const size_t total = o_sync + (c.mode == kModeGrid ? (size_t)L * kSyncWords * sizeof(unsigned) : 0);
         char* sbase = static_cast<char*>(tacg_scratch(ctx, total));
         if (!sbase) return TACG_ERR_CUDA;
+        c.cp.gsync = reinterpret_cast<unsigned*>(sbase + o_sync);
+        if (c.mode == kModeGrid)
+            TACG_CUDA_TRY(ctx, cudaMemsetAsync(c.cp.gsync, 0, (size_t)L * kSyncWords * sizeof(unsigned), ctx->stream));
         c.sp.g = g;
         c.sp.indices = indices; c.sp.family = family; c.sp.primary = primary; c.sp.replicas = c.rep ? replicas : nullptr;
         c.sp.rows = reinterpret_cast<unsigned*>(sbase);
@@ -1442,7 +1539,7 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
         c.cp.ntok = reinterpret_cast<unsigned long long*>(ntok);
         c.cp.cost = cost_per_token;
         c.cp.serve = reinterpret_cast<signed char*>(serve);
-        c.cp.groups = 1;
+        c.cp.groups = 1; c.cp.gper = 1;
         int rc;
         {
             tacg_prof_scope prof(ctx, TACG_PROF_EVAL);

@@ -5,6 +5,7 @@
   * the literal per-token Eq. 15, microbatch = 1, on a long trace: one warp per layer, and the
     library's scratch must not grow with the number of micro-batches (ADVICE.md: round 1 reserved L*nmb*P*8 bytes);
   * short micro-batches on both sides of the switch between the one-warp kernel and the scan + chain kernels;
+  * few layers with long micro-batches: the chain kernel's cooperative grid mode;
   * shapes outside the record format of the scan kernel, which the chain kernel serves from the trace: odd k, more than
     15 replicated experts in a layer, P > 32 (64-bit partition sets), every expert replicated.
 """
@@ -82,6 +83,18 @@ def test_literal_per_token_ema_long_trace(tacg, ctx, cfg_id, N, L):
     _check(tacg, ctx, cfg.E, cfg.F, cfg.P, idx, fam, primary, replicas, 0.15, 0.995, 1, offset=3)
     # the call itself holds inputs and outputs (a few MB); scratch per micro-batch would be hundreds of MB here
     assert before - torch.cuda.mem_get_info()[0] < 256 * 1024 * 1024
+
+
+@pytest.mark.parametrize("cfg_id,N,L,B,offset", [(5, 300007, 1, 65536, 0), (3, 200000, 3, 40000, 5), (5, 150000, 4, 32768, 1),
+                                                  (4, 140000, 2, 65536, 9)])
+def test_few_layers_long_microbatches(tacg, ctx, cfg_id, N, L, B, offset):
+    """L <= 4 with micro-batches of 32 K tokens or more: more CTAs per layer than a cluster holds (cooperative launch,
+    counts exchanged through global memory), several micro-batches and a ragged last one."""
+    cfg, idx, fam = _trace(cfg_id, N, L)
+    primary = tracegen.random_placement(cfg.E, cfg.P, cfg.capacity, L, seed=15)
+    replicas = tracegen.random_replicas(primary, cfg.P, cfg.r, cfg.n_rep, seed=16)
+    _check(tacg, ctx, cfg.E, cfg.F, cfg.P, idx, fam, primary, replicas, 0.15, 0.995, B, offset=offset)
+    _check(tacg, ctx, cfg.E, cfg.F, cfg.P, idx, fam, primary, replicas, 0.05, 0.9, B, offset=offset, outputs=False)
 
 
 @pytest.mark.parametrize("B", [2, 31, 33, 512, 1023, 1024, 1025, 3000, 8192, 8193, 20000])
