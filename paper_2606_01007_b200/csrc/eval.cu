@@ -697,7 +697,6 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     T.cand = csm + off;                                    off += ((size_t)E * kCandStride + 15) & ~(size_t)15;
     T.rep = reinterpret_cast<signed char*>(csm + off);     off += ((size_t)E * r + 15) & ~(size_t)15;
     unsigned* cnt = reinterpret_cast<unsigned*>(csm + off);   off += sizeof(unsigned) * (size_t)P * 32;
-    unsigned* accb = reinterpret_cast<unsigned*>(csm + off);  off += sizeof(unsigned) * (kChainThreads / 32) * 8 * 32;
     unsigned short* replist = reinterpret_cast<unsigned short*>(csm + off);   // [E] ids of the replicated experts
     __shared__ unsigned char ptab_s[kPtab];
     __shared__ unsigned char rank8[kPtab];
@@ -733,8 +732,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     }
     const int cluster_id = blockIdx.x / CS;
     const unsigned cl = saddr(cnt + lane);
-    unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;
-    const unsigned al = saddr(acc);
+    const unsigned db = saddr(dsum32);
     const unsigned cmb = saddr(candm), pb1 = saddr(pre1), pb2 = saddr(pre2), nb1 = saddr(nrec1), nb2 = saddr(nrec2);
     const int W = g.W;
     const int ncols = P + 3 * F;               // row words summed by threads 0..ncols-1
@@ -743,8 +741,6 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         __syncthreads();
         load_ptab(E, r, p.primary + (size_t)layer * E, p.replicas + (size_t)layer * E * r, T.ptab, T.rep);
         for (int i = tid; i < P * 32; i += kChainThreads) cnt[i] = 0u;
-#pragma unroll
-        for (int f = 0; f < 8; ++f) acc[f * 32] = 0u;
         if (tid < 64) {
             Ls[tid] = (p.load_state && tid < P) ? p.load_state[(size_t)layer * P + tid] : 0.0;
             ltot[tid] = 0ull;
@@ -760,23 +756,6 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         const unsigned* rows_l = p.rows + (size_t)layer * g.ipl * W;
         const size_t rec_l = (size_t)layer * g.ipl * g.slice;
 
-        // per-family sums of this thread's deferred tokens -> CTA.  16-bit fields: a thread takes at most 9 tokens
-        // per item, each <= 16, so they are flushed at least every 256 items
-        auto flush_acc = [&]() {
-#pragma unroll
-            for (int fq = 0; fq < 8; ++fq) {
-                if (fq < F) {
-                    const unsigned av = acc[fq * 32];
-                    acc[fq * 32] = 0u;
-                    const unsigned sp = __reduce_add_sync(0xffffffffu, av & 0xffffu);
-                    const unsigned rq = __reduce_add_sync(0xffffffffu, av >> 16);
-                    if (lane == 0) {
-                        if (sp) atomicAdd(&dsum32[fq], sp);
-                        if (rq) atomicAdd(&dsum32[8 + fq], rq);
-                    }
-                }
-            }
-        };
         // a round of at most 32 slices adds less than 2^23 to a 32-bit sum; one thread per entry widens it between barriers
         auto fold_dsum = [&](int i) {
             dsum[i] += dsum32[i];
@@ -827,6 +806,24 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(rp), "r"(bytes) : "memory");
             }
         };
+        // step 3 for the replicated expert of rank i + 1: its candidates in the order of the snapshot
+        auto cand_of = [&](int i, unsigned long long feas) {
+            const int e = (int)replist[i];
+            unsigned char* out = T.cand + e * kCandStride;
+            if (r <= 3) build_candidate_small(e, r, T, feas, out);
+            else build_candidate(e, r, T, feas, out);
+            if (i < kMaxRank) {
+                // by rank: the one-hot masks of the first four candidates (entries beyond the count repeat the first)
+                const int n = out[0];
+                M* cm = reinterpret_cast<M*>(candm) + (i + 1) * 4;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) cm[q] = (M)1 << out[1 + (q < n ? q : 0)];
+                if (n > 4) atomicOr(&bigq_s, 1u << (i + 1));
+                unsigned* dst = reinterpret_cast<unsigned*>(candr + (i + 1) * kCandStride);
+                const unsigned* src = reinterpret_cast<const unsigned*>(out);
+                dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
+            }
+        };
         unsigned cA1 = 0u, cA2 = 0u, cB1 = 0u, cB2 = 0u;
         if (tid >= 32 && tid < 64) {
             if (lane == 0) prefetch_rows(0, 3);
@@ -841,6 +838,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             if (tid < 32) {
                 const unsigned long long fm = load_guard_warp(Ls, P, p.theta, lane);
                 if (lane == 0) { feas_s = fm; bigq_s = 0u; }
+                __syncwarp();
+                if (lane < nrep && nrep <= 32) cand_of(lane, fm);       // step 3: the usual case, no second barrier
             } else if (tid < 64) {
                 fetch_counts(mb + 2, cC1, cC2);
                 if (lane == 0) prefetch_rows(mb + 3, mb + 4);
@@ -859,27 +858,14 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 mine_s[tid - 128] = mine;
             }
             __syncthreads();
-            const unsigned long long feas = feas_s;
-            // step 3: candidate tables of the replicated experts
-            for (int i = tid; i < nrep; i += kChainThreads) {
-                const int e = (int)replist[i];
-                unsigned char* out = T.cand + e * kCandStride;
-                if (r <= 3) build_candidate_small(e, r, T, feas, out);
-                else build_candidate(e, r, T, feas, out);
-                if (i < kMaxRank) {
-                    // by rank: the one-hot masks of the first four candidates (entries beyond the count repeat the first)
-                    const int n = out[0];
-                    M* cm = reinterpret_cast<M*>(candm) + (i + 1) * 4;
-#pragma unroll
-                    for (int q = 0; q < 4; ++q) cm[q] = (M)1 << out[1 + (q < n ? q : 0)];
-                    if (n > 4) atomicOr(&bigq_s, 1u << (i + 1));
-                    unsigned* dst = reinterpret_cast<unsigned*>(candr + (i + 1) * kCandStride);
-                    const unsigned* src = reinterpret_cast<const unsigned*>(out);
-                    dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
-                }
+            // step 3 when the first warp could not take it
+            if (nrep > 32) {
+                const unsigned long long feas = feas_s;
+                for (int i = tid; i < nrep; i += kChainThreads) cand_of(i, feas);
+                __syncthreads();
             }
-            __syncthreads();
             const unsigned bigq = bigq_s;
+
             // one pending slot: rank q of the replicated expert, loc = accessed set so far | home; returns the pick
             auto pick_slot = [&](unsigned q, M loc) -> M {
                 M m1, m2, m3, m4;
@@ -930,7 +916,9 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     }
                     const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~hb);
                     if (OUT && p.cost) p.cost[token_of(x, meta)] = (unsigned char)rem;
-                    sred_add(al + ((meta >> 13) & 7u) * 128u, (unsigned)max(0, nR - 1) | ((unsigned)rem << 16));
+                    // per-family sums of the CTA: lanes of one family hit one word, which the atomic unit merges
+                    sred_add(db + ((meta >> 13) & 7u) * 4u, (unsigned)max(0, nR - 1));
+                    sred_add(db + 32u + ((meta >> 13) & 7u) * 4u, (unsigned)rem);
                 };
 #pragma unroll 1
                 for (int cls = 0; cls < 2; ++cls) {
@@ -987,11 +975,10 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                         if (OUT && p.cost) p.cost[(size_t)layer * g.N + t0 + o] = (unsigned char)rem;
                         if (OUT && p.serve)
                             for (int j = 0; j < k; ++j) p.serve[((size_t)layer * g.N + t0 + o) * k + j] = (signed char)sv[j];
-                        sred_add(al + (unsigned)fq * 128u, (unsigned)max(0, nR - 1) | ((unsigned)rem << 16));
+                        sred_add(db + (unsigned)fq * 4u, (unsigned)max(0, nR - 1));
+                        sred_add(db + 32u + (unsigned)fq * 4u, (unsigned)rem);
                     }
                 }
-                // 16-bit fields: a thread takes at most 32 * 8192 / 1024 tokens of <= 16 each per round
-                flush_acc();
             }
             // step 5: integer dispatch counts of the micro-batch, then Eq. 15
             __syncthreads();
@@ -1364,7 +1351,7 @@ int launch_chain(EvalCall& c) {
     const EvalGeom& g = c.cp.g;
     const size_t smem = (((size_t)g.E * kCandStride + 15) & ~(size_t)15) +
                         (((size_t)g.E * g.r + 15) & ~(size_t)15) + sizeof(unsigned) * (size_t)g.P * 32 +
-                        sizeof(unsigned) * (kChainThreads / 32) * 8 * 32 + sizeof(unsigned short) * (size_t)g.E + 16;
+                        sizeof(unsigned short) * (size_t)g.E + 16;
     const int cs = c.cs;
     c.cp.groups = c.groups;
     c.cp.gper = cs;
