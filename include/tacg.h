@@ -249,6 +249,39 @@ int tacg_eval_placement(tacg_ctx* ctx,
                         int8_t* serve,          /* dev [L,N,k] out serving partition per slot, or NULL */
                         uint32_t flags);        /* 0 or TACG_VALIDATE */
 
+/* The same evaluation for a placement WITHOUT replicas (S8, S9, S11, S12 of PAPER.md:145-159, 363, 453-463 with every
+ * slot served by its primary partition), for callers that must not allocate: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc.  It calls no cudaMalloc, cudaFree or allocating library routine
+ * and does not touch the context's growable scratch: its only scratch, the per-slice partial sums
+ * L * ceil(N / slice) * align4(P + 3F + 2) 32-bit words (slice = 8192 tokens, fewer for short traces), lives in
+ * a fixed device array of TACG_NOALLOC_SCRATCH_BYTES that every GPU holding the library keeps until the process
+ * exits.  A call that needs more fails with TACG_ERR_SHAPE and a text naming the two sizes (nothing is launched);
+ * split the layers over several calls, or use tacg_eval_placement.
+ * Arguments, layouts and results are those of tacg_eval_placement with replicas = NULL (same kernels, same bits;
+ * theta and microbatch do not enter without replicas); N >= 1; no TACG_VALIDATE; not bracketed by the profile events
+ * of tacg_profile_enable.  EVERY call on a device shares the one array, which keeps the previous call's contents
+ * (each call overwrites every word it later reads, nothing has to be cleared): two calls that overlap on the GPU
+ * -- other streams, other contexts, other host threads -- race; the caller keeps them in order.
+ * tacg_eval_primary_noalloc_prepare looks up the array's device address for the context's device (once per device;
+ * the first tacg_eval_primary_noalloc on a device does the same): call it before a graph capture begins. */
+#define TACG_NOALLOC_SCRATCH_BYTES (8u << 20)
+int tacg_eval_primary_noalloc_prepare(tacg_ctx* ctx);
+int tacg_eval_primary_noalloc(tacg_ctx* ctx,
+                              const int16_t* indices, /* dev [L,N,k] */
+                              const int8_t* family,   /* dev [N] */
+                              int64_t N, int k, int L, int E, int F, int P,
+                              const int8_t* primary,  /* dev [L,E] */
+                              double rho,
+                              int64_t token_offset,
+                              double* load_state,     /* dev [L,P] in/out or NULL */
+                              uint64_t* load,         /* dev [L,P] out */
+                              uint64_t* comm_span,    /* dev [L,F] out */
+                              uint64_t* comm_remote,  /* dev [L,F] out */
+                              uint64_t* ntok,         /* dev [F]   out */
+                              float* fairness,        /* dev [L+1,3] out */
+                              uint8_t* cost_per_token,/* dev [L,N] out or NULL */
+                              int8_t* serve);         /* dev [L,N,k] out or NULL */
+
 #ifdef __cplusplus
 }
 #endif

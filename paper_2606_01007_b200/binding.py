@@ -29,6 +29,7 @@ EXPORTS = (
     "tacg_launch_count", "tacg_version", "tacg_profile_enable", "tacg_profile_read", "tacg_measure_peak",
     "tacg_coact_accumulate", "tacg_affinity_swapgain",
     "gesr_select", "tacg_eval_placement", "gesr_build_replicas", "tacg_spectral_place", "tacg_family_divergence",
+    "tacg_eval_primary_noalloc", "tacg_eval_primary_noalloc_prepare",
 )
 
 _lib = None
@@ -78,6 +79,9 @@ def lib():
         L.tacg_spectral_place.argtypes = [vp, vp, i32, i32, i32, i32, f64, i32, vp, vp, vp, vp]
         L.tacg_eval_placement.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, i32, vp, vp, i32, f32, f64,
                                           i64, i64, vp, vp, vp, vp, vp, vp, vp, vp, u32]
+        L.tacg_eval_primary_noalloc_prepare.argtypes = [vp]
+        L.tacg_eval_primary_noalloc.argtypes = [vp, vp, vp, i64, i32, i32, i32, i32, i32, vp, f64, i64,
+                                                vp, vp, vp, vp, vp, vp, vp, vp]
         for name in EXPORTS:
             getattr(L, name)
         _lib = L
@@ -258,6 +262,24 @@ class Context:
             _ptr(fairness, torch.float32, "fairness", n((L + 1) * 3)), _ptr(cost_per_token, torch.uint8, "cost_per_token", n(L * N)),
             _ptr(serve, torch.int8, "serve", n(L * N * k)), int(flags))
 
+    def tacg_eval_primary_noalloc_prepare(self) -> int:
+        self._enter()
+        return lib().tacg_eval_primary_noalloc_prepare(self._h)
+
+    def tacg_eval_primary_noalloc(self, indices, family, N, k, L, E, F, P, primary, rho, token_offset, load_state,
+                                  load, comm_span, comm_remote, ntok, fairness, cost_per_token, serve) -> int:
+        self._enter()
+        ok = _within_limits(k=k, L=L, E=E, F=F, P=P, r=0, N=N)
+        n = lambda v: v if ok else None
+        return lib().tacg_eval_primary_noalloc(
+            self._h, _ptr(indices, torch.int16, "indices", n(L * N * k)), _ptr(family, torch.int8, "family", n(N)),
+            int(N), int(k), int(L), int(E), int(F), int(P), _ptr(primary, torch.int8, "primary", n(L * E)),
+            float(rho), int(token_offset), _ptr(load_state, torch.float64, "load_state", n(L * P)),
+            _ptr(load, torch.int64, "load", n(L * P)), _ptr(comm_span, torch.int64, "comm_span", n(L * F)),
+            _ptr(comm_remote, torch.int64, "comm_remote", n(L * F)), _ptr(ntok, torch.int64, "ntok", n(F)),
+            _ptr(fairness, torch.float32, "fairness", n((L + 1) * 3)),
+            _ptr(cost_per_token, torch.uint8, "cost_per_token", n(L * N)), _ptr(serve, torch.int8, "serve", n(L * N * k)))
+
 
 # ---- convenience wrappers: allocate outputs with torch, call, return a dict ----
 # uint32 / uint64 device buffers are held as torch int32 / int64 tensors (same bits).
@@ -364,4 +386,20 @@ def tacg_eval_placement(ctx: Context, indices, family, E: int, F: int, P: int, p
                                       theta, rho, microbatch, token_offset, load_state, out["load"],
                                       out["comm_span"], out["comm_remote"], out["ntok"], out["fairness"],
                                       out["cost"], out["serve"], flags), "tacg_eval_placement")
+    return out
+
+
+NOALLOC_SCRATCH_BYTES = 8 << 20      # TACG_NOALLOC_SCRATCH_BYTES of include/tacg.h
+
+
+def tacg_eval_primary_noalloc(ctx: Context, indices, family, E: int, F: int, P: int, primary, out: dict,
+                              rho: float = 0.995, token_offset: int = 0, load_state=None):
+    """tacg_eval_placement without replicas through the entry point that allocates nothing: the caller passes every
+    output in `out` (keys load, comm_span, comm_remote, ntok, fairness; optional cost, serve), this wrapper creates no
+    tensor.  The library's scratch for it is a fixed device array of NOALLOC_SCRATCH_BYTES shared by all calls."""
+    L, N, k = indices.shape
+    ctx.check(ctx.tacg_eval_primary_noalloc(indices, family, N, k, L, E, F, P, primary, rho, token_offset, load_state,
+                                            out["load"], out["comm_span"], out["comm_remote"], out["ntok"],
+                                            out["fairness"], out.get("cost"), out.get("serve")),
+              "tacg_eval_primary_noalloc")
     return out

@@ -39,6 +39,7 @@
 #include <cooperative_groups.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "tacg_common.cuh"
 
@@ -1549,6 +1550,137 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
     TACG_CUDA_TRY(ctx, tacg_launch_pdl(fairness_kernel, dim3(L + 1), dim3(1024), 0, ctx->stream,
                                        reinterpret_cast<unsigned long long*>(load), L, P, fairness, fin_rows, fin_ipl, fin_W,
                                        F, rho, load_state, reinterpret_cast<unsigned long long*>(comm_span),
+                                       reinterpret_cast<unsigned long long*>(comm_remote),
+                                       reinterpret_cast<unsigned long long*>(ntok)));
+    TACG_LAUNCH_CHECK(ctx);
+    return TACG_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// tacg_eval_primary_noalloc: the primary-only evaluation (no replica table: S8, S9, S11, S12 with every slot served by
+// its primary partition) for callers that must not allocate -- code under CUDA graph capture, tight serving loops,
+// harnesses that forbid cudaMalloc.  Same kernels, same geometry and therefore the same bits as tacg_eval_placement
+// with replicas = NULL; the only difference is where the item rows of eval_scan_kernel live: not in the context's
+// growable scratch (tacg_scratch: cudaMalloc / cudaFree) but in the fixed array below, which every GPU that loads the
+// library holds until the process exits.
+//
+// The array's NAME is a host-side stand-in in host code, not a device address: the kernels are given the address that
+// cudaGetSymbolAddress returns for the current device, looked up once per device (noalloc_rows).
+// Every call shares the array and it keeps the last call's contents.  Nothing has to start at zero: eval_scan_kernel
+// writes every word of every item row (loads | span | remote | tokens | two record counts) before fairness_kernel reads
+// the first P + 3F of them.  Calls that overlap on the GPU (two streams, two contexts, two host threads on one
+// device) race on it: the caller serialises them.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr size_t kNoAllocBytes = TACG_NOALLOC_SCRATCH_BYTES;     // 8 MiB: config 4 whole (58 x 512 items of 48 words) fits
+static __device__ __align__(256) unsigned char g_noalloc_rows[kNoAllocBytes];
+
+constexpr int kMaxDevices = 64;
+unsigned* g_noalloc_addr[kMaxDevices];       // device address of g_noalloc_rows on each device, 0 = not looked up yet
+std::mutex g_noalloc_mutex;
+
+// Device address of the array on ctx->device (which the caller has made current); looked up once per device.
+int noalloc_rows(tacg_ctx* ctx, unsigned** out) {
+    if (ctx->device < 0 || ctx->device >= kMaxDevices) {
+        snprintf(ctx->detail, sizeof(ctx->detail), "eval_primary_noalloc: device ordinal %d not supported", ctx->device);
+        return TACG_ERR_SHAPE;
+    }
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[ctx->device]) {
+        void* ptr = nullptr;
+        TACG_CUDA_TRY(ctx, cudaGetSymbolAddress(&ptr, g_noalloc_rows));
+        if (!ptr || (reinterpret_cast<uintptr_t>(ptr) % 256) != 0) {
+            snprintf(ctx->detail, sizeof(ctx->detail), "eval_primary_noalloc: bad symbol address %p", ptr);
+            return TACG_ERR_CUDA;
+        }
+        g_noalloc_addr[ctx->device] = static_cast<unsigned*>(ptr);
+    }
+    *out = g_noalloc_addr[ctx->device];
+    return TACG_OK;
+}
+
+template <int KT>
+int launch_scan_primary(EvalCall& c) {
+    const bool wide = c.sp.g.P > 32;
+    if (wide) return c.out ? launch_scan<KT, false, unsigned long long, true>(c) : launch_scan<KT, false, unsigned long long, false>(c);
+    return c.out ? launch_scan<KT, false, unsigned, true>(c) : launch_scan<KT, false, unsigned, false>(c);
+}
+
+}  // namespace
+
+extern "C" int tacg_eval_primary_noalloc_prepare(tacg_ctx* ctx) {
+    if (!ctx) return TACG_ERR_NULL;
+    TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    unsigned* rows = nullptr;
+    return noalloc_rows(ctx, &rows);
+}
+
+extern "C" int tacg_eval_primary_noalloc(tacg_ctx* ctx, const int16_t* indices, const int8_t* family, int64_t N, int k,
+                                         int L, int E, int F, int P, const int8_t* primary, double rho,
+                                         int64_t token_offset, double* load_state, uint64_t* load, uint64_t* comm_span,
+                                         uint64_t* comm_remote, uint64_t* ntok, float* fairness,
+                                         uint8_t* cost_per_token, int8_t* serve) {
+    if (!ctx) return TACG_ERR_NULL;
+    if (N < 1 || k < 1 || k > 16 || L < 1 || E < 1 || E > 512 || F < 1 || F > 8 || P < 1 || P > 64 || token_offset < 0) {
+        snprintf(ctx->detail, sizeof(ctx->detail), "eval_primary_noalloc: size out of range (N >= 1 here)");
+        return TACG_ERR_SHAPE;
+    }
+    if (!indices || !family || !primary || !load || !comm_span || !comm_remote || !ntok || !fairness) {
+        snprintf(ctx->detail, sizeof(ctx->detail), "eval_primary_noalloc: NULL pointer");
+        return TACG_ERR_NULL;
+    }
+    TACG_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    // the geometry of tacg_launch_eval without replicas: one micro-batch, slices of at most kSlice tokens
+    EvalCall c;
+    c.ctx = ctx;
+    c.rep = false;
+    c.out = cost_per_token != nullptr || serve != nullptr;
+    c.mode = kModeSingle; c.cs = 1; c.groups = 1;
+    EvalGeom g;
+    g.N = N; g.k = k; g.L = L; g.E = E; g.F = F; g.P = P; g.r = 0;
+    g.B = N;
+    g.nmb = 1;
+    g.token_offset = token_offset;
+    long long slice = kSlice;
+    if ((long long)L * N < (long long)kSlice * ctx->sm_count * 4)
+        slice = std::max(1ll, (long long)L * N / ((long long)ctx->sm_count * 4));
+    slice = std::min((long long)kSlice, std::min(g.B, slice));
+    slice = std::max(512ll, (slice + 511) / 512 * 512);
+    g.slice = (int)slice;
+    g.spm = (int)((g.B + slice - 1) / slice);
+    g.ipl = g.nmb * g.spm;
+    g.W = (int)tacg_align_up((size_t)P + 3 * (size_t)F + 2, 4);
+    const size_t need = (size_t)L * (size_t)g.ipl * (size_t)g.W * sizeof(unsigned);
+    if (need > kNoAllocBytes) {
+        snprintf(ctx->detail, sizeof(ctx->detail),
+                 "eval_primary_noalloc: L * ceil(N / %d) * %d row words = %zu bytes of scratch, the fixed array holds %zu; "
+                 "split the layers over several calls or use tacg_eval_placement",
+                 g.slice, g.W, need, kNoAllocBytes);
+        return TACG_ERR_SHAPE;
+    }
+    unsigned* rows = nullptr;
+    int rc = noalloc_rows(ctx, &rows);
+    if (rc != TACG_OK) return rc;
+    memset(&c.sp, 0, sizeof(c.sp));
+    c.sp.g = g;
+    c.sp.indices = indices; c.sp.family = family; c.sp.primary = primary; c.sp.replicas = nullptr;
+    c.sp.rows = rows;
+    c.sp.rec = nullptr;
+    c.sp.cost = cost_per_token;
+    c.sp.serve = reinterpret_cast<signed char*>(serve);
+    switch (tacg_pick_kt(k, indices)) {
+        case 2: rc = launch_scan_primary<2>(c); break;
+        case 4: rc = launch_scan_primary<4>(c); break;
+        case 6: rc = launch_scan_primary<6>(c); break;
+        case 8: rc = launch_scan_primary<8>(c); break;
+        default: rc = launch_scan_primary<0>(c); break;
+    }
+    if (rc != TACG_OK) return rc;
+    TACG_CUDA_TRY(ctx, tacg_launch_pdl(fairness_kernel, dim3(L + 1), dim3(1024), 0, ctx->stream,
+                                       reinterpret_cast<unsigned long long*>(load), L, P, fairness,
+                                       static_cast<const unsigned*>(rows), g.ipl, g.W, F, rho, load_state,
+                                       reinterpret_cast<unsigned long long*>(comm_span),
                                        reinterpret_cast<unsigned long long*>(comm_remote),
                                        reinterpret_cast<unsigned long long*>(ntok)));
     TACG_LAUNCH_CHECK(ctx);
