@@ -59,7 +59,8 @@ constexpr unsigned kBadFlag = 0x40u; // ptab bit: not an expert (empty slot, id 
 constexpr int kPtab = 516;           // ids are clamped to 512; entry 512 is "not an expert"
 constexpr int kSink = 64;            // counter row of the slots the scan kernel does not count
 constexpr int kMaxRank = 15;         // replicated experts per layer the 4-bit rank fields can name
-constexpr unsigned kT16Bad = 0x8000u;
+constexpr unsigned kCntAlign = 16384u;  // eval_scan_kernel's counter block (see there)
+constexpr unsigned kT16Bad = 0x10u;     // tab16 entry: row << 7 (bits 7..13) | rank (bits 0..3) | kT16Bad
 constexpr unsigned kOverflow = 0xffffffffu;   // record count of an item the chain kernel serves from the trace
 
 struct LayerTables {
@@ -384,11 +385,13 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
     constexpr int U = KT > 0 ? kEvalBatch : 1;
     constexpr bool RECS = REP && KT > 0;      // the record format covers compile-time k only
     extern __shared__ __align__(16) unsigned char esm[];
-    unsigned* cnt = reinterpret_cast<unsigned*>(esm);                      // [65][32]: lane-private columns, row 64 = sink
+    // [65][32] lane-private columns, row 64 = sink; on a 16 KB boundary of the shared window, so that a counter's address
+    // is (table entry & 0x3f80) | column address: one LOP3 per slot
+    unsigned* cnt = reinterpret_cast<unsigned*>(esm + ((kCntAlign - (saddr(esm) & (kCntAlign - 1u))) & (kCntAlign - 1u)));
     unsigned* accb = cnt + (kSink + 1) * 32;                               // [warps][8][32] per-thread family words
     __shared__ unsigned char ptab[kPtab];
     __shared__ unsigned char rank8[kPtab];
-    __shared__ unsigned short tab16[kPtab];   // row (7) | rank << 8 | kT16Bad
+    __shared__ unsigned short tab16[kPtab];   // row << 7 | rank | kT16Bad: the row field is the counter row's byte offset
     __shared__ unsigned comm_s[16];           // span[8] | remote[8] of this item
     __shared__ unsigned fam_s[8];
     __shared__ unsigned wsum[kEvalThreads / 32 + 1];
@@ -428,9 +431,9 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
             for (int e = tid; e < kPtab; e += kEvalThreads) {
                 const unsigned v = ptab[e];
                 unsigned t16;
-                if (v & kBadFlag) t16 = kSink | kT16Bad;
-                else if (v & kRepFlag) t16 = kSink | ((REP ? (unsigned)rank8[e] & 15u : 0u) << 8);
-                else t16 = v & 63u;
+                if (v & kBadFlag) t16 = (kSink << 7) | kT16Bad;
+                else if (v & kRepFlag) t16 = (kSink << 7) | (REP ? (unsigned)rank8[e] & 15u : 0u);
+                else t16 = (v & 63u) << 7;
                 tab16[e] = (unsigned short)t16;
             }
             cur_layer = layer;
@@ -489,21 +492,14 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                     unsigned a2[KM];            // byte offsets into the table (tab16 with replicas, else the byte table)
                     constexpr unsigned SC = REP ? 2u : 1u;      // bytes per table entry
                     if constexpr (KT > 0) {
-                        unsigned orw = 0u;
 #pragma unroll
                         for (int i = 0; i < NW; ++i) {
-                            if constexpr (REP) {
-                                a2[2 * i] = (w[u][i] << 1) & 0x1fffeu;
-                                a2[2 * i + 1] = (w[u][i] >> 15) & 0x1fffeu;
-                            } else {
-                                a2[2 * i] = w[u][i] & 0xffffu;
-                                a2[2 * i + 1] = w[u][i] >> 16;
-                            }
-                            orw |= w[u][i];
-                        }
-                        if (orw & 0xfe00fe00u) {       // an id outside [0,512): clamp to the "not an expert" entry
-#pragma unroll
-                            for (int j = 0; j < KM; ++j) a2[j] = min(a2[j], 512u * SC);
+                            // both ids of the word at once: anything outside [0,512) becomes 512, the "not an expert"
+                            // entry (unsigned 16-bit minimum: -1 = 0xffff, an empty slot, included)
+                            const unsigned wc = __vminu2(w[u][i], 0x02000200u);
+                            const unsigned ws = REP ? wc + wc : wc;     // ids <= 512: the doubling does not carry
+                            a2[2 * i] = ws & 0xffffu;
+                            a2[2 * i + 1] = ws >> 16;
                         }
                     } else {
 #pragma unroll
@@ -523,18 +519,19 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                     unsigned ranks = 0u;
 #pragma unroll
                     for (int j = 0; j < KM; ++j) {
-                        const unsigned row = REP ? (t[j] & 0x7fu) : t[j];
+                        const unsigned row = REP ? (t[j] >> 7) : t[j];
                         TACG_ASSERT(a2[j] <= 512u * SC && (row < (unsigned)P || row == (unsigned)kSink));
                         R |= bit_or_zero<M>(row);
-                        sred_inc(cl + row * 128u);
-                        if (RECS && j < 8) ranks |= ((t[j] >> 8) & 15u) << (4 * j);
+                        if constexpr (REP) sred_inc((t[j] & 0x3f80u) | cl);      // the row field is the byte offset of the row
+                        else sred_inc(cl + row * 128u);
+                        if (RECS && j < 8) ranks |= (t[j] & 15u) << (4 * j);
                     }
                     if constexpr (OUT) {
                         if (serve_l) {
                             signed char* out = serve_l + (size_t)o * k;
 #pragma unroll
                             for (int j = 0; j < KM; ++j)
-                                if (j < k) out[j] = ((REP ? (t[j] & kT16Bad) : (t[j] & kBadFlag)) != 0u) ? (signed char)-1 : (signed char)(t[j] & 0x3fu);
+                                if (j < k) out[j] = ((REP ? (t[j] & kT16Bad) : (t[j] & kBadFlag)) != 0u) ? (signed char)-1 : (signed char)((REP ? t[j] >> 7 : t[j]) & 0x3fu);
                         }
                     }
                     unsigned packed = 1u << 22;          // one token of family f
@@ -1315,7 +1312,7 @@ template <int KT, bool REP, typename M, bool OUT>
 int launch_scan(EvalCall& c) {
     tacg_ctx* ctx = c.ctx;
     auto kern = eval_scan_kernel<KT, REP, M, OUT>;
-    const size_t smem = sizeof(unsigned) * (kSink + 1) * 32 + sizeof(unsigned) * (kEvalThreads / 32) * 8 * 32;
+    const size_t smem = kCntAlign + sizeof(unsigned) * (kSink + 1) * 32 + sizeof(unsigned) * (kEvalThreads / 32) * 8 * 32;
     const long long T = (long long)c.sp.g.L * c.sp.g.ipl;
     const int grid = (int)max(1ll, min(T, (long long)ctx->sm_count * 2));
     TACG_CUDA_TRY(ctx, tacg_launch_pdl(kern, dim3(grid), dim3(kEvalThreads), smem, ctx->stream, c.sp));
