@@ -39,6 +39,7 @@
 #include <cooperative_groups.h>
 
 #include <algorithm>
+#include <type_traits>
 #include <mutex>
 
 #include "tacg_common.cuh"
@@ -864,7 +865,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             }
             const unsigned bigq = bigq_s;
 
-            // one pending slot: rank q of the replicated expert, loc = accessed set so far | home; returns the pick
+            // one pending slot: rank q of the replicated expert, loc = accessed set so far | home; returns the pick:
+            // the first of the (at most four) candidates in snapshot order that is local, else the first.  No branch.
             auto pick_slot = [&](unsigned q, M loc) -> M {
                 M m1, m2, m3, m4;
                 if constexpr (sizeof(M) == 4) {
@@ -873,8 +875,12 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     asm volatile("ld.shared.v2.u64 {%0,%1}, [%2];" : "=l"(m1), "=l"(m2) : "r"(cmb + q * 32u));
                     asm volatile("ld.shared.v2.u64 {%0,%1}, [%2];" : "=l"(m3), "=l"(m4) : "r"(cmb + q * 32u + 16u));
                 }
-                M pm = (loc & m1) ? m1 : ((loc & m2) ? m2 : ((loc & m3) ? m3 : ((loc & m4) ? m4 : m1)));
-                if (((bigq >> q) & 1u) && !(loc & (m1 | m2 | m3 | m4)))          // more than four candidates listed
+                M pm = m1;
+                pm = (loc & m4) ? m4 : pm;
+                pm = (loc & m3) ? m3 : pm;
+                pm = (loc & m2) ? m2 : pm;
+                pm = (loc & m1) ? m1 : pm;
+                if (r > 3 && ((bigq >> q) & 1u) && !(loc & (m1 | m2 | m3 | m4)))     // more than four candidates listed
                     pm = (M)1 << pick_candidate<M>(candr + q * kCandStride, loc);
                 return pm;
             };
@@ -898,19 +904,28 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     item_tokens(g, mb, s0 + (int)(x / slice), t0, t1);
                     return (size_t)layer * g.N + t0 + (meta & 0x1fffu);
                 };
-                // one record: its pending slots in slot order (lowest nibble first), then the communication cost
-                auto resolve = [&](M R, unsigned rk, unsigned meta, unsigned x) {
+                // the pending slot whose rank sits at bit sh of the record's rank word
+                auto step = [&](M& R, M hb, unsigned rk, int sh, unsigned meta, unsigned x) {
+                    TACG_ASSERT(((rk >> sh) & 15u) >= 1u && (int)((rk >> sh) & 15u) <= nrep);
+                    const M pm = pick_slot((rk >> sh) & 15u, R | hb);
+                    R |= pm;
+                    const int pick = sizeof(M) == 8 ? 63 - __clzll((long long)pm) : 31 - __clz((int)pm);
+                    TACG_ASSERT(pick >= 0 && pick < P);
+                    sred_inc(cl + (unsigned)pick * 128u);
+                    if (OUT && p.serve) p.serve[token_of(x, meta) * k + (sh >> 2)] = (signed char)pick;
+                };
+                // one record: its pending slots in slot order (lowest nibble first), then the communication cost.
+                // MULTI = false: the record class with exactly one pending slot, no loop.
+                auto resolve = [&](auto MULTI, M R, unsigned rk, unsigned meta, unsigned x) {
                     const M hb = (M)1 << ((meta >> 16) & 63u);
-                    while (rk) {
-                        const int sh = (__ffs(rk) - 1) & ~3;
-                        TACG_ASSERT(((rk >> sh) & 15u) >= 1u && (int)((rk >> sh) & 15u) <= nrep);
-                        const M pm = pick_slot((rk >> sh) & 15u, R | hb);
-                        rk &= ~(15u << sh);
-                        R |= pm;
-                        const int pick = sizeof(M) == 8 ? 63 - __clzll((long long)pm) : 31 - __clz((int)pm);
-                        TACG_ASSERT(pick >= 0 && pick < P);
-                        sred_inc(cl + (unsigned)pick * 128u);
-                        if (OUT && p.serve) p.serve[token_of(x, meta) * k + (sh >> 2)] = (signed char)pick;
+                    if constexpr (decltype(MULTI)::value) {
+                        while (rk) {
+                            const int sh = (__ffs(rk) - 1) & ~3;
+                            step(R, hb, rk, sh, meta, x);
+                            rk &= ~(15u << sh);
+                        }
+                    } else {
+                        step(R, hb, rk, (__ffs(rk) - 1) & ~3, meta, x);
                     }
                     const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~hb);
                     if (OUT && p.cost) p.cost[token_of(x, meta)] = (unsigned char)rem;
@@ -918,38 +933,58 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     sred_add(db + ((meta >> 13) & 7u) * 4u, (unsigned)max(0, nR - 1));
                     sred_add(db + 32u + ((meta >> 13) & 7u) * 4u, (unsigned)rem);
                 };
-#pragma unroll 1
-                for (int cls = 0; cls < 2; ++cls) {
-                    const unsigned pb = cls ? pb2 : pb1;               // shared address of the prefix sums
+                // one record class: flat index gi over the slices' records of that class -> entry of the record array.
+                // Within slice sl (flat indices [lo_sl, hi_sl)) the entry is xb + gi (first class, upwards from entry 0)
+                // or xb - gi (second class, downwards from the last entry); a thread's indices only grow, and a whole
+                // round of kRecFlight records usually stays inside one slice: one vote per round, no search.
+                auto run_class = [&](auto MULTI) {
+                    constexpr bool multi = decltype(MULTI)::value;
+                    const unsigned pb = multi ? pb2 : pb1;               // shared address of the prefix sums
                     const unsigned tot = slds_u32(pb + 4u * ns);
-                    // entry of flat index gi; the slice index only moves forward
                     unsigned sl = 0u, lo_sl = 0u, hi_sl = slds_u32(pb + 4u);
-                    auto locate = [&](unsigned gi) -> unsigned {
+                    unsigned xb = multi ? slice - 1u : 0u;
+                    auto advance = [&](unsigned gi) {
                         while (gi >= hi_sl) {
                             ++sl;
                             lo_sl = hi_sl;
                             hi_sl = slds_u32(pb + 4u * (sl + 1u));
                         }
-                        const unsigned within = gi - lo_sl;
-                        TACG_ASSERT(sl < (unsigned)ns && within < slice);
-                        return sl * slice + (cls ? slice - 1u - within : within);
+                        TACG_ASSERT(sl < (unsigned)ns && gi - lo_sl < slice);
+                        xb = multi ? sl * slice + slice - 1u + lo_sl : sl * slice - lo_sl;
                     };
-                    for (unsigned g0 = (unsigned)rank * kChainThreads + tid; g0 < tot; g0 += kRecFlight * stride) {
+                    const unsigned first = (unsigned)rank * kChainThreads + tid;
+                    // the trip count is the warp's (lane 0 has the smallest index): the vote below is by the whole warp
+                    for (unsigned g0 = first; g0 - lane < tot; g0 += kRecFlight * stride) {
                         // kRecFlight records per round, all their loads in flight before the first is used
                         unsigned x[kRecFlight];
                         Rec v[kRecFlight];
+                        const unsigned glast = min(g0 + (kRecFlight - 1u) * stride, tot - 1u);
+                        if (__any_sync(0xffffffffu, g0 < tot && glast >= hi_sl)) {
 #pragma unroll
-                        for (int q = 0; q < kRecFlight; ++q) {
-                            const unsigned gq = g0 + (unsigned)q * stride;
-                            x[q] = gq < tot ? locate(gq) : x[0];
+                            for (int q = 0; q < kRecFlight; ++q) {
+                                const unsigned gq = g0 + (unsigned)q * stride;
+                                x[q] = 0u;
+                                if (gq < tot) {
+                                    advance(gq);
+                                    x[q] = multi ? xb - gq : xb + gq;
+                                }
+                            }
+                        } else {
+#pragma unroll
+                            for (int q = 0; q < kRecFlight; ++q) {
+                                const unsigned gq = g0 + (unsigned)q * stride;
+                                x[q] = gq < tot ? (multi ? xb - gq : xb + gq) : 0u;
+                            }
                         }
 #pragma unroll
                         for (int q = 0; q < kRecFlight; ++q) v[q] = recs[x[q]];
 #pragma unroll
                         for (int q = 0; q < kRecFlight; ++q)
-                            if (g0 + (unsigned)q * stride < tot) resolve(rec_set<M>(v[q]), v[q].z, v[q].w, x[q]);
+                            if (g0 + (unsigned)q * stride < tot) resolve(MULTI, rec_set<M>(v[q]), v[q].z, v[q].w, x[q]);
                     }
-                }
+                };
+                run_class(std::false_type{});
+                run_class(std::true_type{});
                 // items left to this kernel: their tokens are served here, from the trace
                 for (int s = s0; s < s0 + ns; ++s) {
                     if (!ovf_s[s - s0]) continue;
