@@ -340,6 +340,13 @@ template <> __device__ __forceinline__ unsigned long long bit_or_zero<unsigned l
 
 // shared-memory accesses by 32-bit shared-space address (no generic-address arithmetic in the token loop)
 __device__ __forceinline__ unsigned saddr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+// The same address, opaque to the compiler: it stays in its register instead of being recomputed (special-register reads
+// and address arithmetic) at every use inside the hot loops.
+__device__ __forceinline__ unsigned saddr_kept(const void* p) {
+    unsigned a = saddr(p);
+    asm volatile("" : "+r"(a));
+    return a;
+}
 __device__ __forceinline__ void sred_inc(unsigned a) { asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(a) : "memory"); }
 __device__ __forceinline__ void sred_add(unsigned a, unsigned v) {
     asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
@@ -730,9 +737,9 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         rank = (int)(blockIdx.x % (unsigned)CS);
     }
     const int cluster_id = blockIdx.x / CS;
-    const unsigned cl = saddr(cnt + lane);
-    const unsigned db = saddr(dsum32);
-    const unsigned cmb = saddr(candm), pb1 = saddr(pre1), pb2 = saddr(pre2), nb1 = saddr(nrec1), nb2 = saddr(nrec2);
+    const unsigned cl = saddr_kept(cnt + lane);
+    const unsigned db = saddr_kept(dsum32);
+    const unsigned cmb = saddr_kept(candm), pb1 = saddr(pre1), pb2 = saddr(pre2), nb1 = saddr(nrec1), nb2 = saddr(nrec2);
     const int W = g.W;
     const int ncols = P + 3 * F;               // row words summed by threads 0..ncols-1
 
