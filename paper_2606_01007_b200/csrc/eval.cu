@@ -180,8 +180,15 @@ __device__ __forceinline__ unsigned long long load_guard_warp(const double* S, i
 
 // build_candidate for r <= 3 (at most four candidates) without a data-dependent loop: the position of a candidate in
 // the stable order is the number of kept candidates that are lighter, or as heavy and earlier in slot order.
-__device__ __forceinline__ void build_candidate_small(int e, int r, const LayerTables& T, unsigned long long feas,
-                                                      unsigned char* out) {
+// The loads are compared through order_key: integer compares instead of fp64 ones, the same order.
+__device__ __forceinline__ unsigned long long order_key(double x) {
+    // -0.0 + 0.0 = +0.0, so equal loads have equal keys; then the usual map of IEEE bits onto unsigned order
+    const long long b = __double_as_longlong(__dadd_rn(x, 0.0));
+    return (unsigned long long)b ^ ((unsigned long long)(b >> 63) | 0x8000000000000000ull);
+}
+
+__device__ __forceinline__ void build_candidate_small(int e, int r, const LayerTables& T, const unsigned long long* K,
+                                                      unsigned long long feas, unsigned char* out) {
     int c[4];
     bool ok[4];
     c[0] = (int)(T.ptab[e] & 63u);
@@ -197,11 +204,11 @@ __device__ __forceinline__ void build_candidate_small(int e, int r, const LayerT
     for (int i = 0; i < 4; ++i)
         if (ok[i]) cmask |= 1ull << c[i];
     const bool anyfeas = (cmask & feas) != 0ull;
-    double s[4];
+    unsigned long long s[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
         ok[i] = ok[i] && (!anyfeas || ((feas >> c[i]) & 1ull));
-        s[i] = T.S[c[i]];
+        s[i] = K[c[i]];
     }
     unsigned b[4] = {0u, 0u, 0u, 0u};      // partitions by position
     int m = 0;
@@ -708,6 +715,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     __shared__ unsigned char rank8[kPtab];
     __shared__ __align__(16) unsigned char candr[(kMaxRank + 1) * kCandStride];   // candidate tables by rank
     __shared__ double Ls[64];                  // EMA state of this layer
+    __shared__ unsigned long long Ks[64];      // order_key of Ls
     __shared__ unsigned long long ltot[64];    // cumulative integer load of this layer
     __shared__ unsigned long long csum[24];    // span | remote | tokens per family: rows of the scan kernel
     __shared__ unsigned long long dsum[16];    // span | remote of the deferred tokens handled by THIS CTA
@@ -749,6 +757,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         for (int i = tid; i < P * 32; i += kChainThreads) cnt[i] = 0u;
         if (tid < 64) {
             Ls[tid] = (p.load_state && tid < P) ? p.load_state[(size_t)layer * P + tid] : 0.0;
+            Ks[tid] = order_key(Ls[tid]);
             ltot[tid] = 0ull;
         }
         if (tid < 24) csum[tid] = 0ull;
@@ -816,7 +825,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         auto cand_of = [&](int i, unsigned long long feas) {
             const int e = (int)replist[i];
             unsigned char* out = T.cand + e * kCandStride;
-            if (r <= 3) build_candidate_small(e, r, T, feas, out);
+            if (r <= 3) build_candidate_small(e, r, T, Ks, feas, out);
             else build_candidate(e, r, T, feas, out);
             if (i < kMaxRank) {
                 // by rank: the one-hot masks of the first four candidates (entries beyond the count repeat the first)
@@ -1049,7 +1058,9 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 } else {
                     for (int q = 0; q < CS; ++q) d += exch[par][q][tid];
                 }
-                Ls[tid] = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
+                const double ln = __dadd_rn(__dmul_rn(p.rho, Ls[tid]), (double)d);   // no FMA (Q19)
+                Ls[tid] = ln;
+                Ks[tid] = order_key(ln);
                 ltot[tid] += d;
             } else if (tid < ncols) {
                 csum[tid - P] += mine_s[tid];
