@@ -187,8 +187,10 @@ __device__ __forceinline__ unsigned long long order_key(double x) {
     return (unsigned long long)b ^ ((unsigned long long)(b >> 63) | 0x8000000000000000ull);
 }
 
+// The table entry is returned in two words: w0 = count | c1 << 8 | c2 << 16 | c3 << 24 (entries beyond the count repeat
+// c1), w1 = c4.
 __device__ __forceinline__ void build_candidate_small(int e, int r, const LayerTables& T, const unsigned long long* K,
-                                                      unsigned long long feas, unsigned char* out) {
+                                                      unsigned long long feas, unsigned& w0, unsigned& w1) {
     int c[4];
     bool ok[4];
     c[0] = (int)(T.ptab[e] & 63u);
@@ -227,9 +229,9 @@ __device__ __forceinline__ void build_candidate_small(int e, int r, const LayerT
     }
     if (m < 2) b[1] = b[0];
     if (m < 3) b[2] = b[0];
-    unsigned* o = reinterpret_cast<unsigned*>(out);     // entries are 4-byte aligned (kCandStride = 12)
-    o[0] = (unsigned)m | (b[0] << 8) | (b[1] << 16) | (b[2] << 24);
-    o[1] = b[3];
+    if (m < 4) b[3] = b[0];
+    w0 = (unsigned)m | (b[0] << 8) | (b[1] << 16) | (b[2] << 24);
+    w1 = b[3];
 }
 
 __device__ __forceinline__ void build_candidates(int E, int r, const LayerTables& T, unsigned long long feas) {
@@ -825,8 +827,25 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         auto cand_of = [&](int i, unsigned long long feas) {
             const int e = (int)replist[i];
             unsigned char* out = T.cand + e * kCandStride;
-            if (r <= 3) build_candidate_small(e, r, T, Ks, feas, out);
-            else build_candidate(e, r, T, feas, out);
+            if (r <= 3) {
+                // at most four candidates: everything stays in registers between the order and the tables
+                unsigned w0, w1;
+                build_candidate_small(e, r, T, Ks, feas, w0, w1);
+                unsigned* o = reinterpret_cast<unsigned*>(out);     // entries are 4-byte aligned (kCandStride = 12)
+                o[0] = w0;
+                o[1] = w1;
+                if (i < kMaxRank) {
+                    M* cm = reinterpret_cast<M*>(candm) + (i + 1) * 4;
+                    cm[0] = (M)1 << ((w0 >> 8) & 0xffu);
+                    cm[1] = (M)1 << ((w0 >> 16) & 0xffu);
+                    cm[2] = (M)1 << (w0 >> 24);
+                    cm[3] = (M)1 << (w1 & 0xffu);
+                    unsigned* dst = reinterpret_cast<unsigned*>(candr + (i + 1) * kCandStride);
+                    dst[0] = w0; dst[1] = w1; dst[2] = 0u;
+                }
+                return;
+            }
+            build_candidate(e, r, T, feas, out);
             if (i < kMaxRank) {
                 // by rank: the one-hot masks of the first four candidates (entries beyond the count repeat the first)
                 const int n = out[0];
