@@ -712,6 +712,9 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     T.cand = csm + off;                                    off += ((size_t)E * kCandStride + 15) & ~(size_t)15;
     T.rep = reinterpret_cast<signed char*>(csm + off);     off += ((size_t)E * r + 15) & ~(size_t)15;
     unsigned* cnt = reinterpret_cast<unsigned*>(csm + off);   off += sizeof(unsigned) * (size_t)P * 32;
+    // [warps][8][32] lane-private family words (span | remote << 16), not in grid mode (see finish below)
+    unsigned* accb = reinterpret_cast<unsigned*>(csm + off);
+    if (MODE != kModeGrid) off += sizeof(unsigned) * (kChainThreads / 32) * 8 * 32;
     unsigned short* replist = reinterpret_cast<unsigned short*>(csm + off);   // [E] ids of the replicated experts
     __shared__ unsigned char ptab_s[kPtab];
     __shared__ unsigned char rank8[kPtab];
@@ -749,6 +752,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     const int cluster_id = blockIdx.x / CS;
     const unsigned cl = saddr_kept(cnt + lane);
     const unsigned db = saddr_kept(dsum32);
+    unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;
+    const unsigned al = saddr_kept(acc);
     const unsigned cmb = saddr_kept(candm), pb1 = saddr(pre1), pb2 = saddr(pre2), nb1 = saddr(nrec1), nb2 = saddr(nrec2);
     const int W = g.W;
     const int ncols = P + 3 * F;               // row words summed by threads 0..ncols-1
@@ -764,6 +769,10 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         }
         if (tid < 24) csum[tid] = 0ull;
         if (tid < 16) { dsum[tid] = 0ull; dsum32[tid] = 0u; }
+        if constexpr (MODE != kModeGrid) {
+#pragma unroll
+            for (int f = 0; f < 8; ++f) acc[f * 32] = 0u;
+        }
         __syncthreads();
         const int nrep = build_ranks(E, T.ptab, rank8, replist, wsum);
         unsigned* gsl = MODE == kModeGrid ? p.gsync + (size_t)layer * kSyncWords : nullptr;
@@ -773,6 +782,36 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         const unsigned* rows_l = p.rows + (size_t)layer * g.ipl * W;
         const size_t rec_l = (size_t)layer * g.ipl * g.slice;
 
+        // Per-family communication sums of a record.  Many records per thread and micro-batch (cluster, single CTA): one
+        // conflict-free atomic into the thread's own word, span | remote << 16, folded once per round of slices
+        // (flush_acc; 16-bit fields: a thread takes at most 32 * 8192 / 512 records of <= 16 each per round).  Few
+        // records per thread (grid mode): two atomics straight into the CTA's words -- ATOMS.ADD does not merge lanes
+        // that hit one word, so this costs several wavefronts per instruction, but there is no fold to pay for.
+        auto add_comm = [&](unsigned fam, unsigned span, unsigned rem) {
+            if constexpr (MODE == kModeGrid) {
+                sred_add(db + fam * 4u, span);
+                sred_add(db + 32u + fam * 4u, rem);
+            } else {
+                sred_add(al + fam * 128u, span | (rem << 16));
+            }
+        };
+        auto flush_acc = [&]() {
+            if constexpr (MODE != kModeGrid) {
+#pragma unroll
+                for (int fq = 0; fq < 8; ++fq) {
+                    if (fq < F) {
+                        const unsigned av = acc[fq * 32];
+                        acc[fq * 32] = 0u;
+                        const unsigned sp = __reduce_add_sync(0xffffffffu, av & 0xffffu);
+                        const unsigned rq = __reduce_add_sync(0xffffffffu, av >> 16);
+                        if (lane == 0) {
+                            if (sp) atomicAdd(&dsum32[fq], sp);
+                            if (rq) atomicAdd(&dsum32[8 + fq], rq);
+                        }
+                    }
+                }
+            }
+        };
         // a round of at most 32 slices adds less than 2^23 to a 32-bit sum; one thread per entry widens it between barriers
         auto fold_dsum = [&](int i) {
             dsum[i] += dsum32[i];
@@ -964,9 +1003,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     }
                     const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~hb);
                     if (OUT && p.cost) p.cost[token_of(x, meta)] = (unsigned char)rem;
-                    // per-family sums of the CTA: lanes of one family hit one word, which the atomic unit merges
-                    sred_add(db + ((meta >> 13) & 7u) * 4u, (unsigned)max(0, nR - 1));
-                    sred_add(db + 32u + ((meta >> 13) & 7u) * 4u, (unsigned)rem);
+                    add_comm((meta >> 13) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
                 };
                 // one record class: flat index gi over the slices' records of that class -> entry of the record array.
                 // Within slice sl (flat indices [lo_sl, hi_sl)) the entry is xb + gi (first class, upwards from entry 0)
@@ -1043,10 +1080,10 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                         if (OUT && p.cost) p.cost[(size_t)layer * g.N + t0 + o] = (unsigned char)rem;
                         if (OUT && p.serve)
                             for (int j = 0; j < k; ++j) p.serve[((size_t)layer * g.N + t0 + o) * k + j] = (signed char)sv[j];
-                        sred_add(db + (unsigned)fq * 4u, (unsigned)max(0, nR - 1));
-                        sred_add(db + 32u + (unsigned)fq * 4u, (unsigned)rem);
+                        add_comm((unsigned)fq, (unsigned)max(0, nR - 1), (unsigned)rem);
                     }
                 }
+                flush_acc();
             }
             // step 5: integer dispatch counts of the micro-batch, then Eq. 15
             __syncthreads();
@@ -1421,6 +1458,7 @@ int launch_chain(EvalCall& c) {
     const EvalGeom& g = c.cp.g;
     const size_t smem = (((size_t)g.E * kCandStride + 15) & ~(size_t)15) +
                         (((size_t)g.E * g.r + 15) & ~(size_t)15) + sizeof(unsigned) * (size_t)g.P * 32 +
+                        (c.mode != kModeGrid ? sizeof(unsigned) * (kChainThreads / 32) * 8 * 32 : 0) +
                         sizeof(unsigned short) * (size_t)g.E + 16;
     const int cs = c.cs;
     c.cp.groups = c.groups;
