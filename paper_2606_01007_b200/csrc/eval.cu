@@ -24,8 +24,12 @@
 //   fairness_kernel    S12; without replicas it first adds the rows of a layer (nothing depends on
 //                      the snapshot then, the whole trace is one micro-batch).
 //
-// No CTA ever spins on another launch-mate: the only waits are cluster barriers, and a cluster is
-// co-scheduled by the hardware.
+// The only waits between CTAs are cluster barriers (a cluster is co-scheduled by the hardware) and, when one
+// layer gets more CTAs than a cluster holds (few layers, long micro-batches: kModeGrid), a per-layer arrival
+// counter inside a COOPERATIVE launch, where every CTA is resident by construction.
+//
+// tacg_eval_primary_noalloc (end of the file) runs the no-replica evaluation with the item rows in a fixed
+// __device__ array instead of the context's scratch: an entry point that allocates nothing.
 //
 // The pick rule of Q17 orders candidates by (not local, snapshot load, candidate slot).  Only the
 // first key depends on the token, so once per micro-batch each replicated expert's feasible
