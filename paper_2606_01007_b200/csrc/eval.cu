@@ -56,7 +56,8 @@ constexpr int kEvalThreads = 512;    // eval_scan_kernel, select_kernel
 constexpr int kEvalBatch = 4;        // tokens per thread with their loads in flight together
 constexpr int kSlice = 8192;         // most tokens of a scan item (13-bit offsets in the records, 16 per thread)
 constexpr int kChainThreads = 512;    // two CTAs per SM, so that clusters of 4 at L = 58 still use every SM
-constexpr unsigned kRecFlight = 4;    // records a chain thread loads before it resolves the first
+constexpr unsigned kRecFlight = 4;    // records a chain thread loads before it resolves the first (cluster, single CTA)
+constexpr unsigned kRecFlightGrid = 1; // the same in grid mode, where a thread has one or two records per micro-batch
 constexpr long long kSeqBelow = 1024; // micro-batches shorter than this go to the one-warp-per-layer kernel
 constexpr int kCandStride = 12;      // bytes per expert in the candidate table: [0] = count, [1..9] = partitions
 constexpr unsigned kRepFlag = 0x80u; // ptab bit: the expert has at least one replica
@@ -1012,8 +1013,9 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 // one record class: flat index gi over the slices' records of that class -> entry of the record array.
                 // Within slice sl (flat indices [lo_sl, hi_sl)) the entry is xb + gi (first class, upwards from entry 0)
                 // or xb - gi (second class, downwards from the last entry); a thread's indices only grow, and a whole
-                // round of kRecFlight records usually stays inside one slice: one vote per round, no search.
+                // round of RF records usually stays inside one slice: one vote per round, no search.
                 auto run_class = [&](auto MULTI) {
+                    constexpr unsigned RF = MODE == kModeGrid ? kRecFlightGrid : kRecFlight;
                     constexpr bool multi = decltype(MULTI)::value;
                     const unsigned pb = multi ? pb2 : pb1;               // shared address of the prefix sums
                     const unsigned tot = slds_u32(pb + 4u * ns);
@@ -1030,14 +1032,14 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     };
                     const unsigned first = (unsigned)rank * kChainThreads + tid;
                     // the trip count is the warp's (lane 0 has the smallest index): the vote below is by the whole warp
-                    for (unsigned g0 = first; g0 - lane < tot; g0 += kRecFlight * stride) {
-                        // kRecFlight records per round, all their loads in flight before the first is used
-                        unsigned x[kRecFlight];
-                        Rec v[kRecFlight];
-                        const unsigned glast = min(g0 + (kRecFlight - 1u) * stride, tot - 1u);
+                    for (unsigned g0 = first; g0 - lane < tot; g0 += RF * stride) {
+                        // RF records per round, all their loads in flight before the first is used
+                        unsigned x[RF];
+                        Rec v[RF];
+                        const unsigned glast = min(g0 + (RF - 1u) * stride, tot - 1u);
                         if (__any_sync(0xffffffffu, g0 < tot && glast >= hi_sl)) {
 #pragma unroll
-                            for (int q = 0; q < kRecFlight; ++q) {
+                            for (int q = 0; q < RF; ++q) {
                                 const unsigned gq = g0 + (unsigned)q * stride;
                                 x[q] = 0u;
                                 if (gq < tot) {
@@ -1047,15 +1049,15 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                             }
                         } else {
 #pragma unroll
-                            for (int q = 0; q < kRecFlight; ++q) {
+                            for (int q = 0; q < RF; ++q) {
                                 const unsigned gq = g0 + (unsigned)q * stride;
                                 x[q] = gq < tot ? (multi ? xb - gq : xb + gq) : 0u;
                             }
                         }
 #pragma unroll
-                        for (int q = 0; q < kRecFlight; ++q) v[q] = recs[x[q]];
+                        for (int q = 0; q < RF; ++q) v[q] = recs[x[q]];
 #pragma unroll
-                        for (int q = 0; q < kRecFlight; ++q)
+                        for (int q = 0; q < RF; ++q)
                             if (g0 + (unsigned)q * stride < tot) resolve(MULTI, rec_set<M>(v[q]), v[q].z, v[q].w, x[q]);
                     }
                 };
