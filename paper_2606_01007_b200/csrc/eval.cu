@@ -740,7 +740,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     __shared__ unsigned bigq_s;                                 // ranks that list more than four candidates
     __shared__ unsigned pre1[33], pre2[33];                     // records of up to 32 slices, prefix sums
     __shared__ unsigned nrec1[32], nrec2[32];                   // records per slice (one pending slot | several)
-    __shared__ unsigned ovf_s[32];
+    __shared__ unsigned ovf_s;                                  // bit s: slice s of the round is left to this kernel
     T.ptab = ptab_s;
     T.S = Ls;                                  // the snapshot of a micro-batch IS the EMA state at its start
 
@@ -826,7 +826,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         auto put_counts = [&](unsigned n1, unsigned n2, int ln) {
             const bool ovf = n1 == kOverflow;
             if (ovf) { n1 = 0u; n2 = 0u; }
-            ovf_s[ln] = ovf ? 1u : 0u;
+            const unsigned om = __ballot_sync(0xffffffffu, ovf);
+            if (ln == 0) ovf_s = om;
             nrec1[ln] = n1;
             nrec2[ln] = n2;
             unsigned a1 = n1, a2 = n2;
@@ -1064,8 +1065,8 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 run_class(std::false_type{});
                 run_class(std::true_type{});
                 // items left to this kernel: their tokens are served here, from the trace
-                for (int s = s0; s < s0 + ns; ++s) {
-                    if (!ovf_s[s - s0]) continue;
+                for (unsigned om = ovf_s; om; om &= om - 1u) {
+                    const int s = s0 + __ffs(om) - 1;
                     long long t0, t1;
                     item_tokens(g, mb, s, t0, t1);
                     const unsigned hb0 = (unsigned)((g.token_offset + t0) % P);
