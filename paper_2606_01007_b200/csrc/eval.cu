@@ -678,12 +678,22 @@ constexpr int kModeSingle = 0;    // one CTA per layer: nothing to exchange
 constexpr int kModeCluster = 1;   // one thread-block cluster per layer: distributed shared memory + the cluster barrier
 constexpr int kModeGrid = 2;      // few layers: more CTAs per layer than a cluster holds, launched cooperatively (all
                                   // resident); counts through global atomics, one arrival counter per layer
-// per-layer words of ChainParams::gsync: counts[2][64] (cumulative, by micro-batch parity) | sums u64[16] | arrivals
-constexpr int kSyncSums = 128, kSyncBar = 160, kSyncWords = 192;
+// per-layer words of ChainParams::gsync: one 64-bit word per (micro-batch parity, partition), each on its own 128-byte
+// line: arrivals << 48 | cumulative dispatch count.  A CTA adds (1 << 48) | its count with ONE atomic; the thread that
+// owns partition m polls that word until the arrivals reach gper * (rounds of this parity): count and flag are one word,
+// so there is no fence, no separate arrival counter and no read-back.  Then sums u64[16] | arrivals of the layer's
+// last barrier (layer_barrier).
+constexpr int kSyncSums = 4096, kSyncBar = 4160, kSyncWords = 4224;
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* ptr) {
     unsigned v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ptr) : "memory");
+    return v;
+}
+
+__device__ __forceinline__ unsigned long long ld_relaxed_u64(const unsigned long long* ptr) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ptr) : "memory");
     return v;
 }
 
@@ -781,7 +791,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
         __syncthreads();
         const int nrep = build_ranks(E, T.ptab, rank8, replist, wsum);
         unsigned* gsl = MODE == kModeGrid ? p.gsync + (size_t)layer * kSyncWords : nullptr;
-        unsigned gprev[2] = {0u, 0u};       // kModeGrid: the cumulative counts this thread read last, by parity
+        unsigned long long gprev[2] = {0ull, 0ull};       // kModeGrid: the cumulative counts this thread read last, by parity
         unsigned nbar = 0u;                 // kModeGrid: barriers of this layer passed so far
         const int16_t* base = p.indices + (size_t)layer * (size_t)g.N * (size_t)k;
         const unsigned* rows_l = p.rows + (size_t)layer * g.ipl * W;
@@ -1104,18 +1114,25 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 } else if constexpr (MODE == kModeGrid) {
                     // cumulative per parity: nobody adds to this parity again before every CTA has passed the NEXT
                     // barrier, that is, after every CTA has read it
-                    if (lane == 0 && sm) atomicAdd(gsl + par * 64 + m, sm);
+                    if (lane == 0)
+                        atomicAdd(reinterpret_cast<unsigned long long*>(gsl + (par * 64 + m) * 32), (1ull << 48) | sm);
                 } else {
                     if (lane == 0) exch[par][0][m] = sm;
                 }
             }
             if constexpr (MODE == kModeCluster) cg::this_cluster().sync();
-            else if constexpr (MODE == kModeGrid) layer_barrier(gsl + kSyncBar, (unsigned)CS * ++nbar);
-            else __syncthreads();
+            else if constexpr (MODE != kModeGrid) __syncthreads();
             if (tid < P) {
                 unsigned long long d = mine_s[tid];
                 if constexpr (MODE == kModeGrid) {
-                    const unsigned now = __ldcg(gsl + par * 64 + tid);
+                    // wait for the gper additions of this micro-batch to this partition's word
+                    const unsigned long long* src = reinterpret_cast<const unsigned long long*>(gsl + (par * 64 + tid) * 32);
+                    const unsigned want = ((unsigned)CS * (unsigned)((mb >> 1) + 1)) & 0xffffu;
+                    unsigned long long now;
+                    const long long t0 = clock64();
+                    while ((short)((unsigned)((now = ld_relaxed_u64(src)) >> 48) - want) < 0)
+                        if (clock64() - t0 > (1ll << 33)) __trap();          // a bug, not a slow peer: do not hang the GPU
+                    now &= (1ull << 48) - 1ull;
                     d += now - gprev[par];
                     gprev[par] = now;
                 } else {
