@@ -1025,7 +1025,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 // Within slice sl (flat indices [lo_sl, hi_sl)) the entry is xb + gi (first class, upwards from entry 0)
                 // or xb - gi (second class, downwards from the last entry); a thread's indices only grow, and a whole
                 // round of RF records usually stays inside one slice: one vote per round, no search.
-                auto run_class = [&](auto MULTI) {
+                auto run_class = [&](auto MULTI, unsigned skip) {
                     constexpr unsigned RF = MODE == kModeGrid ? kRecFlightGrid : kRecFlight;
                     constexpr bool multi = decltype(MULTI)::value;
                     const unsigned pb = multi ? pb2 : pb1;               // shared address of the prefix sums
@@ -1043,7 +1043,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     };
                     const unsigned first = (unsigned)rank * kChainThreads + tid;
                     // the trip count is the warp's (lane 0 has the smallest index): the vote below is by the whole warp
-                    for (unsigned g0 = first; g0 - lane < tot; g0 += RF * stride) {
+                    for (unsigned g0 = first + skip * stride; g0 - lane < tot; g0 += RF * stride) {
                         // RF records per round, all their loads in flight before the first is used
                         unsigned x[RF];
                         Rec v[RF];
@@ -1072,8 +1072,33 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                             if (g0 + (unsigned)q * stride < tot) resolve(MULTI, rec_set<M>(v[q]), v[q].z, v[q].w, x[q]);
                     }
                 };
-                run_class(std::false_type{});
-                run_class(std::true_type{});
+                if constexpr (MODE == kModeGrid) {
+                    // A thread has one record per class and micro-batch here, and the time of a micro-batch is a chain of
+                    // latencies: the first record of BOTH classes is located and loaded before either is resolved (one
+                    // L2 round trip instead of two); what is left, if anything, goes through the general loops.
+                    const unsigned first = (unsigned)rank * kChainThreads + tid;
+                    auto locate0 = [&](unsigned pb, bool multi, unsigned gi) -> unsigned {
+                        unsigned sl = 0u, lo_sl = 0u, hi_sl = slds_u32(pb + 4u);
+                        while (gi >= hi_sl) {
+                            ++sl;
+                            lo_sl = hi_sl;
+                            hi_sl = slds_u32(pb + 4u * (sl + 1u));
+                        }
+                        TACG_ASSERT(sl < (unsigned)ns && gi - lo_sl < slice);
+                        return multi ? sl * slice + slice - 1u - (gi - lo_sl) : sl * slice + (gi - lo_sl);
+                    };
+                    const bool has1 = first < slds_u32(pb1 + 4u * ns), has2 = first < slds_u32(pb2 + 4u * ns);
+                    const unsigned x1 = has1 ? locate0(pb1, false, first) : 0u;
+                    const unsigned x2 = has2 ? locate0(pb2, true, first) : 0u;
+                    const Rec v1 = recs[x1], v2 = recs[x2];
+                    if (has1) resolve(std::false_type{}, rec_set<M>(v1), v1.z, v1.w, x1);
+                    if (has2) resolve(std::true_type{}, rec_set<M>(v2), v2.z, v2.w, x2);
+                    run_class(std::false_type{}, 1u);
+                    run_class(std::true_type{}, 1u);
+                } else {
+                    run_class(std::false_type{}, 0u);
+                    run_class(std::true_type{}, 0u);
+                }
                 // items left to this kernel: their tokens are served here, from the trace
                 for (unsigned om = ovf_s; om; om &= om - 1u) {
                     const int s = s0 + __ffs(om) - 1;
