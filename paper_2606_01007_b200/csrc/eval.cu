@@ -717,7 +717,7 @@ __device__ __forceinline__ void layer_barrier(unsigned* bar, unsigned target) {
 // item's records; the integer dispatch counts of a micro-batch are exchanged through distributed shared
 // memory (two alternating buffers, one cluster barrier per micro-batch).
 template <typename M, bool OUT, int MODE>
-__global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const ChainParams p) {
+__global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval_chain_kernel(const ChainParams p) {
     tacg_pdl_prologue();
     extern __shared__ __align__(16) unsigned char csm[];
     const EvalGeom& g = p.g;
@@ -748,9 +748,10 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     __shared__ unsigned long long mine_s[64 + 24];   // the scan kernel's sums of the current micro-batch (row words)
     __shared__ __align__(16) unsigned long long candm[(kMaxRank + 1) * 4];   // by rank: one-hot masks (type M) of the first four candidates
     __shared__ unsigned bigq_s;                                 // ranks that list more than four candidates
-    __shared__ unsigned pre1[33], pre2[33];                     // records of up to 32 slices, prefix sums
-    __shared__ unsigned nrec1[32], nrec2[32];                   // records per slice (one pending slot | several)
-    __shared__ unsigned ovf_s;                                  // bit s: slice s of the round is left to this kernel
+    // record counts of up to 32 slices as prefix sums (one pending slot | several), and bit s = slice s of the round is
+    // left to this kernel; two copies by micro-batch parity: the next micro-batch's are published during the current one
+    __shared__ unsigned pre1[2][36], pre2[2][36];
+    __shared__ unsigned ovf_s[2];
     T.ptab = ptab_s;
     T.S = Ls;                                  // the snapshot of a micro-batch IS the EMA state at its start
 
@@ -769,7 +770,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
     const unsigned db = saddr_kept(dsum32);
     unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;
     const unsigned al = saddr_kept(acc);
-    const unsigned cmb = saddr_kept(candm), pb1 = saddr(pre1), pb2 = saddr(pre2), nb1 = saddr(nrec1), nb2 = saddr(nrec2);
+    const unsigned cmb = saddr_kept(candm), pbase1 = saddr(pre1), pbase2 = saddr(pre2);
     const int W = g.W;
     const int ncols = P + 3 * F;               // row words summed by threads 0..ncols-1
 
@@ -833,30 +834,28 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             dsum32[i] = 0u;
         };
         // record counts of up to 32 slices (one pending slot | several) and their prefix sums; one warp
-        auto put_counts = [&](unsigned n1, unsigned n2, int ln) {
+        auto put_counts = [&](unsigned n1, unsigned n2, int ln, int buf) {
             const bool ovf = n1 == kOverflow;
             if (ovf) { n1 = 0u; n2 = 0u; }
             const unsigned om = __ballot_sync(0xffffffffu, ovf);
-            if (ln == 0) ovf_s = om;
-            nrec1[ln] = n1;
-            nrec2[ln] = n2;
+            if (ln == 0) ovf_s[buf] = om;
             unsigned a1 = n1, a2 = n2;
 #pragma unroll
             for (int d = 1; d < 32; d <<= 1) {
                 const unsigned v1 = __shfl_up_sync(0xffffffffu, a1, d), v2 = __shfl_up_sync(0xffffffffu, a2, d);
                 if (ln >= d) { a1 += v1; a2 += v2; }
             }
-            pre1[ln + 1] = a1;
-            pre2[ln + 1] = a2;
-            if (ln == 0) { pre1[0] = 0u; pre2[0] = 0u; }
+            pre1[buf][ln + 1] = a1;
+            pre2[buf][ln + 1] = a2;
+            if (ln == 0) { pre1[buf][0] = 0u; pre2[buf][0] = 0u; }
         };
-        auto load_counts = [&](const unsigned* rows_mb, int s0, int ns, int ln) {
+        auto load_counts = [&](const unsigned* rows_mb, int s0, int ns, int ln, int buf) {
             unsigned n1 = 0u, n2 = 0u;
             if (ln < ns) {
                 n1 = rows_mb[(size_t)(s0 + ln) * W + ncols];
                 n2 = rows_mb[(size_t)(s0 + ln) * W + ncols + 1];
             }
-            put_counts(n1, n2, ln);
+            put_counts(n1, n2, ln, buf);
         };
         // The second warp keeps the record counts of the first 32 slices of this micro-batch and the next in registers
         // (A, B) and has those of the one after in flight (C): nothing the chain waits for is a miss.
@@ -918,9 +917,43 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
             if (lane == 0) prefetch_rows(0, 3);
             fetch_counts(0, cA1, cA2);
             fetch_counts(1, cB1, cB2);
+            put_counts(cA1, cA2, lane, 0);
         }
+        __syncthreads();
         for (long long mb = 0; mb < g.nmb; ++mb) {
             const unsigned* rows_mb = rows_l + (size_t)mb * g.spm * W;
+            const int cur = (int)(mb & 1);                      // this micro-batch's copy of the record counts
+            const unsigned pb1 = pbase1 + (unsigned)cur * 36u * 4u, pb2 = pbase2 + (unsigned)cur * 36u * 4u;
+            // Grid mode: a thread has about one record per class and micro-batch, and the time of a micro-batch is a chain
+            // of latencies.  The records do not depend on the snapshot: the first one of BOTH classes is located and its
+            // load issued here, before the guard, so that the data is there when the candidate tables are.
+            const unsigned first = (unsigned)rank * kChainThreads + tid;
+            bool has1 = false, has2 = false;
+            unsigned x1 = 0u, x2 = 0u;
+            Rec v1 = {0u, 0u, 0u, 0u}, v2 = {0u, 0u, 0u, 0u};
+            const unsigned slice0 = (unsigned)g.slice;
+            auto locate0 = [&](unsigned pb, bool multi, unsigned gi) -> unsigned {
+                unsigned sl = 0u, lo_sl = 0u, hi_sl = slds_u32(pb + 4u);
+                while (gi >= hi_sl) {
+                    ++sl;
+                    lo_sl = hi_sl;
+                    hi_sl = slds_u32(pb + 4u * (sl + 1u));
+                }
+                TACG_ASSERT(sl < (unsigned)ns0 && gi - lo_sl < slice0);
+                return multi ? sl * slice0 + slice0 - 1u - (gi - lo_sl) : sl * slice0 + (gi - lo_sl);
+            };
+            auto early = [&]() {
+                has1 = first < slds_u32(pb1 + 4u * ns0);
+                has2 = first < slds_u32(pb2 + 4u * ns0);
+                x1 = has1 ? locate0(pb1, false, first) : 0u;
+                x2 = has2 ? locate0(pb2, true, first) : 0u;
+                const Rec* recs0 = p.rec + rec_l + (size_t)mb * g.spm * (size_t)g.slice;
+                v1 = recs0[x1];
+                v2 = recs0[x2];
+            };
+            if constexpr (MODE == kModeGrid) {
+                if (tid >= 32) early();       // the first warp has the guard to do first: its records follow the tables
+            }
             // steps 1-2 by the first warp: guard of the snapshot (the EMA state: it only changes at the end of a
             // micro-batch).  The second warp meanwhile publishes this micro-batch's record counts.
             unsigned cC1 = 0u, cC2 = 0u;
@@ -929,10 +962,11 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 if (lane == 0) { feas_s = fm; bigq_s = 0u; }
                 __syncwarp();
                 if (lane < nrep && nrep <= 32) cand_of(lane, fm);       // step 3: the usual case, no second barrier
+                if constexpr (MODE == kModeGrid) early();
             } else if (tid < 64) {
                 fetch_counts(mb + 2, cC1, cC2);
                 if (lane == 0) prefetch_rows(mb + 3, mb + 4);
-                put_counts(cA1, cA2, lane);
+                put_counts(cB1, cB2, lane, cur ^ 1);      // the next micro-batch's counts: read after the barrier at its end
                 // The records of the NEXT micro-batch do not depend on the chain: one bulk prefetch per slice and record
                 // class pulls them into L2 now (a single instruction each, issued by one lane of one CTA per slice).
                 if (mb + 1 < g.nmb && lane < ns0 && lane % CS == rank && cB1 != kOverflow) {
@@ -980,7 +1014,7 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                 const int ns = min(32, g.spm - s0);
                 if (s0 > 0) {
                     __syncthreads();
-                    if (tid < 32) load_counts(rows_mb, s0, ns, tid);
+                    if (tid < 32) load_counts(rows_mb, s0, ns, tid, cur);
                     else if (tid >= 96 && tid < 112) fold_dsum(tid - 96);
                     __syncthreads();
                 }
@@ -1073,34 +1107,19 @@ __global__ void __launch_bounds__(kChainThreads, 2) eval_chain_kernel(const Chai
                     }
                 };
                 if constexpr (MODE == kModeGrid) {
-                    // A thread has one record per class and micro-batch here, and the time of a micro-batch is a chain of
-                    // latencies: the first record of BOTH classes is located and loaded before either is resolved (one
-                    // L2 round trip instead of two); what is left, if anything, goes through the general loops.
-                    const unsigned first = (unsigned)rank * kChainThreads + tid;
-                    auto locate0 = [&](unsigned pb, bool multi, unsigned gi) -> unsigned {
-                        unsigned sl = 0u, lo_sl = 0u, hi_sl = slds_u32(pb + 4u);
-                        while (gi >= hi_sl) {
-                            ++sl;
-                            lo_sl = hi_sl;
-                            hi_sl = slds_u32(pb + 4u * (sl + 1u));
-                        }
-                        TACG_ASSERT(sl < (unsigned)ns && gi - lo_sl < slice);
-                        return multi ? sl * slice + slice - 1u - (gi - lo_sl) : sl * slice + (gi - lo_sl);
-                    };
-                    const bool has1 = first < slds_u32(pb1 + 4u * ns), has2 = first < slds_u32(pb2 + 4u * ns);
-                    const unsigned x1 = has1 ? locate0(pb1, false, first) : 0u;
-                    const unsigned x2 = has2 ? locate0(pb2, true, first) : 0u;
-                    const Rec v1 = recs[x1], v2 = recs[x2];
-                    if (has1) resolve(std::false_type{}, rec_set<M>(v1), v1.z, v1.w, x1);
-                    if (has2) resolve(std::true_type{}, rec_set<M>(v2), v2.z, v2.w, x2);
-                    run_class(std::false_type{}, 1u);
-                    run_class(std::true_type{}, 1u);
+                    if (s0 == 0) {
+                        // the two records loaded before the guard; what is left, if anything, goes through the loops
+                        if (has1) resolve(std::false_type{}, rec_set<M>(v1), v1.z, v1.w, x1);
+                        if (has2) resolve(std::true_type{}, rec_set<M>(v2), v2.z, v2.w, x2);
+                    }
+                    run_class(std::false_type{}, s0 == 0 ? 1u : 0u);
+                    run_class(std::true_type{}, s0 == 0 ? 1u : 0u);
                 } else {
                     run_class(std::false_type{}, 0u);
                     run_class(std::true_type{}, 0u);
                 }
                 // items left to this kernel: their tokens are served here, from the trace
-                for (unsigned om = ovf_s; om; om &= om - 1u) {
+                for (unsigned om = ovf_s[cur]; om; om &= om - 1u) {
                     const int s = s0 + __ffs(om) - 1;
                     long long t0, t1;
                     item_tokens(g, mb, s, t0, t1);
