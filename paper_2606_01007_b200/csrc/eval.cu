@@ -176,7 +176,9 @@ __device__ __forceinline__ unsigned long long load_guard_warp(const double* S, i
         for (int i = 0; i < 8; ++i)
             if (m0 + i < P) tot = __dadd_rn(tot, v[i]);
     }
-    const double Lbar = tot / (double)P;
+    // P a power of two: tot * 2^-k is the same real number as tot / 2^k, so the rounded result is the same bits, without
+    // the division's long dependent sequence
+    const double Lbar = (P & (P - 1)) == 0 ? __dmul_rn(tot, 1.0 / (double)P) : tot / (double)P;
     const double thr = __dmul_rn(__dadd_rn(1.0, (double)theta), Lbar);
     unsigned long long fm = __ballot_sync(0xffffffffu, lane < P && S[lane] <= thr);
     if (P > 32) fm |= (unsigned long long)__ballot_sync(0xffffffffu, lane + 32 < P && S[lane + 32] <= thr) << 32;
@@ -237,6 +239,66 @@ __device__ __forceinline__ void build_candidate_small(int e, int r, const LayerT
     if (m < 4) b[3] = b[0];
     w0 = (unsigned)m | (b[0] << 8) | (b[1] << 16) | (b[2] << 24);
     w1 = b[3];
+}
+
+// The same in three steps for the chain kernel, where one lane owns one replicated expert for a whole layer:
+//   cand_fixed   once per layer: the candidates (one byte each, primary first), which of them exist, their partition set
+//   cand_order   per micro-batch, BEFORE the guard is known (it only needs the loads): bit 4*i + j = candidate j sorts
+//                before candidate i (lighter, or as heavy and earlier in slot order)
+//   cand_tables  per micro-batch, after the guard: drop the infeasible ones (unless none is feasible), positions by
+//                counting, table words as build_candidate_small returns them
+struct CandFixed {
+    unsigned cpk, okm;
+    unsigned long long cmask;
+};
+__device__ __forceinline__ CandFixed cand_fixed(int e, int r, const LayerTables& T) {
+    CandFixed f;
+    f.cpk = T.ptab[e] & 63u;
+    f.okm = 1u;
+    f.cmask = 1ull << (T.ptab[e] & 63u);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const int v = a < r ? (int)T.rep[e * r + a] : -1;
+        if (v >= 0) {
+            f.cpk |= (unsigned)(v & 63) << (8 * (a + 1));
+            f.okm |= 1u << (a + 1);
+            f.cmask |= 1ull << (v & 63);
+        }
+    }
+    return f;
+}
+__device__ __forceinline__ unsigned cand_order(unsigned cpk, const unsigned long long* K) {
+    unsigned long long s[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) s[i] = K[(cpk >> (8 * i)) & 63u];
+    unsigned bef = 0u;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (j != i && (s[j] < s[i] || (j < i && s[j] == s[i]))) bef |= 1u << (4 * i + j);
+    return bef;
+}
+__device__ __forceinline__ void cand_tables(const CandFixed& f, unsigned bef, unsigned long long feas, unsigned& w0,
+                                            unsigned& w1) {
+    unsigned okf = f.okm;
+    if (f.cmask & feas) {
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+            if (!((feas >> ((f.cpk >> (8 * i)) & 63u)) & 1ull)) okf &= ~(1u << i);
+    }
+    const int m = __popc(okf);
+    unsigned bb = 0u;                       // partitions by position, one byte each
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int pos = __popc(okf & (bef >> (4 * i)) & 15u);
+        if ((okf >> i) & 1u) bb |= ((f.cpk >> (8 * i)) & 0xffu) << (8 * pos);
+    }
+    // positions beyond the count repeat the first
+    const unsigned keep = m >= 4 ? 0xffffffffu : (1u << (8 * m)) - 1u;
+    bb = (bb & keep) | (((bb & 0xffu) * 0x01010101u) & ~keep);
+    w0 = (unsigned)m | (bb << 8);
+    w1 = bb >> 24;
 }
 
 __device__ __forceinline__ void build_candidates(int E, int r, const LayerTables& T, unsigned long long feas) {
@@ -745,6 +807,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                                                // each CTA stores its own row into all its peers before the barrier
     __shared__ unsigned wsum[kChainThreads / 32 + 1];
     __shared__ unsigned long long feas_s;
+    __shared__ uint4 candfix[32];              // cand_fixed of the replicated experts of ranks 1..32
     __shared__ unsigned long long mine_s[64 + 24];   // the scan kernel's sums of the current micro-batch (row words)
     __shared__ __align__(16) unsigned long long candm[(kMaxRank + 1) * 4];   // by rank: one-hot masks (type M) of the first four candidates
     __shared__ unsigned bigq_s;                                 // ranks that list more than four candidates
@@ -912,6 +975,28 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                 dst[0] = src[0]; dst[1] = src[1]; dst[2] = src[2];
             }
         };
+        // r <= 3 and at most 32 replicated experts (the usual case): lane i of the first warp owns the expert of rank i + 1
+        const bool lane_owns = tid < nrep && nrep <= 32 && r <= 3;
+        // (kept in shared memory, not in registers: the record loop of the other warps needs every register it has)
+        if (lane_owns) {
+            const CandFixed f0 = cand_fixed((int)replist[tid], r, T);
+            candfix[tid] = make_uint4(f0.cpk, f0.okm, (unsigned)f0.cmask, (unsigned)(f0.cmask >> 32));
+        }
+        __syncwarp();
+        auto put_tables = [&](int i, unsigned w0, unsigned w1) {
+            unsigned* o = reinterpret_cast<unsigned*>(T.cand + (int)replist[i] * kCandStride);   // 4-byte aligned entries
+            o[0] = w0;
+            o[1] = w1;
+            if (i < kMaxRank) {
+                M* cm = reinterpret_cast<M*>(candm) + (i + 1) * 4;
+                cm[0] = (M)1 << ((w0 >> 8) & 0xffu);
+                cm[1] = (M)1 << ((w0 >> 16) & 0xffu);
+                cm[2] = (M)1 << (w0 >> 24);
+                cm[3] = (M)1 << (w1 & 0xffu);
+                unsigned* dst = reinterpret_cast<unsigned*>(candr + (i + 1) * kCandStride);
+                dst[0] = w0; dst[1] = w1; dst[2] = 0u;
+            }
+        };
         unsigned cA1 = 0u, cA2 = 0u, cB1 = 0u, cB2 = 0u;
         if (tid >= 32 && tid < 64) {
             if (lane == 0) prefetch_rows(0, 3);
@@ -958,10 +1043,24 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
             // micro-batch).  The second warp meanwhile publishes this micro-batch's record counts.
             unsigned cC1 = 0u, cC2 = 0u;
             if (tid < 32) {
+                // the order of an expert's candidates needs the loads only: its compares run under the guard's fp64 chain
+                CandFixed cf = {0u, 0u, 0ull};
+                if (lane_owns) {
+                    const uint4 q = candfix[lane];
+                    cf.cpk = q.x;
+                    cf.okm = q.y;
+                    cf.cmask = (unsigned long long)q.z | ((unsigned long long)q.w << 32);
+                }
+                const unsigned bef = lane_owns ? cand_order(cf.cpk, Ks) : 0u;
                 const unsigned long long fm = load_guard_warp(Ls, P, p.theta, lane);
                 if (lane == 0) { feas_s = fm; bigq_s = 0u; }
                 __syncwarp();
-                if (lane < nrep && nrep <= 32) cand_of(lane, fm);       // step 3: the usual case, no second barrier
+                // step 3: the usual case, no second barrier
+                if (lane_owns) {
+                    unsigned w0, w1;
+                    cand_tables(cf, bef, fm, w0, w1);
+                    put_tables(lane, w0, w1);
+                } else if (lane < nrep && nrep <= 32) cand_of(lane, fm);
                 if constexpr (MODE == kModeGrid) early();
             } else if (tid < 64) {
                 fetch_counts(mb + 2, cC1, cC2);
