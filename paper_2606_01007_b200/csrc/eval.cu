@@ -1200,6 +1200,35 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                         }
 #pragma unroll
                         for (int q = 0; q < RF; ++q) v[q] = recs[x[q]];
+                        if constexpr (!multi && !OUT && RF > 1) {
+                            if (r <= 3) {
+                                // One pending slot each and at most four candidates: straight-line code without a branch,
+                                // so that the RF independent chains (shared load -> pick -> counter) overlap.  A record
+                                // beyond the end stands in as rank 1 with its increments switched off.
+                                M R[RF], hb[RF], pm[RF];
+                                bool live[RF];
+#pragma unroll
+                                for (int q = 0; q < RF; ++q) {
+                                    live[q] = g0 + (unsigned)q * stride < tot;
+                                    const unsigned rk = live[q] ? v[q].z : 1u;
+                                    const unsigned rq = (rk >> ((__ffs(rk) - 1) & ~3)) & 15u;
+                                    R[q] = rec_set<M>(v[q]);
+                                    hb[q] = (M)1 << ((v[q].w >> 16) & 63u);
+                                    pm[q] = pick_slot(rq, R[q] | hb[q]);
+                                }
+#pragma unroll
+                                for (int q = 0; q < RF; ++q) {
+                                    R[q] |= pm[q];
+                                    const int pick = sizeof(M) == 8 ? 63 - __clzll((long long)pm[q]) : 31 - __clz((int)pm[q]);
+                                    const int nR = popc_m<M>(R[q]), rem = popc_m<M>(R[q] & ~hb[q]);
+                                    if (live[q]) {
+                                        sred_inc(cl + (unsigned)pick * 128u);
+                                        add_comm((v[q].w >> 13) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
+                                    }
+                                }
+                                continue;
+                            }
+                        }
 #pragma unroll
                         for (int q = 0; q < RF; ++q)
                             if (g0 + (unsigned)q * stride < tot) resolve(MULTI, rec_set<M>(v[q]), v[q].z, v[q].w, x[q]);
