@@ -44,7 +44,9 @@
 
 #include <algorithm>
 #include <type_traits>
+#include <map>
 #include <mutex>
+#include <tuple>
 
 #include "tacg_common.cuh"
 
@@ -1630,10 +1632,11 @@ void chain_plan(const tacg_ctx* ctx, const EvalGeom& g, int& mode, int& cs, int&
     // cluster size: as many CTAs per layer as the SM count allows, up to 16 (non-portable above 8)
     const int slots = 2 * ctx->sm_count;           // resident CTAs (two per SM)
     const long long tokens = std::min<long long>(g.B, g.N);
-    cs = 1;
-    while (cs < 16 && (long long)g.L * cs * 2 <= slots) cs *= 2;
+    // any size, not only powers of two: 5 at L = 58, 6 at L = 48; launch_chain lowers it if the clusters do not all fit
+    cs = (int)std::max<long long>(1, std::min<long long>(16, slots / std::max(1, g.L)));
+    if (cs > 8 && cs < 16) cs = 8;              // above the portable 8 only the full 16
     // a micro-batch with few records gains nothing from more CTAs
-    while (cs > 1 && tokens < (long long)cs * 2048) cs /= 2;
+    cs = (int)std::max<long long>(1, std::min<long long>(cs, tokens / 2048));
     groups = std::min(g.L, std::max(1, slots / cs));
     mode = cs > 1 ? kModeCluster : kModeSingle;
     // few layers and long micro-batches: the largest cluster leaves most SMs idle.  One CTA per SM at most, about 1024
@@ -1676,13 +1679,47 @@ int launch_chain(EvalCall& c) {
         TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         TACG_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, c.cp));
     } else if (c.mode == kModeCluster) {
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = cs;
-        attr[0].val.clusterDim.y = 1;
-        attr[0].val.clusterDim.z = 1;
         auto kern = eval_chain_kernel<M, OUT, kModeCluster>;
         TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         if (cs > 8) TACG_CUDA_TRY(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        // The clusters of all layers should be resident at once (a second wave would double the time): a cluster needs
+        // its CTAs inside one GPC, so slots / cs over-estimates how many fit.  Ask the runtime, largest size first.
+        // (the answer depends on the kernel, its shared memory, the device and L: remembered per process)
+        static std::mutex memo_mutex;
+        static std::map<std::tuple<const void*, size_t, int, int, int>, int> memo;
+        const auto key = std::make_tuple((const void*)kern, smem, ctx->device, g.L, cs);
+        int use = 0;
+        {
+            std::lock_guard<std::mutex> lock(memo_mutex);
+            auto it = memo.find(key);
+            if (it != memo.end()) use = it->second;
+        }
+        if (use == 0) {
+            for (use = cs; use > 1; --use) {
+                if (use > 8 && use < 16) continue;
+                attr[0].val.clusterDim.x = use;
+                cfg.gridDim = dim3(std::min(g.L, std::max(1, 2 * ctx->sm_count / use)) * use);
+                int fit = 0;
+                if (cudaOccupancyMaxActiveClusters(&fit, kern, &cfg) == cudaSuccess && fit * use >= (int)cfg.gridDim.x) break;
+                (void)cudaGetLastError();
+            }
+            std::lock_guard<std::mutex> lock(memo_mutex);
+            memo[key] = use;
+        }
+        if (use <= 1) {
+            // not even pairs fit side by side: plain CTAs
+            c.mode = kModeSingle;
+            c.cs = 1;
+            c.groups = std::min(g.L, 2 * ctx->sm_count);
+            return launch_chain<M, OUT>(c);
+        }
+        c.cp.groups = std::min(g.L, std::max(1, 2 * ctx->sm_count / use));
+        c.cp.gper = use;
+        attr[0].val.clusterDim.x = use;
+        cfg.gridDim = dim3(c.cp.groups * use);
         TACG_CUDA_TRY(ctx, cudaLaunchKernelEx(&cfg, kern, c.cp));
     } else {
         auto kern = eval_chain_kernel<M, OUT, kModeSingle>;
