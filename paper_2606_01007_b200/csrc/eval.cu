@@ -1231,6 +1231,51 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                                 continue;
                             }
                         }
+                        if constexpr (multi && !OUT && RF > 1) {
+                            if (r <= 3) {
+                                // Several pending slots each: the RF records advance in lock step, one slot per pass, each
+                                // pass straight-line code (RF independent chains); a record that is done, or beyond the
+                                // end, stands in as rank 1 with its updates switched off.
+                                M R[RF], hb[RF];
+                                unsigned rk[RF], any = 0u;
+                                bool live[RF];
+#pragma unroll
+                                for (int q = 0; q < RF; ++q) {
+                                    live[q] = g0 + (unsigned)q * stride < tot;
+                                    rk[q] = live[q] ? v[q].z : 0u;
+                                    any |= rk[q];
+                                    R[q] = rec_set<M>(v[q]);
+                                    hb[q] = (M)1 << ((v[q].w >> 16) & 63u);
+                                }
+                                while (any) {
+                                    M pm[RF];
+                                    int sh[RF];
+#pragma unroll
+                                    for (int q = 0; q < RF; ++q) {
+                                        const unsigned rkx = rk[q] ? rk[q] : 1u;
+                                        sh[q] = (__ffs(rkx) - 1) & ~3;
+                                        pm[q] = pick_slot((rkx >> sh[q]) & 15u, R[q] | hb[q]);
+                                    }
+                                    any = 0u;
+#pragma unroll
+                                    for (int q = 0; q < RF; ++q) {
+                                        const int pick = sizeof(M) == 8 ? 63 - __clzll((long long)pm[q]) : 31 - __clz((int)pm[q]);
+                                        if (rk[q]) {
+                                            R[q] |= pm[q];
+                                            sred_inc(cl + (unsigned)pick * 128u);
+                                            rk[q] &= ~(15u << sh[q]);
+                                        }
+                                        any |= rk[q];
+                                    }
+                                }
+#pragma unroll
+                                for (int q = 0; q < RF; ++q) {
+                                    const int nR = popc_m<M>(R[q]), rem = popc_m<M>(R[q] & ~hb[q]);
+                                    if (live[q]) add_comm((v[q].w >> 13) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
+                                }
+                                continue;
+                            }
+                        }
 #pragma unroll
                         for (int q = 0; q < RF; ++q)
                             if (g0 + (unsigned)q * stride < tot) resolve(MULTI, rec_set<M>(v[q]), v[q].z, v[q].w, x[q]);
