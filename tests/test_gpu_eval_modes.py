@@ -105,6 +105,30 @@ def test_microbatch_lengths_around_the_kernel_switch(tacg, ctx, B):
     _check(tacg, ctx, cfg.E, cfg.F, cfg.P, idx, fam, primary, replicas, 0.1, 0.9, B, offset=11)
 
 
+@pytest.mark.parametrize("cfg_id,N,L,B", [(3, 70000, 2, 8192), (5, 140000, 1, 65536), (4, 60000, 3, 4096)])
+def test_initial_state_with_ties_and_signed_zeros(tacg, ctx, cfg_id, N, L, B):
+    """The chain kernel orders an expert's candidates by integer keys of the loads (order_key): equal loads must keep
+    slot order, +0.0 and -0.0 are equal, and a guard decided on the very first micro-batch has to see the given state.
+    Rounded initial loads give many exact ties; the three launch modes of the chain kernel each get a case."""
+    cfg, idx, fam = _trace(cfg_id, N, L)
+    primary = tracegen.random_placement(cfg.E, cfg.P, cfg.capacity, L, seed=31)
+    replicas = tracegen.random_replicas(primary, cfg.P, cfg.r, cfg.n_rep, seed=32)
+    rng = np.random.default_rng(33)
+    state0 = np.round(rng.uniform(0.0, 3.0, size=(L, cfg.P))) * 1000.0        # few distinct values: ties
+    state0[:, ::5] = -0.0
+    state0[:, 1::7] = 0.0
+    want = cbind.eval_placement(idx.numpy(), fam.numpy(), cfg.E, cfg.F, cfg.P, primary, replicas, theta=0.15, rho=0.995,
+                                microbatch=B, load_state=state0.copy())
+    st = torch.from_numpy(state0.copy()).cuda()
+    got = tacg.tacg_eval_placement(ctx, idx.cuda(), fam.cuda(), cfg.E, cfg.F, cfg.P, torch.from_numpy(primary).cuda(),
+                                   torch.from_numpy(replicas).cuda(), theta=0.15, rho=0.995, microbatch=B, load_state=st)
+    torch.cuda.synchronize()
+    assert (_u64(got["load"]) == want["load"]).all()
+    assert (_u64(got["comm_span"]) == want["comm_span"]).all()
+    assert (_u64(got["comm_remote"]) == want["comm_remote"]).all()
+    assert (st.cpu().numpy().view(np.uint64) == want["load_state"].view(np.uint64)).all()
+
+
 def _random_trace(E, k, L, N, F, seed):
     g = torch.Generator().manual_seed(seed)
     idx = torch.stack([torch.stack([torch.randperm(E, generator=g)[:k] for _ in range(N)]) for _ in range(L)]).to(torch.int16)
