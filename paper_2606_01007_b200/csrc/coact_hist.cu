@@ -28,7 +28,7 @@ namespace {
 constexpr int kThreads = 1024;           // one CTA per SM
 constexpr int kWarps = kThreads / 32;
 constexpr int kBatch = 4;                 // tokens per thread whose loads are issued together
-constexpr int kRun = 4;                   // items (of kThreads tokens) walked together
+constexpr int kRun = 256;                   // items (of kThreads tokens) walked together
 constexpr int kRunFam = 256;              // the same in family mode (long runs: the set-up of a run, list bounds and
                                           // 64-bit bases, costs as much as four tokens)
 
