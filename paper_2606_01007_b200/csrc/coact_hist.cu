@@ -447,14 +447,25 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
             const unsigned* __restrict__ list = p.perm + (size_t)fg * (size_t)p.N;
             if (l == 0 && tid == 0) sntok[0] += j1 - j0;
             if constexpr (KT >= 2) {
+                // the token ids of a round are read from the list one round ahead: the row gather does not wait for them
+                unsigned tok[kBatch];
+#pragma unroll
+                for (int u = 0; u < kBatch; ++u) {
+                    const unsigned j = j0 + tid + u * kThreads;
+                    tok[u] = j < j1 ? __ldg(list + j) : 0u;
+                }
                 for (unsigned jb = j0 + tid; jb - lane < j1; jb += kThreads * kBatch) {     // warp-uniform trip count
                     unsigned w[kBatch][KT / 2];
                     bool live[kBatch];
 #pragma unroll
                     for (int u = 0; u < kBatch; ++u) {
-                        const unsigned j = jb + u * kThreads;
-                        live[u] = j < j1;
-                        if (live[u]) load_raw<KT>(lbase + (size_t)__ldg(list + j) * KT, w[u]);
+                        live[u] = jb + u * kThreads < j1;
+                        if (live[u]) load_raw<KT>(lbase + (size_t)tok[u] * KT, w[u]);
+                    }
+#pragma unroll
+                    for (int u = 0; u < kBatch; ++u) {
+                        const unsigned jn = jb + (kBatch + u) * kThreads;
+                        tok[u] = jn < j1 ? __ldg(list + jn) : 0u;
                     }
 #pragma unroll
                     for (int u = 0; u < kBatch; ++u) process(live[u], w[u], 0);
