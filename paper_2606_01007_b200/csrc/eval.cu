@@ -492,7 +492,11 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
     unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;                    // this thread's family words
     const unsigned al = saddr(acc);
     const unsigned tb = saddr(tab16), pb8 = saddr(ptab);
-    const int stepP = kEvalThreads % P;
+    // A thread's tokens of an item are S apart, S the largest multiple of P not above the CTA size (448..512): the home
+    // partition (token index mod P) of all of them is the same, no per-token update.  The kEvalThreads % P last threads
+    // idle when P does not divide the CTA size (no configuration of the paper).
+    const int S = kEvalThreads - kEvalThreads % P;
+    const bool worker = tid < S;
 
     for (int i = tid; i < (kSink + 1) * 32; i += kEvalThreads) cnt[i] = 0u;
 #pragma unroll
@@ -535,18 +539,18 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
         unsigned char* cost_l = (OUT && p.cost) ? p.cost + (size_t)layer * g.N + t0 : nullptr;
         signed char* serve_l = (OUT && p.serve) ? p.serve + ((size_t)layer * g.N + t0) * k : nullptr;
         Rec* recs = RECS ? p.rec + (size_t)item * g.slice : nullptr;
-        int home = (hm0 + tid) % P;
+        const int home = (hm0 + tid) % P;
         const int8_t* fam0 = p.family + t0;
         const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
 
-        for (int ob = tid; ob < n + tid; ob += kEvalThreads * U) {      // uniform trip count across the CTA
+        for (int ob = tid; ob < n + tid; ob += S * U) {      // uniform trip count across the CTA
             int f[U];
             unsigned w[U][NW];
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int o = ob + u * kEvalThreads;
+                const int o = ob + u * S;
                 f[u] = -1;
-                if (o < n) {
+                if (worker && o < n) {
                     f[u] = fam0[o];
                     if constexpr (KT == 8) {
                         const uint4 v = __ldg(reinterpret_cast<const uint4*>(rows0) + o);
@@ -568,7 +572,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
             int ndef = 0;            // this lane's deferred tokens of the batch: one pending slot | several << 16
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                const int o = ob + u * kEvalThreads;
+                const int o = ob + u * S;
                 const bool live = (unsigned)f[u] < (unsigned)F;
                 drank[u] = 0u;
                 dmeta[u] = 0u;
@@ -634,14 +638,10 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                         ndef += dmulti[u] ? 0x10000 : 1;
                     }
                     sred_add(al + (unsigned)f[u] * 128u, packed);
-                } else if (o < n) {
+                } else if (worker && o < n) {
                     if (OUT && cost_l) cost_l[o] = 0;
                     if (OUT && serve_l)
                         for (int j = 0; j < k; ++j) serve_l[(size_t)o * k + j] = -1;
-                }
-                if (stepP) {
-                    home += stepP;
-                    if (home >= P) home -= P;
                 }
             }
             if constexpr (RECS) {
