@@ -488,10 +488,10 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
     const int P = g.P, k = KT > 0 ? KT : g.k, E = g.E, F = g.F;
     const long long T = (long long)g.L * g.ipl;
     const long long lo = (long long)blockIdx.x * T / gridDim.x, hi = (long long)(blockIdx.x + 1) * T / gridDim.x;
-    const unsigned cl = saddr(cnt + lane);                                  // this lane's counter column
+    const unsigned cl = saddr_kept(cnt + lane);                             // this lane's counter column
     unsigned* acc = accb + (tid >> 5) * (8 * 32) + lane;                    // this thread's family words
-    const unsigned al = saddr(acc);
-    const unsigned tb = saddr(tab16), pb8 = saddr(ptab);
+    const unsigned al = saddr_kept(acc);
+    const unsigned tb = saddr(tab16), pb8 = saddr(ptab), nrb = saddr(&nrec_s);
     // A thread's tokens of an item are S apart, S the largest multiple of P not above the CTA size (448..512): the home
     // partition (token index mod P) of all of them is the same, no per-token update.  The kEvalThreads % P last threads
     // idle when P does not divide the CTA size (no configuration of the paper).
@@ -539,6 +539,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
         unsigned char* cost_l = (OUT && p.cost) ? p.cost + (size_t)layer * g.N + t0 : nullptr;
         signed char* serve_l = (OUT && p.serve) ? p.serve + ((size_t)layer * g.N + t0) * k : nullptr;
         Rec* recs = RECS ? p.rec + (size_t)item * g.slice : nullptr;
+        asm volatile("" : "+l"(recs));      // kept in its register pair: otherwise rebuilt from item and slice per record
         const int home = (hm0 + tid) % P;
         const int8_t* fam0 = p.family + t0;
         const unsigned* rows0 = reinterpret_cast<const unsigned*>(base + (size_t)t0 * k);   // KT > 0 only
@@ -656,7 +657,10 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                     }
                     const int total = __shfl_sync(0xffffffffu, inc, 31);
                     unsigned wbase = 0u;
-                    if (lane == 31) wbase = atomicAdd(&nrec_s, (unsigned)total);
+                    // (PTX directly: for atomicAdd under `if (lane == 31)` the compiler emits its generic warp-aggregation
+                    // sequence, a vote, a leader election and a popcount, for an add that one lane executes)
+                    if (lane == 31)
+                        asm volatile("atom.shared.add.u32 %0, [%1], %2;" : "=r"(wbase) : "r"(nrb), "r"((unsigned)total) : "memory");
                     wbase = __shfl_sync(0xffffffffu, wbase, 31);
                     const unsigned mine = wbase + (unsigned)(inc - ndef);
                     unsigned pos1 = mine & 0xffffu;                               // singles: upwards from entry 0
