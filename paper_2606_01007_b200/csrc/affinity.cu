@@ -99,8 +99,11 @@ struct AffArgs {
 // Dynamic smem: region A = 4*F*E doubles (u, c, sc, dv of the preference step; afterwards the W rows of
 // this CTA's row block and the partition order), region B = E*F doubles (the preference table).
 // FT = the family count at compile time (4 and 8: the paper's F = 4 and the ABI maximum), 0 = runtime.
-template <int FT>
-__global__ void __cluster_dims__(kCluster, 1, 1) __launch_bounds__(kRowThreads)
+// MINB = CTAs per SM the register budget must allow.  The kernel is bound by the latency of its loads of C: with E >= 256
+// (eight rounds per lane) the unrolled loops keep four rounds in flight and want the registers (MINB = 2: 128 of them,
+// two CTAs per SM); below that three resident CTAs per SM matter more (MINB = 3: 80 registers).
+template <int FT, int MINB>
+__global__ void __cluster_dims__(kCluster, 1, 1) __launch_bounds__(kRowThreads, MINB)
 affinity_fused_kernel(AffArgs a) {
     tacg_pdl_prologue();
     extern __shared__ double fsm[];
@@ -160,6 +163,8 @@ affinity_fused_kernel(AffArgs a) {
         unsigned long long acc[8];
 #pragma unroll
         for (int f = 0; f < 8; ++f) acc[f] = 0ull;
+        // (unrolled: the kernel is bound by the latency of these loads, four rounds of F of them in flight per lane)
+#pragma unroll 4
         for (int j = lane; j < E; j += 32) {
             double ab = 0.0;
 #pragma unroll
@@ -275,6 +280,7 @@ affinity_fused_kernel(AffArgs a) {
         const int i = b * kRowsPerCta + warp;
         if (i >= E) continue;
         const double* pi = ptab + (size_t)i * F;
+#pragma unroll 4
         for (int j = lane; j < E; j += 32) {
             const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), iamax, pi, ptab + (size_t)j * F, F, a.alpha);
             wr[j] = w;
@@ -302,11 +308,13 @@ affinity_fused_kernel(AffArgs a) {
         if (i >= E) continue;
         const double* pi = ptab + (size_t)i * F;
         const int pa = pr[i] & 63;
+#pragma unroll 4
         for (int j = lane; j < E; j += 32) {
             const int pb = pr[j] & 63;
             double g = 0.0;
+            // (the entry is loaded for every pair, also the 1 in P inside one partition: no branch around the loads)
+            const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), iamax, pi, ptab + (size_t)j * F, F, a.alpha);
             if (pa != pb) {
-                const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), iamax, pi, ptab + (size_t)j * F, F, a.alpha);
                 g = affl[(size_t)i * P + pb] + affl[(size_t)j * P + pa] - affl[(size_t)i * P + pa] - affl[(size_t)j * P + pb] - 2.0 * w;
             }
             a.gain_out[((size_t)l * E + i) * E + j] = (float)g;
@@ -486,7 +494,8 @@ int tacg_launch_affinity(tacg_ctx* ctx, const uint32_t* D, const uint32_t* C, co
         TACG_LAUNCH_CHECK(ctx);
         return TACG_OK;
     };
-    const int rc = F == 4 ? launch(affinity_fused_kernel<4>) : F == 8 ? launch(affinity_fused_kernel<8>) : launch(affinity_fused_kernel<0>);
+    const int rc = F == 4 ? (E >= 256 ? launch(affinity_fused_kernel<4, 2>) : launch(affinity_fused_kernel<4, 3>))
+                 : F == 8 ? launch(affinity_fused_kernel<8, 3>) : launch(affinity_fused_kernel<0, 3>);
     if (rc != TACG_OK) return rc;
     if (gesr) {
         TACG_CUDA_TRY(ctx, tacg_launch_pdl(gesr_score_kernel, rows, dim3(kRowThreads), 0, ctx->stream, C, nt, E, F, gesr->lambda1,
