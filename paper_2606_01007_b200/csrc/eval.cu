@@ -685,10 +685,10 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                 const unsigned s = __reduce_add_sync(0xffffffffu, av & 0x7ffu);
                 const unsigned q = __reduce_add_sync(0xffffffffu, (av >> 11) & 0x7ffu);
                 const unsigned c = __reduce_add_sync(0xffffffffu, av >> 22);
-                if (lane == 0) {
-                    if (s) atomicAdd(&comm_s[fq], s);
-                    if (q) atomicAdd(&comm_s[8 + fq], q);
-                    if (c) atomicAdd(&fam_s[fq], c);
+                if (lane == 0) {          // plain PTX: no compiler-generated warp aggregation around a one-lane add
+                    if (s) sred_add(saddr(comm_s) + 4u * fq, s);
+                    if (q) sred_add(saddr(comm_s) + 4u * (8 + fq), q);
+                    if (c) sred_add(saddr(fam_s) + 4u * fq, c);
                 }
             }
         }
@@ -890,8 +890,8 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                         const unsigned sp = __reduce_add_sync(0xffffffffu, av & 0xffffu);
                         const unsigned rq = __reduce_add_sync(0xffffffffu, av >> 16);
                         if (lane == 0) {
-                            if (sp) atomicAdd(&dsum32[fq], sp);
-                            if (rq) atomicAdd(&dsum32[8 + fq], rq);
+                            if (sp) sred_add(db + 4u * fq, sp);
+                            if (rq) sred_add(db + 4u * (8 + fq), rq);
                         }
                     }
                 }
