@@ -548,15 +548,41 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
 
 // ---- family mode: the tokens of every family as an increasing list, with the list position of every block of
 // kThreads tokens (= one work item), built once per call in three small launches.
-// (1) boff[f][b] = tokens of family f in block b
-__global__ void __launch_bounds__(kThreads)
+// (1) boff[f][b] = tokens of family f in block b.  256 threads per block of kThreads tokens, four consecutive tokens each.
+constexpr int kPartThreads = kThreads / 4;
+constexpr int kPartWarps = kPartThreads / 32;
+
+__device__ __forceinline__ void part_load4(const int8_t* __restrict__ family, long long N, long long t4, int (&f)[4]) {
+    if (t4 + 3 < N && ((reinterpret_cast<uintptr_t>(family) + (uintptr_t)t4) & 3u) == 0u) {
+        const unsigned v = *reinterpret_cast<const unsigned*>(family + t4);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) f[q] = (int)(signed char)((v >> (8 * q)) & 0xffu);
+    } else {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) f[q] = t4 + q < N ? (int)family[t4 + q] : -1;
+    }
+}
+
+__global__ void __launch_bounds__(kPartThreads)
 part_count_kernel(const int8_t* __restrict__ family, long long N, int F, int nb, unsigned* __restrict__ boff) {
     tacg_pdl_prologue();
-    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
-    const int f = t < N ? (int)family[t] : -1;
+    __shared__ unsigned wc[8][kPartWarps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int f[4];
+    part_load4(family, N, (long long)blockIdx.x * kThreads + (long long)threadIdx.x * 4, f);
     for (int ff = 0; ff < F; ++ff) {
-        const int c = __syncthreads_count(f == ff);
-        if (threadIdx.x == 0) boff[(size_t)ff * (nb + 1) + blockIdx.x] = (unsigned)c;
+        unsigned c = 0;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) c += f[q] == ff;
+        c = __reduce_add_sync(0xffffffffu, c);
+        if (lane == 0) wc[ff][warp] = c;
+    }
+    __syncthreads();
+    if ((int)threadIdx.x < F) {
+        unsigned c = 0;
+#pragma unroll
+        for (int w = 0; w < kPartWarps; ++w) c += wc[threadIdx.x][w];
+        boff[(size_t)threadIdx.x * (nb + 1) + blockIdx.x] = c;
     }
 }
 
@@ -595,26 +621,50 @@ __global__ void __launch_bounds__(kThreads) part_scan_kernel(int nb, unsigned* _
     }
 }
 
-// (3) perm[f][boff[f][b] + rank of the token among its family's tokens of block b] = token
-__global__ void __launch_bounds__(kThreads)
+// (3) perm[f][boff[f][b] + rank of the token among its family's tokens of block b] = token.  The per-thread counts of
+// four families travel through one warp scan as 8-bit fields of a word (a warp holds 128 tokens: 128 fits).
+__global__ void __launch_bounds__(kPartThreads)
 part_scatter_kernel(const int8_t* __restrict__ family, long long N, int F, int nb, const unsigned* __restrict__ boff,
                     unsigned* __restrict__ perm) {
     tacg_pdl_prologue();
-    __shared__ unsigned wc[8][kWarps];
+    __shared__ unsigned wc[2][kPartWarps];          // warp totals, packed like the scan words
+    __shared__ unsigned base_s[8];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const long long t = (long long)blockIdx.x * kThreads + threadIdx.x;
-    const int f = t < N ? (int)family[t] : -1;
-    unsigned rank = 0;
-    for (int ff = 0; ff < F; ++ff) {
-        const unsigned b = __ballot_sync(0xffffffffu, f == ff);
-        if (lane == 0) wc[ff][warp] = __popc(b);
-        if (f == ff) rank = __popc(b & ((1u << lane) - 1u));
+    const long long t4 = (long long)blockIdx.x * kThreads + (long long)threadIdx.x * 4;
+    int f[4];
+    part_load4(family, N, t4, f);
+    if ((int)threadIdx.x < F) base_s[threadIdx.x] = boff[(size_t)threadIdx.x * (nb + 1) + blockIdx.x];
+    unsigned own[2] = {0u, 0u};                     // this thread's tokens per family, packed
+#pragma unroll
+    for (int q = 0; q < 4; ++q)
+        if ((unsigned)f[q] < (unsigned)F) own[f[q] >> 2] += 1u << (8 * (f[q] & 3));
+    unsigned inc[2] = {own[0], own[1]};
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const unsigned v0 = __shfl_up_sync(0xffffffffu, inc[0], d), v1 = __shfl_up_sync(0xffffffffu, inc[1], d);
+        if (lane >= d) { inc[0] += v0; inc[1] += v1; }
     }
+    if (lane == 31) { wc[0][warp] = inc[0]; wc[1][warp] = inc[1]; }
     __syncthreads();
-    if ((unsigned)f < (unsigned)F) {
-        for (int w = 0; w < warp; ++w) rank += wc[f][w];
-        TACG_ASSERT((long long)boff[(size_t)f * (nb + 1) + blockIdx.x] + rank < N);
-        perm[(size_t)f * (size_t)N + boff[(size_t)f * (nb + 1) + blockIdx.x] + rank] = (unsigned)t;
+    // tokens of each family before this thread in the block: earlier warps (fields up to 128 * 7: sum them unpacked)
+    unsigned before[8];
+#pragma unroll
+    for (int ff = 0; ff < 8; ++ff) {
+        unsigned c = ((inc[ff >> 2] - own[ff >> 2]) >> (8 * (ff & 3))) & 0xffu;
+        for (int w = 0; w < warp; ++w) c += (wc[ff >> 2][w] >> (8 * (ff & 3))) & 0xffu;
+        before[ff] = c;
+    }
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int ff = f[q];
+        if ((unsigned)ff < (unsigned)F) {
+            unsigned r = 0;
+#pragma unroll
+            for (int x = 0; x < 8; ++x)
+                if (x == ff) { r = before[x]; before[x] += 1u; }
+            TACG_ASSERT((long long)base_s[ff] + r < N);
+            perm[(size_t)ff * (size_t)N + base_s[ff] + r] = (unsigned)(t4 + q);
+        }
     }
 }
 
@@ -736,12 +786,12 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
     if (filter) {
         unsigned* perm = const_cast<unsigned*>(p.perm);
         unsigned* boff = const_cast<unsigned*>(p.boff);
-        TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_count_kernel, dim3(p.cps), dim3(kThreads), 0, ctx->stream, family,
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_count_kernel, dim3(p.cps), dim3(kPartThreads), 0, ctx->stream, family,
                                            (long long)N, F, p.cps, boff));
         TACG_LAUNCH_CHECK(ctx);
         TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_scan_kernel, dim3(F), dim3(kThreads), 0, ctx->stream, p.cps, boff));
         TACG_LAUNCH_CHECK(ctx);
-        TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_scatter_kernel, dim3(p.cps), dim3(kThreads), 0, ctx->stream, family,
+        TACG_CUDA_TRY(ctx, tacg_launch_pdl(part_scatter_kernel, dim3(p.cps), dim3(kPartThreads), 0, ctx->stream, family,
                                            (long long)N, F, p.cps, (const unsigned*)boff, perm));
         TACG_LAUNCH_CHECK(ctx);
     }
