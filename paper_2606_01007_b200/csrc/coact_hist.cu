@@ -517,7 +517,7 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
     unsigned rs = 0;
     unsigned corr = 0;
     for (int g = lane; g < ng; g += 32) corr += slot0[(size_t)g * gstride + (size_t)p.Fs * tri + (size_t)fs * E + i];
-#pragma unroll 2
+#pragma unroll 4
     for (int j = lane; j < E; j += 32) {
         unsigned v = 0;
         if (j != i) {
