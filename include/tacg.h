@@ -253,7 +253,7 @@ int tacg_eval_placement(tacg_ctx* ctx,
  * slot served by its primary partition), for callers that must not allocate: code under CUDA graph capture, tight
  * serving loops, harnesses that forbid cudaMalloc.  It calls no cudaMalloc, cudaFree or allocating library routine
  * and does not touch the context's growable scratch: its only scratch, the per-slice partial sums
- * L * ceil(N / slice) * align4(P + 3F + 2) 32-bit words (slice = 8192 tokens, fewer for short traces), lives in
+ * L * ceil(N / slice) * align4(P + 3F + 2) 32-bit words (slice <= 32768 tokens, chosen for the balance of the scan grid), lives in
  * a fixed device array of TACG_NOALLOC_SCRATCH_BYTES that every GPU holding the library keeps until the process
  * exits.  A call that needs more fails with TACG_ERR_SHAPE and a text naming the two sizes (nothing is launched);
  * split the layers over several calls, or use tacg_eval_placement.

@@ -7,7 +7,7 @@
 //
 //   eval_scan_kernel   everything that does NOT depend on the load snapshot, at streaming speed and
 //                      without any wait: persistent CTAs walk items = (layer, micro-batch, slice of
-//                      <= 8192 tokens); per token the primary map is looked up in a 16-bit table, the
+//                      <= 32768 tokens); per token the primary map is looked up in a 16-bit table, the
 //                      slots of experts without replicas are counted (lane-private shared-memory
 //                      counters, no branch) and, when the token has no replicated slot, its communication
 //                      cost is final.  A token WITH replicated slots leaves one 16-byte record (accessed
@@ -56,7 +56,11 @@ namespace {
 
 constexpr int kEvalThreads = 512;    // eval_scan_kernel, select_kernel
 constexpr int kEvalBatch = 4;        // tokens per thread with their loads in flight together
-constexpr int kSlice = 8192;         // most tokens of a scan item (13-bit offsets in the records, 16 per thread)
+constexpr int kSlice = 32768;        // most tokens of a scan item (64 per thread).  Bounded by the packed sums: a thread's
+                                     // 11-bit span field (74 tokens x 16), the 16-bit record counts of an item, the chain
+                                     // kernel's 16-bit per-thread fields over a round of 32 slices
+constexpr int kOffBits = 15;         // record meta word: offset in the item (kOffBits) | family (3) | home partition (6)
+static_assert(kSlice <= (1 << kOffBits), "record offsets");
 constexpr int kChainThreads = 512;    // two CTAs per SM, so that clusters of 4 at L = 58 still use every SM
 constexpr unsigned kRecFlight = 4;    // records a chain thread loads before it resolves the first (cluster, single CTA)
 constexpr unsigned kRecFlightGrid = 1; // the same in grid mode, where a thread has one or two records per micro-batch
@@ -633,7 +637,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
                     } else {
                         dR[u] = R;
                         drank[u] = ranks;
-                        dmeta[u] = (unsigned)o | ((unsigned)f[u] << 13) | ((unsigned)home << 16);
+                        dmeta[u] = (unsigned)o | ((unsigned)f[u] << kOffBits) | ((unsigned)home << (kOffBits + 3));
                         const unsigned nz = (ranks | (ranks >> 1) | (ranks >> 2) | (ranks >> 3)) & 0x11111111u;
                         dmulti[u] = (nz & (nz - 1u)) != 0u;
                         ndef += dmulti[u] ? 0x10000 : 1;
@@ -647,7 +651,7 @@ __global__ void __launch_bounds__(kEvalThreads, 2) eval_scan_kernel(const ScanPa
             }
             if constexpr (RECS) {
                 // records of this batch: one warp-wide reservation (tokens with one pending slot | with several, 16 bits
-                // each: an item has at most 8192 tokens), then every lane writes its own
+                // each: an item has at most 32768 tokens), then every lane writes its own
                 if (__any_sync(0xffffffffu, ndef != 0)) {
                     int inc = ndef;
 #pragma unroll
@@ -869,7 +873,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
 
         // Per-family communication sums of a record.  Many records per thread and micro-batch (cluster, single CTA): one
         // conflict-free atomic into the thread's own word, span | remote << 16, folded once per round of slices
-        // (flush_acc; 16-bit fields: a thread takes at most 32 * 8192 / 512 records of <= 16 each per round).  Few
+        // (flush_acc; 16-bit fields: a thread takes at most 32 * 32768 / 512 records of <= 16 each per round).  Few
         // records per thread (grid mode): two atomics straight into the CTA's words -- ATOMS.ADD does not merge lanes
         // that hit one word, so this costs several wavefronts per instruction, but there is no fold to pay for.
         auto add_comm = [&](unsigned fam, unsigned span, unsigned rem) {
@@ -897,7 +901,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                 }
             }
         };
-        // a round of at most 32 slices adds less than 2^23 to a 32-bit sum; one thread per entry widens it between barriers
+        // a round of at most 32 slices adds less than 2^25 to a 32-bit sum; one thread per entry widens it between barriers
         auto fold_dsum = [&](int i) {
             dsum[i] += dsum32[i];
             dsum32[i] = 0u;
@@ -1131,7 +1135,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                 auto token_of = [&](unsigned x, unsigned meta) -> size_t {
                     long long t0, t1;
                     item_tokens(g, mb, s0 + (int)(x / slice), t0, t1);
-                    return (size_t)layer * g.N + t0 + (meta & 0x1fffu);
+                    return (size_t)layer * g.N + t0 + (meta & ((1u << kOffBits) - 1u));
                 };
                 // the pending slot whose rank sits at bit sh of the record's rank word
                 auto step = [&](M& R, M hb, unsigned rk, int sh, unsigned meta, unsigned x) {
@@ -1146,7 +1150,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                 // one record: its pending slots in slot order (lowest nibble first), then the communication cost.
                 // MULTI = false: the record class with exactly one pending slot, no loop.
                 auto resolve = [&](auto MULTI, M R, unsigned rk, unsigned meta, unsigned x) {
-                    const M hb = (M)1 << ((meta >> 16) & 63u);
+                    const M hb = (M)1 << ((meta >> (kOffBits + 3)) & 63u);
                     if constexpr (decltype(MULTI)::value) {
                         while (rk) {
                             const int sh = (__ffs(rk) - 1) & ~3;
@@ -1158,7 +1162,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                     }
                     const int nR = popc_m<M>(R), rem = popc_m<M>(R & ~hb);
                     if (OUT && p.cost) p.cost[token_of(x, meta)] = (unsigned char)rem;
-                    add_comm((meta >> 13) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
+                    add_comm((meta >> kOffBits) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
                 };
                 // one record class: flat index gi over the slices' records of that class -> entry of the record array.
                 // Within slice sl (flat indices [lo_sl, hi_sl)) the entry is xb + gi (first class, upwards from entry 0)
@@ -1219,7 +1223,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                                     const unsigned rk = live[q] ? v[q].z : 1u;
                                     const unsigned rq = (rk >> ((__ffs(rk) - 1) & ~3)) & 15u;
                                     R[q] = rec_set<M>(v[q]);
-                                    hb[q] = (M)1 << ((v[q].w >> 16) & 63u);
+                                    hb[q] = (M)1 << ((v[q].w >> (kOffBits + 3)) & 63u);
                                     pm[q] = pick_slot(rq, R[q] | hb[q]);
                                 }
 #pragma unroll
@@ -1229,7 +1233,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                                     const int nR = popc_m<M>(R[q]), rem = popc_m<M>(R[q] & ~hb[q]);
                                     if (live[q]) {
                                         sred_inc(cl + (unsigned)pick * 128u);
-                                        add_comm((v[q].w >> 13) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
+                                        add_comm((v[q].w >> kOffBits) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
                                     }
                                 }
                                 continue;
@@ -1249,7 +1253,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
                                     rk[q] = live[q] ? v[q].z : 0u;
                                     any |= rk[q];
                                     R[q] = rec_set<M>(v[q]);
-                                    hb[q] = (M)1 << ((v[q].w >> 16) & 63u);
+                                    hb[q] = (M)1 << ((v[q].w >> (kOffBits + 3)) & 63u);
                                 }
                                 while (any) {
                                     M pm[RF];
@@ -1275,7 +1279,7 @@ __global__ void __launch_bounds__(kChainThreads, MODE == kModeGrid ? 1 : 2) eval
 #pragma unroll
                                 for (int q = 0; q < RF; ++q) {
                                     const int nR = popc_m<M>(R[q]), rem = popc_m<M>(R[q] & ~hb[q]);
-                                    if (live[q]) add_comm((v[q].w >> 13) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
+                                    if (live[q]) add_comm((v[q].w >> kOffBits) & 7u, (unsigned)max(0, nR - 1), (unsigned)rem);
                                 }
                                 continue;
                             }
@@ -1676,6 +1680,24 @@ int launch_scan(EvalCall& c) {
     return TACG_OK;
 }
 
+// Tokens per scan item: the multiple of 512, at most kSlice, that gives the busiest CTA of the scan grid the least to do.
+// A CTA takes ceil(items / CTAs) items; an item costs its tokens plus a fixed part (barriers, row sums: about 400 tokens'
+// worth).  Large slices amortise the fixed part, small ones balance short traces.
+static long long pick_slice(const tacg_ctx* ctx, int L, long long nmb, long long B) {
+    const long long ctas = 2ll * ctx->sm_count;
+    long long best = 512, best_cost = -1;
+    for (long long sl = 512; sl <= kSlice; sl += 512) {
+        const long long spm = (B + sl - 1) / sl;
+        const long long items = (long long)L * nmb * spm;
+        const long long per = (items + std::min(items, ctas) - 1) / std::min(items, ctas);
+        // the last slice of a micro-batch may be short: count the slices a CTA takes at their real average length
+        const long long cost = per * (std::min(sl, (B + spm - 1) / spm) + 400);
+        if (best_cost < 0 || cost <= best_cost) { best = sl; best_cost = cost; }
+        if (sl >= B) break;
+    }
+    return best;
+}
+
 // How the chain kernel is launched for a geometry: cluster size (or CTAs per layer of a cooperative grid) and mode.
 void chain_plan(const tacg_ctx* ctx, const EvalGeom& g, int& mode, int& cs, int& groups) {
     // cluster size: as many CTAs per layer as the SM count allows, up to 16 (non-portable above 8)
@@ -1875,13 +1897,7 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
             }
             TACG_LAUNCH_CHECK(ctx);
         } else {
-        // slice: as large as the record format allows (the per-item epilogue is amortised over 16 tokens per
-        // thread); smaller only when the whole trace would otherwise give the scan grid fewer than two items per CTA
-        long long slice = kSlice;
-        if ((long long)L * N < (long long)kSlice * ctx->sm_count * 4)
-            slice = std::max(1ll, (long long)L * N / ((long long)ctx->sm_count * 4));
-        slice = std::min((long long)kSlice, std::min(g.B, slice));
-        slice = std::max(512ll, (slice + 511) / 512 * 512);
+        const long long slice = pick_slice(ctx, L, g.nmb, g.B);
         g.slice = (int)slice;
         g.spm = (int)((g.B + slice - 1) / slice);
         g.ipl = g.nmb * g.spm;
@@ -1962,7 +1978,7 @@ int tacg_launch_eval(tacg_ctx* ctx, const int16_t* indices, const int8_t* family
 // ---------------------------------------------------------------------------------------------------------------------
 namespace {
 
-constexpr size_t kNoAllocBytes = TACG_NOALLOC_SCRATCH_BYTES;     // 8 MiB: config 4 whole (58 x 512 items of 48 words) fits
+constexpr size_t kNoAllocBytes = TACG_NOALLOC_SCRATCH_BYTES;     // 8 MiB: config 4 whole (58 x 128 items of 48 words) fits many times
 static __device__ __align__(256) unsigned char g_noalloc_rows[kNoAllocBytes];
 
 constexpr int kMaxDevices = 64;
@@ -2031,11 +2047,7 @@ extern "C" int tacg_eval_primary_noalloc(tacg_ctx* ctx, const int16_t* indices, 
     g.B = N;
     g.nmb = 1;
     g.token_offset = token_offset;
-    long long slice = kSlice;
-    if ((long long)L * N < (long long)kSlice * ctx->sm_count * 4)
-        slice = std::max(1ll, (long long)L * N / ((long long)ctx->sm_count * 4));
-    slice = std::min((long long)kSlice, std::min(g.B, slice));
-    slice = std::max(512ll, (slice + 511) / 512 * 512);
+    const long long slice = pick_slice(ctx, L, g.nmb, g.B);
     g.slice = (int)slice;
     g.spm = (int)((g.B + slice - 1) / slice);
     g.ipl = g.nmb * g.spm;

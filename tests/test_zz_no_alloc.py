@@ -99,11 +99,10 @@ def test_no_alloc_entry_leaves_the_allocator_alone(tacg, ctx):
 
 
 def test_no_alloc_entry_refuses_what_does_not_fit(tacg, ctx):
-    # rows: L * ceil(N / 8192) * align4(P + 3F + 2) words.  P = 64, F = 8 -> 92 words; 64 layers x 512 slices = 12 MB
-    L, N, k, E, F, P = 64, 512 * 8192, 2, 64, 8, 64
-    assert L * (N // 8192) * 92 * 4 > tacg.NOALLOC_SCRATCH_BYTES
+    # rows: L * ceil(N / slice) * align4(P + 3F + 2) words, slice <= 32768.  P = 64, F = 8 -> 92 words; 256 layers x 128 slices
+    L, N, k, E, F, P = 256, 128 * 32768, 1, 64, 8, 64
+    assert L * (N // 32768) * 92 * 4 > tacg.NOALLOC_SCRATCH_BYTES
     idx = torch.zeros((L, N, k), dtype=torch.int16, device="cuda")
-    idx[:, :, 1] = 1
     fam = torch.zeros((N,), dtype=torch.int8, device="cuda")
     primary = torch.zeros((L, E), dtype=torch.int8, device="cuda")
     out = dict(load=torch.empty((L, P), dtype=torch.int64, device="cuda"),
