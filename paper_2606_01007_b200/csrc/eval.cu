@@ -1686,14 +1686,16 @@ int launch_scan(EvalCall& c) {
 static long long pick_slice(const tacg_ctx* ctx, int L, long long nmb, long long B) {
     const long long ctas = 2ll * ctx->sm_count;
     long long best = 512, best_cost = -1;
-    for (long long sl = 512; sl <= kSlice; sl += 512) {
-        const long long spm = (B + sl - 1) / sl;
-        const long long items = (long long)L * nmb * spm;
+    // by the number of slices per micro-batch: the slices of a micro-batch are made as even as multiples of 512 allow
+    for (long long spm = 1; spm <= (B + 511) / 512; ++spm) {
+        const long long sl = ((B + spm - 1) / spm + 511) / 512 * 512;
+        if (sl > kSlice) continue;
+        const long long real_spm = (B + sl - 1) / sl;
+        const long long items = (long long)L * nmb * real_spm;
         const long long per = (items + std::min(items, ctas) - 1) / std::min(items, ctas);
-        // the last slice of a micro-batch may be short: count the slices a CTA takes at their real average length
-        const long long cost = per * (std::min(sl, (B + spm - 1) / spm) + 400);
-        if (best_cost < 0 || cost <= best_cost) { best = sl; best_cost = cost; }
-        if (sl >= B) break;
+        const long long cost = per * ((B + real_spm - 1) / real_spm + 400);
+        if (best_cost < 0 || cost < best_cost) { best = sl; best_cost = cost; }
+        if (sl <= 512) break;
     }
     return best;
 }
