@@ -308,16 +308,24 @@ affinity_fused_kernel(AffArgs a) {
         if (i >= E) continue;
         const double* pi = ptab + (size_t)i * F;
         const int pa = pr[i] & 63;
+        // row i of the affinities sits in the warp's registers (lane p holds partitions p and p + 32): two of the four
+        // affinity reads of a pair become shuffles
+        const double arow0 = lane < P ? affl[(size_t)i * P + lane] : 0.0;
+        const double arow1 = lane + 32 < P ? affl[(size_t)i * P + lane + 32] : 0.0;
+        const double ai_pa = affl[(size_t)i * P + pa];
 #pragma unroll 4
-        for (int j = lane; j < E; j += 32) {
+        for (int jb = 0; jb < E; jb += 32) {         // warp-uniform trip count: the shuffles below are by the whole warp
+            const int j = min(jb + lane, E - 1);
             const int pb = pr[j] & 63;
             double g = 0.0;
             // (the entry is loaded for every pair, also the 1 in P inside one partition: no branch around the loads)
             const double w = w_entry(abar_entry(Cl, nf, F, E, i, j), iamax, pi, ptab + (size_t)j * F, F, a.alpha);
+            const double s0 = __shfl_sync(0xffffffffu, arow0, pb & 31), s1 = __shfl_sync(0xffffffffu, arow1, pb & 31);
+            const double ai_pb = pb < 32 ? s0 : s1;
             if (pa != pb) {
-                g = affl[(size_t)i * P + pb] + affl[(size_t)j * P + pa] - affl[(size_t)i * P + pa] - affl[(size_t)j * P + pb] - 2.0 * w;
+                g = ai_pb + affl[(size_t)j * P + pa] - ai_pa - affl[(size_t)j * P + pb] - 2.0 * w;
             }
-            a.gain_out[((size_t)l * E + i) * E + j] = (float)g;
+            if (jb + lane < E) a.gain_out[((size_t)l * E + i) * E + j] = (float)g;
         }
     }
 }
