@@ -1681,8 +1681,10 @@ int launch_scan(EvalCall& c) {
 }
 
 // Tokens per scan item: the multiple of 512, at most kSlice, that gives the busiest CTA of the scan grid the least to do.
-// A CTA takes ceil(items / CTAs) items; an item costs its tokens plus a fixed part (barriers, row sums: about 400 tokens'
-// worth).  Large slices amortise the fixed part, small ones balance short traces.
+// A CTA takes ceil(items / CTAs) items; an item costs its tokens plus a fixed part, set to 2000 tokens' worth by
+// measurement (the scan kernel's barriers and row sums, and what the chain kernel pays per slice: 400 gave three slices per
+// micro-batch at config 4 and 2.82 ms, 2000 and more give two and 2.76 ms).  Large slices amortise the fixed part, small
+// ones balance short traces.
 static long long pick_slice(const tacg_ctx* ctx, int L, long long nmb, long long B) {
     const long long ctas = 2ll * ctx->sm_count;
     long long best = 512, best_cost = -1;
@@ -1693,7 +1695,7 @@ static long long pick_slice(const tacg_ctx* ctx, int L, long long nmb, long long
         const long long real_spm = (B + sl - 1) / sl;
         const long long items = (long long)L * nmb * real_spm;
         const long long per = (items + std::min(items, ctas) - 1) / std::min(items, ctas);
-        const long long cost = per * ((B + real_spm - 1) / real_spm + 400);
+        const long long cost = per * ((B + real_spm - 1) / real_spm + 2000);
         if (best_cost < 0 || cost < best_cost) { best = sl; best_cost = cost; }
         if (sl <= 512) break;
     }
