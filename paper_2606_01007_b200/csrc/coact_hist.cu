@@ -9,7 +9,7 @@
 //                          kernels build once per call -- the labels are shared by all layers).  Four bank-spread copies of the bins when they fit; for
 //                          k = 8 a small token-set table short-cuts repeated expert sets.  The
 //                          histogram is written once per (CTA, layer) to a scratch slot.
-//   coact_finalize_kernel  grid (E/8, L*F), one warp per output row: sums the slots of the layer (L2
+//   coact_finalize_kernel  grid (E/4, L*F), one warp per output row: sums the slots of the layer (L2
 //                          resident), mirrors the triangle into the symmetric C, derives D, adds ntok.
 //                          With TACG_ZERO_FIRST it stores (diagonal cleared), otherwise it adds to what
 //                          is there (diagonal untouched).
@@ -478,12 +478,13 @@ __global__ void __launch_bounds__(kThreads, 1) coact_hist_kernel(const HistParam
     }
 }
 
-// One warp per output row: grid (ceil(E/8), L*F), 8 rows per CTA.  Each lane sums the slots' bins of its
-// (i,j) elements straight from scratch (L2 resident; the eight neighbouring rows of a CTA share the
+// One warp per output row: grid (ceil(E/4), L*F), 4 rows per CTA (small CTAs: the kernel waits on its loads, and
+// measured 4 rows beat 8 and 16).  Each lane sums the slots' bins of its
+// (i,j) elements straight from scratch (L2 resident; the four neighbouring rows of a CTA share the
 // sectors of the column part), writes the symmetric C row, and the warp reduces the row sum for D.
 // ZERO: overwrite instead of accumulate (the diagonal is then cleared with the rest).
 template <bool ZERO>
-__global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p, unsigned* __restrict__ D,
+__global__ void __launch_bounds__(128) coact_finalize_kernel(const HistParams p, unsigned* __restrict__ D,
                                                             unsigned* __restrict__ C,
                                                             unsigned long long* __restrict__ ntok) {
     tacg_pdl_prologue();
@@ -491,7 +492,7 @@ __global__ void __launch_bounds__(256) coact_finalize_kernel(const HistParams p,
     const int l = lf / p.F, f = lf % p.F;
     const int E = p.E, tri = p.tri;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int i = blockIdx.x * 8 + warp;
+    const int i = blockIdx.x * 4 + warp;
     const int fgi = p.nfg > 1 ? f : 0;                   // which CTA of a group holds family f
     const int fs = p.nfg > 1 ? 0 : f;                    // family index inside a slot
     __shared__ int g01[2];                               // first and last group that visited the layer
@@ -799,9 +800,9 @@ int tacg_launch_coact_hist(tacg_ctx* ctx, const int16_t* indices, const int8_t* 
                     : (copies ? launch_hist_k<false, 4>(ctx, p, smem, grid) : launch_hist_k<false, 1>(ctx, p, smem, grid));
     if (rc != TACG_OK) return rc;
     unsigned long long* nt = reinterpret_cast<unsigned long long*>(ntok);
-    const dim3 fgrid((E + 7) / 8, L * F);
-    if (zero_first) TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_finalize_kernel<true>, fgrid, dim3(256), 0, ctx->stream, p, D, C, nt));
-    else TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_finalize_kernel<false>, fgrid, dim3(256), 0, ctx->stream, p, D, C, nt));
+    const dim3 fgrid((E + 3) / 4, L * F);
+    if (zero_first) TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_finalize_kernel<true>, fgrid, dim3(128), 0, ctx->stream, p, D, C, nt));
+    else TACG_CUDA_TRY(ctx, tacg_launch_pdl(coact_finalize_kernel<false>, fgrid, dim3(128), 0, ctx->stream, p, D, C, nt));
     TACG_LAUNCH_CHECK(ctx);
     return TACG_OK;
 }
